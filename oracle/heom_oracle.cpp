@@ -1,0 +1,448 @@
+/*
+ * heom_oracle.cpp -- plain, slow, obviously-correct CPU ORACLE of the HEOM
+ * right-hand side (hierarchical Liouvillian) and the RK4 propagator of
+ * arXiv 1803.03498 (DM-HEOM), written from the paper's equations.
+ *
+ * TEST INFRASTRUCTURE, NOT THE PRODUCT (see heom_oracle.h).  No blocking, no
+ * fusion, no table or code shared with the CUDA path.  Everything is fp64.
+ *
+ * "P:n" = line n of /root/reference/PAPER.md.  "R*" = a reading listed in
+ * DESIGN.md section 3.
+ *
+ * Parity pins (tests/test_oracle_*.py, all -m "not gpu"):
+ *   tables        : Eq. 9 closed form incl. the paper's printed 12 271 512
+ *                    and the 3.3 GiB figure; link-count closed
+ *                   form; minus[plus[u][l]][l]==u; brute force for small W, D.
+ *   coefficients  : Mittag-Leffler series of cot (Delta_b -> 0+ as K -> inf).
+ *   commutator,
+ *   hbar, RK4     : lambda=0 -> closed-form two-level Rabi oscillation; dt^4.
+ *   +/- couplings,
+ *   V^x, V^o, c_0,
+ *   terminator    : pure-dephasing closed form (line-shape function g(t));
+ *                   trace and Hermiticity invariants; relaxation towards
+ *                   Boltzmann populations; independence of sigma_0 from the
+ *                   rescaling of Eq. 35-36; dense-Liouvillian expm comparison.
+ *   Parity unpinned: nothing in this file is without a pin, but configs 2-5 of
+ *   BASELINE.json have no printed values anywhere (the paper prints none);
+ *   they rest on the pins above evaluated at those shapes.
+ */
+#include "heom_oracle.h"
+
+#include <algorithm>
+#include <cmath>
+#include <complex>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+typedef std::complex<double> cplx;
+
+/* BASELINE.json config 1 fixes hbar; k_B is reading R3. */
+const double HBAR_CM_FS = 5308.8;      /* cm^-1 fs */
+const double KB_CM_PER_K = 0.6950348;  /* cm^-1 / K */
+const double PI = 3.14159265358979323846;
+
+}  // namespace
+
+struct oracle_ctx {
+  int N = 0;       /* sites = states = baths (per-site baths)          */
+  int K = 0;       /* Matsubara terms beyond the Drude pole                   */
+  int M = 0;       /* modes per bath = K+1 = the paper's K             */
+  int W = 0;       /* tuple length W = B*K_paper                        */
+  int D = 0;       /* truncation depth                                        */
+  int64_t nodes = 0;
+  int scaling = 1;
+  int terminator = 1;
+  int threads = 0;
+  std::vector<double> H;        /* [N][N] cm^-1                               */
+  std::vector<double> lambda;   /* [N] cm^-1                                  */
+  std::vector<double> nu;       /* [N] fs^-1                                  */
+  double beta_hbar = 0;         /* beta*hbar = hbar/(k_B T), fs               */
+  std::vector<double> gamma;    /* [W] Eq. 19, fs^-1                          */
+  std::vector<double> c_re;     /* [W] Re c(b,k)/hbar, Eq. 20, fs^-2          */
+  std::vector<double> c_im;     /* [W] Im part carried by Eq. 17's V^o term   */
+  std::vector<double> delta;    /* [N] Eq. 14 bracket, fs^-1                  */
+  std::vector<uint8_t> tuples;  /* [nodes][W]                                 */
+  std::vector<int32_t> plus;    /* [nodes][W]                                 */
+  std::vector<int32_t> minus;   /* [nodes][W]                                 */
+  std::vector<cplx> y;          /* state [nodes][N][N]                        */
+  bool have_state = false;
+};
+
+namespace {
+
+/* ---------------------------------------------------------------- index set
+ * all tuples n in N^W with sum <= D.  The paper leaves the linear
+ * numbering open; reading R1 pins it: level L = 0..D, and inside a
+ * level  for n_0 = L..0: for n_1 = (L-n_0)..0: ... ; n_{W-1} = remainder.   */
+void enumerate_level(int W, int pos, int remaining, std::vector<uint8_t>& cur,
+                     std::vector<uint8_t>& out) {
+  if (pos == W - 1) {
+    cur[pos] = (uint8_t)remaining;
+    out.insert(out.end(), cur.begin(), cur.end());
+    return;
+  }
+  for (int v = remaining; v >= 0; --v) {
+    cur[pos] = (uint8_t)v;
+    enumerate_level(W, pos + 1, remaining - v, cur, out);
+  }
+}
+
+int level_of(const uint8_t* t, int W) {
+  int s = 0;
+  for (int l = 0; l < W; ++l) s += t[l];
+  return s;
+}
+
+/* Ordering predicate of the enumeration above: lower level first; inside a
+ * level the tuple that is lexicographically LARGER comes first. */
+bool comes_before(const uint8_t* a, const uint8_t* b, int W) {
+  int la = level_of(a, W), lb = level_of(b, W);
+  if (la != lb) return la < lb;
+  for (int l = 0; l < W; ++l)
+    if (a[l] != b[l]) return a[l] > b[l];
+  return false;
+}
+
+/* Look a tuple up in the enumerated list by bisection (the list is sorted by
+ * comes_before by construction).  Returns -1 if absent. */
+int64_t find_tuple(const std::vector<uint8_t>& tuples, int64_t nodes, int W,
+                   const uint8_t* key) {
+  int64_t lo = 0, hi = nodes;
+  while (lo < hi) {
+    int64_t mid = lo + (hi - lo) / 2;
+    if (comes_before(&tuples[(size_t)mid * W], key, W)) lo = mid + 1;
+    else hi = mid;
+  }
+  if (lo < nodes && std::memcmp(&tuples[(size_t)lo * W], key, (size_t)W) == 0) return lo;
+  return -1;
+}
+
+int nthreads(const oracle_ctx* c) {
+#ifdef _OPENMP
+  return c->threads > 0 ? c->threads : omp_get_max_threads();
+#else
+  (void)c;
+  return 1;
+#endif
+}
+
+/* "+" link valid iff sum(n + e_l) <= D; "-" link valid iff n_l - 1 >= 0. */
+void build_links(oracle_ctx* c) {
+  const int W = c->W;
+  c->plus.assign((size_t)c->nodes * W, -1);
+  c->minus.assign((size_t)c->nodes * W, -1);
+#pragma omp parallel for schedule(static) num_threads(nthreads(c))
+  for (int64_t u = 0; u < c->nodes; ++u) {
+    std::vector<uint8_t> t(&c->tuples[(size_t)u * W], &c->tuples[(size_t)u * W] + W);
+    const int L = level_of(t.data(), W);
+    for (int l = 0; l < W; ++l) {
+      if (L + 1 <= c->D) {
+        t[l] += 1;
+        c->plus[(size_t)u * W + l] = (int32_t)find_tuple(c->tuples, c->nodes, W, t.data());
+        t[l] -= 1;
+      }
+      if (t[l] >= 1) {
+        t[l] -= 1;
+        c->minus[(size_t)u * W + l] = (int32_t)find_tuple(c->tuples, c->nodes, W, t.data());
+        t[l] += 1;
+      }
+    }
+  }
+}
+
+/* -------------------------------------------------------------- coefficients
+ * P:121 Eq. 19, Eq. 20, Eq. 14 bracket.  Mode index (0-based)
+ * l = b*M + k (Eq. 10 rewritten 0-based), k = 0 the Drude pole.
+ * Reading R2: every c of Eq. 16-17 and 35-36 enters as c-hat = c/hbar so that
+ * all terms of the RHS are rates.                                            */
+int build_coefficients(oracle_ctx* c, double T_kelvin) {
+  const int N = c->N, M = c->M;
+  c->beta_hbar = HBAR_CM_FS / (KB_CM_PER_K * T_kelvin);
+  c->gamma.assign((size_t)c->W, 0.0);
+  c->c_re.assign((size_t)c->W, 0.0);
+  c->c_im.assign((size_t)c->W, 0.0);
+  c->delta.assign((size_t)N, 0.0);
+  for (int b = 0; b < N; ++b) {
+    const double lam = c->lambda[b] / HBAR_CM_FS; /* lambda_b / hbar, fs^-1 */
+    const double nu = c->nu[b];
+    for (int k = 0; k < M; ++k) {
+      const int l = b * M + k;
+      if (k == 0) {
+        c->gamma[l] = nu;                                           /* Eq. 19 */
+        const double x = c->beta_hbar * nu / 2.0;
+        const double t = std::tan(x);
+        if (lam != 0.0 && (t == 0.0 || !std::isfinite(1.0 / t))) return -1;
+        c->c_re[l] = (lam == 0.0) ? 0.0 : nu * lam / t;             /* Eq. 20 */
+        c->c_im[l] = -lam * nu;           /* the V^o term of Eq. 17 (R4)     */
+      } else {
+        const double g = 2.0 * PI * k / c->beta_hbar;               /* Eq. 19 */
+        c->gamma[l] = g;
+        if (lam != 0.0 && g * g - nu * nu == 0.0) return -1;
+        c->c_re[l] = (lam == 0.0) ? 0.0
+                     : 4.0 * lam * nu / c->beta_hbar * g / (g * g - nu * nu); /* Eq. 20 */
+      }
+    }
+    /* Eq. 14:  2 lambda_b/(beta hbar^2 nu_b) - sum_k c(b,k)/(hbar gamma(b,k)) */
+    double d = 2.0 * lam / (c->beta_hbar * nu);
+    for (int k = 0; k < M; ++k) d -= c->c_re[b * M + k] / c->gamma[b * M + k];
+    c->delta[b] = d;
+  }
+  return 0;
+}
+
+/* ------------------------------------------------------- site superoperators
+ * P:136-140 Eq. 23-25 (Eq. 23's printed left subscript "ii" read as "ij").   */
+inline double Vx(int s, int i, int j) { return (double)(i == s) - (double)(s == j); }
+inline double VxVx(int s, int i, int j) {
+  return (double)(i != j) * ((double)(i == s) + (double)(s == j));
+}
+inline double Vo(int s, int i, int j) { return (double)(i == s) + (double)(s == j); }
+
+/* |c(b,k)| of Eq. 35-36 under the chosen reading (R5). */
+inline double abs_c(const oracle_ctx* c, int l) {
+  if (c->scaling == 2) return std::sqrt(c->c_re[l] * c->c_re[l] + c->c_im[l] * c->c_im[l]);
+  return std::fabs(c->c_re[l]);
+}
+
+/* ------------------------------------------------------------ right-hand side
+ * d sigma_u / dt, Eq. 12-17, for one node u of the state `st`.               */
+void rhs_node(const oracle_ctx* c, const cplx* st, int64_t u, cplx* out) {
+  const int N = c->N, M = c->M, W = c->W;
+  const size_t NN = (size_t)N * N;
+  const cplx I(0.0, 1.0);
+  const cplx* s = st + (size_t)u * NN;
+  const uint8_t* n = &c->tuples[(size_t)u * W];
+
+  /* Eq. 12:  -(i/hbar) [H, sigma_u] */
+  for (int i = 0; i < N; ++i)
+    for (int j = 0; j < N; ++j) {
+      cplx comm(0.0, 0.0);
+      for (int m = 0; m < N; ++m)
+        comm += c->H[(size_t)i * N + m] * s[(size_t)m * N + j] -
+                s[(size_t)i * N + m] * c->H[(size_t)m * N + j];
+      out[(size_t)i * N + j] = -(I / HBAR_CM_FS) * comm;
+    }
+
+  /* Eq. 13:  - sigma_u sum_{b,k} n_{u,(b,k)} gamma(b,k) */
+  double damp = 0.0;
+  for (int l = 0; l < W; ++l) damp += (double)n[l] * c->gamma[l];
+  for (size_t e = 0; e < NN; ++e) out[e] -= damp * s[e];
+
+  /* Eq. 14:  - sum_b [ ... ] V_b^x V_b^x sigma_u   (S(b)=1, bs(b)=b) */
+  if (c->terminator)
+    for (int b = 0; b < N; ++b)
+      for (int i = 0; i < N; ++i)
+        for (int j = 0; j < N; ++j)
+          out[(size_t)i * N + j] -= c->delta[b] * VxVx(b, i, j) * s[(size_t)i * N + j];
+
+  /* Eq. 15 -> Eq. 35:  + sum_{b,k} i sqrt((n+1)|c|) V_b^x sigma^+_{(u,b,k)} */
+  for (int l = 0; l < W; ++l) {
+    const int32_t up = c->plus[(size_t)u * W + l];
+    if (up < 0) continue; /* invalid link contributes nothing */
+    const int b = l / M;  /* Eq. 11 */
+    const cplx* sp = st + (size_t)up * NN;
+    const double f = c->scaling ? std::sqrt(((double)n[l] + 1.0) * abs_c(c, l)) : 1.0;
+    for (int i = 0; i < N; ++i)
+      for (int j = 0; j < N; ++j)
+        out[(size_t)i * N + j] += I * (f * Vx(b, i, j)) * sp[(size_t)i * N + j];
+  }
+
+  /* Eq. 16-17 -> Eq. 36:  + sum_{b,k} sqrt(n/|c|) theta_MA(b,k) sigma^-_{(u,b,k)},
+   * theta_MA = i c V^x + delta_{k,0} (lambda_b nu_b / hbar) V^o.
+   * Unscaled (Eq. 16) the prefactor is n.  |c| = 0 (lambda_b = 0): the bath is
+   * decoupled and the term is dropped (limit of the printed 0/0). */
+  for (int l = 0; l < W; ++l) {
+    const int32_t um = c->minus[(size_t)u * W + l];
+    if (um < 0) continue;
+    const int b = l / M, k = l % M;
+    const cplx* sm = st + (size_t)um * NN;
+    double f;
+    if (c->scaling) {
+      const double a = abs_c(c, l);
+      f = (a > 0.0) ? std::sqrt((double)n[l] / a) : 0.0;
+    } else {
+      f = (double)n[l];
+    }
+    const double lam_nu = (k == 0) ? -c->c_im[l] : 0.0; /* lambda_b nu_b / hbar */
+    for (int i = 0; i < N; ++i)
+      for (int j = 0; j < N; ++j) {
+        const cplx theta = I * (c->c_re[l] * Vx(b, i, j)) + lam_nu * Vo(b, i, j);
+        out[(size_t)i * N + j] += f * theta * sm[(size_t)i * N + j];
+      }
+  }
+}
+
+void rhs_all(const oracle_ctx* c, const cplx* st, cplx* out) {
+  const size_t NN = (size_t)c->N * c->N;
+#pragma omp parallel for schedule(static) num_threads(nthreads(c))
+  for (int64_t u = 0; u < c->nodes; ++u) rhs_node(c, st, u, out + (size_t)u * NN);
+}
+
+}  // namespace
+
+extern "C" {
+
+int oracle_create(oracle_ctx** out, int n_sites, const double* H_cm, const double* lambda_cm,
+                  const double* nu_per_fs, double T_kelvin, int K, int D) {
+  if (!out || !H_cm || !lambda_cm || !nu_per_fs) return -1;
+  if (n_sites < 1 || K < 0 || D < 0 || D > 255 || !(T_kelvin > 0.0)) return -1;
+  for (int i = 0; i < n_sites; ++i) {
+    if (!(lambda_cm[i] >= 0.0) || !(nu_per_fs[i] > 0.0)) return -1;
+    for (int j = 0; j < n_sites; ++j) {
+      if (!std::isfinite(H_cm[i * n_sites + j])) return -1;
+      if (H_cm[i * n_sites + j] != H_cm[j * n_sites + i]) return -1;
+    }
+  }
+  oracle_ctx* c = new (std::nothrow) oracle_ctx();
+  if (!c) return -2;
+  try {
+    c->N = n_sites; c->K = K; c->M = K + 1; c->W = n_sites * (K + 1); c->D = D;
+    c->H.assign(H_cm, H_cm + (size_t)n_sites * n_sites);
+    c->lambda.assign(lambda_cm, lambda_cm + n_sites);
+    c->nu.assign(nu_per_fs, nu_per_fs + n_sites);
+    if (build_coefficients(c, T_kelvin) != 0) { delete c; return -1; }
+    std::vector<uint8_t> cur((size_t)c->W, 0);
+    for (int L = 0; L <= D; ++L) enumerate_level(c->W, 0, L, cur, c->tuples);
+    c->nodes = (int64_t)(c->tuples.size() / (size_t)c->W);
+    if (c->nodes > 2147483647LL) { delete c; return -1; }
+    build_links(c);
+  } catch (const std::bad_alloc&) {
+    delete c;
+    return -2;
+  }
+  *out = c;
+  return 0;
+}
+
+void oracle_destroy(oracle_ctx* c) { delete c; }
+
+int oracle_set_option(oracle_ctx* c, const char* name, int value) {
+  if (!c || !name) return -1;
+  const std::string s(name);
+  if (s == "scaling") { if (value < 0 || value > 2) return -1; c->scaling = value; return 0; }
+  if (s == "terminator") { c->terminator = value ? 1 : 0; return 0; }
+  if (s == "threads") { if (value < 0) return -1; c->threads = value; return 0; }
+  return -1;
+}
+
+int64_t oracle_num_nodes(const oracle_ctx* c) { return c ? c->nodes : -1; }
+int oracle_num_modes(const oracle_ctx* c) { return c ? c->W : -1; }
+int oracle_num_threads(const oracle_ctx* c) { return c ? nthreads(c) : -1; }
+
+int oracle_get_tables(const oracle_ctx* c, uint8_t* tuples, int32_t* plus, int32_t* minus) {
+  if (!c) return -1;
+  if (tuples) std::memcpy(tuples, c->tuples.data(), c->tuples.size());
+  if (plus) std::memcpy(plus, c->plus.data(), c->plus.size() * sizeof(int32_t));
+  if (minus) std::memcpy(minus, c->minus.data(), c->minus.size() * sizeof(int32_t));
+  return 0;
+}
+
+int oracle_get_coefficients(const oracle_ctx* c, double* gamma, double* c_re, double* c_im,
+                            double* delta) {
+  if (!c) return -1;
+  if (gamma) std::memcpy(gamma, c->gamma.data(), c->gamma.size() * sizeof(double));
+  if (c_re) std::memcpy(c_re, c->c_re.data(), c->c_re.size() * sizeof(double));
+  if (c_im) std::memcpy(c_im, c->c_im.data(), c->c_im.size() * sizeof(double));
+  if (delta) std::memcpy(delta, c->delta.data(), c->delta.size() * sizeof(double));
+  return 0;
+}
+
+int oracle_set_state(oracle_ctx* c, const double* sigma0) {
+  if (!c || !sigma0) return -1;
+  const size_t NN = (size_t)c->N * c->N;
+  try { c->y.assign((size_t)c->nodes * NN, cplx(0.0, 0.0)); }
+  catch (const std::bad_alloc&) { return -2; }
+  for (size_t e = 0; e < NN; ++e) c->y[e] = cplx(sigma0[2 * e], sigma0[2 * e + 1]);
+  c->have_state = true;
+  return 0;
+}
+
+int oracle_set_full_state(oracle_ctx* c, const double* sigma) {
+  if (!c || !sigma) return -1;
+  const size_t total = (size_t)c->nodes * c->N * c->N;
+  try { c->y.resize(total); } catch (const std::bad_alloc&) { return -2; }
+  for (size_t e = 0; e < total; ++e) c->y[e] = cplx(sigma[2 * e], sigma[2 * e + 1]);
+  c->have_state = true;
+  return 0;
+}
+
+int oracle_get_full_state(const oracle_ctx* c, double* sigma) {
+  if (!c || !sigma) return -1;
+  if (!c->have_state) return -4;
+  for (size_t e = 0; e < c->y.size(); ++e) { sigma[2 * e] = c->y[e].real(); sigma[2 * e + 1] = c->y[e].imag(); }
+  return 0;
+}
+
+int oracle_rhs(oracle_ctx* c, double* dsigma) {
+  if (!c || !dsigma) return -1;
+  if (!c->have_state) return -4;
+  rhs_all(c, c->y.data(), reinterpret_cast<cplx*>(dsigma));
+  return 0;
+}
+
+int oracle_rhs_nodes(oracle_ctx* c, const int64_t* ids, int64_t count, double* out) {
+  if (!c || !ids || !out || count < 0) return -1;
+  if (!c->have_state) return -4;
+  const size_t NN = (size_t)c->N * c->N;
+  for (int64_t q = 0; q < count; ++q)
+    if (ids[q] < 0 || ids[q] >= c->nodes) return -1;
+#pragma omp parallel for schedule(static) num_threads(nthreads(c))
+  for (int64_t q = 0; q < count; ++q)
+    rhs_node(c, c->y.data(), ids[q], reinterpret_cast<cplx*>(out) + (size_t)q * NN);
+  return 0;
+}
+
+/* Classical fourth-order Runge-Kutta ("Runge-Kutta integration", P:503
+ * "4 intermediate results", "4 copies of the ADOs"; reading R6):
+ *   k1 = f(y); k2 = f(y + dt/2 k1); k3 = f(y + dt/2 k2); k4 = f(y + dt k3);
+ *   y <- y + dt/6 (k1 + 2 k2 + 2 k3 + k4).
+ * Four state-sized arrays (y, stage input, k, running sum), like the paper. */
+int oracle_rk4_steps(oracle_ctx* c, double dt, int nsteps) {
+  if (!c || nsteps < 0 || !std::isfinite(dt)) return -1;
+  if (!c->have_state) return -4;
+  const size_t total = c->y.size();
+  std::vector<cplx> x, k, sum;
+  try { x.resize(total); k.resize(total); sum.resize(total); }
+  catch (const std::bad_alloc&) { return -2; }
+  cplx* y = c->y.data();
+  const int nt = nthreads(c);
+  for (int step = 0; step < nsteps; ++step) {
+    rhs_all(c, y, k.data());                                   /* k1 */
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (size_t e = 0; e < total; ++e) { sum[e] = k[e]; x[e] = y[e] + (dt / 2.0) * k[e]; }
+    rhs_all(c, x.data(), k.data());                            /* k2 */
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (size_t e = 0; e < total; ++e) { sum[e] += 2.0 * k[e]; x[e] = y[e] + (dt / 2.0) * k[e]; }
+    rhs_all(c, x.data(), k.data());                            /* k3 */
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (size_t e = 0; e < total; ++e) { sum[e] += 2.0 * k[e]; x[e] = y[e] + dt * k[e]; }
+    rhs_all(c, x.data(), k.data());                            /* k4 */
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (size_t e = 0; e < total; ++e) { sum[e] += k[e]; y[e] += (dt / 6.0) * sum[e]; }
+  }
+  return 0;
+}
+
+/* P:144 Eq. 26: rho = sigma_0. */
+int oracle_populations(const oracle_ctx* c, double* pop, double* tr_re, double* tr_im) {
+  if (!c) return -1;
+  if (!c->have_state) return -4;
+  cplx tr(0.0, 0.0);
+  for (int i = 0; i < c->N; ++i) {
+    const cplx d = c->y[(size_t)i * c->N + i];
+    if (pop) pop[i] = d.real();
+    tr += d;
+  }
+  if (tr_re) *tr_re = tr.real();
+  if (tr_im) *tr_im = tr.imag();
+  return 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,141 @@
+"""ctypes binding of the CPU oracle (oracle/libheom_oracle.so).
+
+TEST INFRASTRUCTURE: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this module.  It imports
+nothing from the CUDA package.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build_oracle
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = build_oracle.build()
+    lib = C.CDLL(path)
+    P = C.c_void_p
+    dp = C.POINTER(C.c_double)
+    lib.oracle_create.argtypes = [C.POINTER(P), C.c_int, dp, dp, dp, C.c_double, C.c_int, C.c_int]
+    lib.oracle_create.restype = C.c_int
+    lib.oracle_destroy.argtypes = [P]
+    lib.oracle_destroy.restype = None
+    lib.oracle_set_option.argtypes = [P, C.c_char_p, C.c_int]
+    lib.oracle_num_nodes.argtypes = [P]
+    lib.oracle_num_nodes.restype = C.c_int64
+    lib.oracle_num_modes.argtypes = [P]
+    lib.oracle_num_threads.argtypes = [P]
+    lib.oracle_get_tables.argtypes = [P, P, P, P]
+    lib.oracle_get_coefficients.argtypes = [P, P, P, P, P]
+    lib.oracle_set_state.argtypes = [P, P]
+    lib.oracle_set_full_state.argtypes = [P, P]
+    lib.oracle_get_full_state.argtypes = [P, P]
+    lib.oracle_rhs.argtypes = [P, P]
+    lib.oracle_rhs_nodes.argtypes = [P, P, C.c_int64, P]
+    lib.oracle_rk4_steps.argtypes = [P, C.c_double, C.c_int]
+    lib.oracle_populations.argtypes = [P, P, P, P]
+    _lib = lib
+    return lib
+
+
+def _dptr(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+class Oracle:
+    """One truncated hierarchy on the CPU.  Arguments as heom_oracle.h."""
+
+    def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, scaling=1, terminator=1,
+                 threads=0):
+        lib = _load()
+        H = np.ascontiguousarray(H_cm, dtype=np.float64)
+        self.N = H.shape[0]
+        lam = np.ascontiguousarray(np.broadcast_to(lambda_cm, (self.N,)), dtype=np.float64)
+        nu = np.ascontiguousarray(np.broadcast_to(nu_per_fs, (self.N,)), dtype=np.float64)
+        h = C.c_void_p()
+        rc = lib.oracle_create(C.byref(h), self.N, _dptr(H), _dptr(lam), _dptr(nu),
+                               float(T_kelvin), int(K), int(D))
+        if rc != 0:
+            raise ValueError(f"oracle_create failed with status {rc}")
+        self._h = h
+        self._lib = lib
+        self.K, self.D = int(K), int(D)
+        self.nodes = int(lib.oracle_num_nodes(h))
+        self.W = int(lib.oracle_num_modes(h))
+        for name, v in (("scaling", scaling), ("terminator", terminator), ("threads", threads)):
+            self._ck(lib.oracle_set_option(h, name.encode(), int(v)))
+
+    def _ck(self, rc):
+        if rc != 0:
+            raise RuntimeError(f"oracle call failed with status {rc}")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.oracle_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        self.close()
+
+    @property
+    def threads(self):
+        return int(self._lib.oracle_num_threads(self._h))
+
+    def tables(self):
+        t = np.empty((self.nodes, self.W), dtype=np.uint8)
+        p = np.empty((self.nodes, self.W), dtype=np.int32)
+        m = np.empty((self.nodes, self.W), dtype=np.int32)
+        self._ck(self._lib.oracle_get_tables(self._h, t.ctypes.data, p.ctypes.data, m.ctypes.data))
+        return t, p, m
+
+    def coefficients(self):
+        g = np.empty(self.W); cr = np.empty(self.W); ci = np.empty(self.W); d = np.empty(self.N)
+        self._ck(self._lib.oracle_get_coefficients(self._h, g.ctypes.data, cr.ctypes.data,
+                                                   ci.ctypes.data, d.ctypes.data))
+        return g, cr, ci, d
+
+    def set_state(self, sigma0):
+        s = np.ascontiguousarray(sigma0, dtype=np.complex128)
+        assert s.shape == (self.N, self.N)
+        self._ck(self._lib.oracle_set_state(self._h, s.ctypes.data))
+
+    def set_full_state(self, sigma):
+        s = np.ascontiguousarray(sigma, dtype=np.complex128)
+        assert s.shape == (self.nodes, self.N, self.N)
+        self._ck(self._lib.oracle_set_full_state(self._h, s.ctypes.data))
+
+    def get_full_state(self):
+        out = np.empty((self.nodes, self.N, self.N), dtype=np.complex128)
+        self._ck(self._lib.oracle_get_full_state(self._h, out.ctypes.data))
+        return out
+
+    def rhs(self):
+        out = np.empty((self.nodes, self.N, self.N), dtype=np.complex128)
+        self._ck(self._lib.oracle_rhs(self._h, out.ctypes.data))
+        return out
+
+    def rhs_nodes(self, ids):
+        ids = np.ascontiguousarray(ids, dtype=np.int64)
+        out = np.empty((ids.size, self.N, self.N), dtype=np.complex128)
+        self._ck(self._lib.oracle_rhs_nodes(self._h, ids.ctypes.data, ids.size, out.ctypes.data))
+        return out
+
+    def rk4_steps(self, dt_fs, nsteps):
+        self._ck(self._lib.oracle_rk4_steps(self._h, float(dt_fs), int(nsteps)))
+
+    def populations(self):
+        pop = np.empty(self.N)
+        tr = C.c_double(), C.c_double()
+        self._ck(self._lib.oracle_populations(self._h, pop.ctypes.data, C.byref(tr[0]),
+                                              C.byref(tr[1])))
+        return pop, complex(tr[0].value, tr[1].value)
+
+    def sigma0(self):
+        """rho = sigma_0 (Eq. 26) as an N x N array (reads the full state; small cases)."""
+        return self.get_full_state()[0]

@@ -1,0 +1,148 @@
+"""Seeded synthetic inputs shaped like the paper's light-harvesting complexes.
+
+This module serves BOTH the CPU oracle (tests, cpu_baseline) and the CUDA path
+(tests, bench.py).  It holds none of the method's arithmetic: it only draws
+Hamiltonians, bath parameters, initial matrices and random test states.  It
+imports neither `oracle` nor `paper_1803_03498_b200`.
+
+The five configurations are BASELINE.json's `configs[0..4]`, stand-ins for the
+paper's FMO workloads (Eq. 78: 7 sites, couplings 1-100 cm^-1, energy
+spread ~400 cm^-1; Table 1: lambda = 35 cm^-1, 1/nu = 50 fs, Omega = 0;
+P:443: T = 30..300 K; "more than 100 states" for supercomplexes).
+Generator recipe: numpy PCG64 `default_rng(seed)`, draws in the
+order written below, upper triangle row-major, then symmetrised.
+"""
+from dataclasses import dataclass, replace
+from math import comb
+
+import numpy as np
+
+SEED_FMO = 1803034982      # configs 2 and 3 share one H (BASELINE.json)
+SEED_LHCII = 1803034983
+SEED_LARGE = 1803034984
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    H_cm: np.ndarray          # [N][N] real symmetric, cm^-1
+    lambda_cm: float          # reorganisation energy of every site's bath
+    inv_nu_fs: float          # bath correlation time 1/nu_b, fs
+    T_kelvin: float
+    K: int                    # Matsubara terms beyond the Drude pole
+    D: int                    # truncation depth
+    dt_fs: float
+    steps: int
+
+    @property
+    def N(self):
+        return self.H_cm.shape[0]
+
+    @property
+    def W(self):
+        return self.N * (self.K + 1)
+
+    @property
+    def nodes(self):
+        return comb(self.W + self.D, self.D)
+
+    @property
+    def nu_per_fs(self):
+        return 1.0 / self.inv_nu_fs
+
+    @property
+    def state_bytes(self):
+        return 16 * self.N * self.N * self.nodes
+
+    def with_(self, **kw):
+        return replace(self, **kw)
+
+    def sigma0(self):
+        """sigma_0(0) = |1><1| (BASELINE.json: all configs)."""
+        s = np.zeros((self.N, self.N), dtype=np.complex128)
+        s[0, 0] = 1.0
+        return s
+
+
+def _symmetric_from_upper(N, diag, upper):
+    H = np.zeros((N, N))
+    iu = np.triu_indices(N, k=1)
+    H[iu] = upper
+    H = H + H.T
+    H[np.diag_indices(N)] = diag
+    return H
+
+
+def dimer():
+    H = np.array([[100.0, 100.0], [100.0, 0.0]])
+    return Workload("cfg1_dimer", H, 35.0, 50.0, 300.0, 1, 4, 1.0, 1000)
+
+
+def _fmo_like_H():
+    rng = np.random.default_rng(SEED_FMO)
+    eps = rng.uniform(0.0, 500.0, size=7)
+    J = rng.normal(0.0, 40.0, size=7 * 6 // 2)
+    return _symmetric_from_upper(7, eps, J)
+
+
+def fmo_like():
+    return Workload("cfg2_fmo7", _fmo_like_H(), 35.0, 50.0, 77.0, 1, 8, 1.0, 1000)
+
+
+def deep():
+    return Workload("cfg3_deep7", _fmo_like_H(), 35.0, 50.0, 300.0, 1, 12, 1.0, 200)
+
+
+def lhcii_like():
+    N = 14
+    rng = np.random.default_rng(SEED_LHCII)
+    eps = rng.uniform(0.0, 600.0, size=N)
+    sign = rng.choice([-1.0, 1.0], size=N * (N - 1) // 2)
+    iu = np.triu_indices(N, k=1)
+    J = 80.0 * np.exp(-np.abs(iu[0] - iu[1]) / 3.0) * sign
+    return Workload("cfg4_lhcii14", _symmetric_from_upper(N, eps, J), 37.0, 40.0, 300.0, 0, 8,
+                    0.5, 500)
+
+
+def large():
+    N = 96
+    rng = np.random.default_rng(SEED_LARGE)
+    eps = rng.uniform(0.0, 800.0, size=N)
+    pos = rng.uniform(0.0, 6.0, size=(N, 3))
+    iu = np.triu_indices(N, k=1)
+    d = np.linalg.norm(pos[iu[0]] - pos[iu[1]], axis=1)
+    J = 300.0 / (1.0 + d ** 3)
+    return Workload("cfg5_large96", _symmetric_from_upper(N, eps, J), 35.0, 50.0, 300.0, 0, 3,
+                    0.5, 50)
+
+
+CONFIGS = {
+    "cfg1": dimer, "cfg2": fmo_like, "cfg3": deep, "cfg4": lhcii_like, "cfg5": large,
+}
+
+
+def get(name):
+    return CONFIGS[name]()
+
+
+def random_state(nodes, N, seed, hermitian=False):
+    """A dense seeded test state [nodes][N][N] complex128 with O(1) entries
+    (for single-RHS parity, where every term of the equation must be exercised)."""
+    rng = np.random.default_rng(seed)
+    out = np.empty((nodes, N, N), dtype=np.complex128)
+    chunk = max(1, (1 << 22) // (N * N))
+    for a in range(0, nodes, chunk):
+        b = min(nodes, a + chunk)
+        blk = rng.standard_normal((b - a, N, N)) + 1j * rng.standard_normal((b - a, N, N))
+        if hermitian:
+            blk = 0.5 * (blk + np.conj(np.swapaxes(blk, 1, 2)))
+        out[a:b] = blk
+    return out
+
+
+def random_density(N, seed):
+    """A seeded random density matrix (Hermitian, positive, trace 1)."""
+    rng = np.random.default_rng(seed)
+    A = rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
+    rho = A @ A.conj().T
+    return rho / np.trace(rho).real
