@@ -1,0 +1,129 @@
+/*
+ * heom.h -- C ABI of the B200-native HEOM right-hand side + RK4 propagator.
+ *
+ * The hot path of DM-HEOM (arXiv 1803.03498): the hierarchical Liouvillian
+ * (Eq. 12-17 with the site superoperators Eq. 23-25 and the ADO rescaling
+ * Eq. 35-36) applied to every auxiliary density matrix sigma_n of a
+ * depth-truncated hierarchy (Eq. 9), inside a fixed-step classical RK4
+ * propagator whose stage combinations are fused into the
+ * right-hand-side kernel.  "P:n" = line n of the paper text PAPER.md; "R*" = a
+ * reading of the paper listed in DESIGN.md section 3.
+ *
+ * Plain C: opaque handle, plain pointers, sizes.  No torch types.  Every
+ * pointer argument says HOST or DEVICE.  Errors are integer statuses; nothing
+ * throws or aborts.  There is NO CPU fallback: without a CUDA device every
+ * compute entry point returns HEOM_ECUDA.
+ *
+ * Units: energies cm^-1, time fs, hbar = 5308.8 cm^-1 fs (BASELINE.json),
+ * k_B = 0.6950348 cm^-1/K (R3).  Matrices row-major; complex numbers are
+ * interleaved (re, im) doubles ("complex128").
+ *
+ * Node order of every HOST-visible table or state: the PINNED order (R1):
+ * level-major (L = sum n = 0..D), inside a level descending lexicographic on
+ * (n_0..n_{W-1}).  The device-side storage order is internal.
+ *
+ * Threading: one context per stream; calls on one context are not re-entrant.
+ */
+#ifndef HEOM_H
+#define HEOM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct heom_ctx heom_ctx; /* opaque; owns host tables, coefficients, H copy */
+
+typedef enum {
+  HEOM_OK = 0,
+  HEOM_EINVAL = -1, /* bad argument (NULL, NaN, non-symmetric H, singular coefficient) */
+  HEOM_ENOMEM = -2, /* host allocation failed or workspace too small                   */
+  HEOM_ECUDA = -3,  /* CUDA error or no device; heom_last_error() has the text         */
+  HEOM_ESTATE = -4  /* call order: no workspace bound / no state set                   */
+} heom_status;
+
+/* Build the hierarchy (index set Eq. 9, +/- link graph P:90, mode map Eq. 10-11)
+ * and the coefficients (Eq. 14, 19, 20, 35, 36) on the host.  No CUDA call.
+ *   H_cm        HOST  n_sites*n_sites doubles, real symmetric (checked exactly), cm^-1
+ *   lambda_cm   HOST  [n_sites] reorganisation energies >= 0 of the per-site
+ *                     Drude-Lorentz baths (Eq. 6 with Omega = 0; S(b)=1, bs(b)=b)
+ *   nu_per_fs   HOST  [n_sites] Drude rates nu_b > 0 in fs^-1 (BASELINE's "gamma")
+ *   T_kelvin    > 0
+ *   K           >= 0 Matsubara terms beyond the Drude pole: modes per bath M = K+1
+ *               (= the paper's "K"); tuple length W = n_sites*M
+ *   D           >= 0 truncation depth (sum n <= D)
+ *   device      CUDA ordinal used by heom_bind_workspace
+ * The caller keeps ownership of all input arrays (they are copied). */
+heom_status heom_create(heom_ctx** out, int n_sites, const double* H_cm,
+                        const double* lambda_cm, const double* nu_per_fs,
+                        double T_kelvin, int K, int D, int device);
+void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
+
+/* Options, to be set before heom_bind_workspace:
+ *   "order"   device storage order of the nodes: 0 = pinned order, 1 = plain
+ *             lexicographic (default 1)
+ *   "kernel"  0 = generic element-per-thread kernel, 1 = auto (specialised
+ *             kernels where available; default)
+ *   "timing"  1 = bracket every RHS launch with CUDA events (heom_kernel_time) */
+heom_status heom_set_option(heom_ctx* ctx, const char* name, int value);
+
+int64_t heom_num_nodes(const heom_ctx* ctx); /* Eq. 9: C(W+D, D) */
+int heom_num_modes(const heom_ctx* ctx);     /* W = n_sites*(K+1) */
+
+/* Copies the host tables in the PINNED order.  Any pointer may be NULL.
+ *   tuples HOST uint8 [nodes][W]; plus, minus HOST int32 [nodes][W]:
+ *   index of n + e_l / n - e_l, or -1 where the link is invalid. */
+heom_status heom_get_tables(const heom_ctx* ctx, uint8_t* tuples, int32_t* plus,
+                            int32_t* minus);
+/* gamma[W] (Eq. 19, fs^-1); c_re[W], c_im[W] = c(b,k)/hbar (Eq. 20 and the V^o
+ * part of Eq. 17, fs^-2); delta[n_sites] = Eq. 14 bracket (fs^-1).  All HOST. */
+heom_status heom_get_coefficients(const heom_ctx* ctx, double* gamma, double* c_re,
+                                  double* c_im, double* delta);
+
+/* The state lives in caller-owned DEVICE memory (e.g. a torch tensor): the
+ * library never allocates state memory.  heom_workspace_bytes = 4 padded state
+ * buffers ("4 copies") + device tables.  dev_ptr must be 256-byte
+ * aligned and stay valid until heom_destroy or the next bind.  cuda_stream is
+ * a cudaStream_t (NULL = default stream); all work is enqueued on it.
+ * Uploads the tables (synchronous). */
+size_t heom_workspace_bytes(const heom_ctx* ctx);
+heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes,
+                                void* cuda_stream);
+
+/* sigma_0 = the given matrix, every ADO zero.
+ *   sigma0 HOST n_sites*n_sites complex128, row-major. */
+heom_status heom_set_state(heom_ctx* ctx, const double* sigma0);
+/* Full-state I/O, PINNED node order, unpadded [nodes][N][N] complex128, HOST.
+ * These are also the checkpoint/resume path. */
+heom_status heom_set_full_state(heom_ctx* ctx, const double* sigma);
+heom_status heom_get_full_state(heom_ctx* ctx, double* sigma);
+
+/* dsigma = L(current state): one evaluation of Eq. 12-17 on every node; the
+ * state is not changed.  dsigma HOST, same layout as heom_get_full_state. */
+heom_status heom_rhs(heom_ctx* ctx, double* dsigma);
+/* Advance the state by nsteps classical RK4 steps of dt_fs (R6).  Enqueues
+ * 4*nsteps fused kernels on the bound stream and returns; heom_sync or any
+ * HOST getter synchronises. */
+heom_status heom_rk4_steps(heom_ctx* ctx, double dt_fs, int nsteps);
+heom_status heom_sync(heom_ctx* ctx);
+/* Eq. 26: pop[i] = Re sigma_0[i][i] (HOST [n_sites]); trace = sum_i sigma_0[i][i].
+ * Computed by a device reduction kernel; output pointers may be NULL. */
+heom_status heom_populations(heom_ctx* ctx, double* pop, double* trace_re,
+                             double* trace_im);
+
+/* Introspection for the harness. */
+int64_t heom_launch_count(const heom_ctx* ctx); /* kernels launched so far */
+/* With option "timing"=1: sum of CUDA-event durations of the RHS/stage kernels
+ * launched since the last call, and their number.  Synchronises. */
+heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches);
+/* Name of the RHS kernel variant the bound configuration uses (static string). */
+const char* heom_kernel_name(const heom_ctx* ctx);
+/* Human-readable text of the last error on this context (ctx-owned). */
+const char* heom_last_error(const heom_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,209 @@
+"""Thin Python binding of include/heom.h: argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libheom_b200.so; PyTorch is
+used for the device workspace tensor and the stream, nothing else.  There is no CPU
+fallback: if the library is missing or no GPU is present the calls raise.
+This module never imports `oracle`.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libheom_b200.so")
+
+HEOM_OK, HEOM_EINVAL, HEOM_ENOMEM, HEOM_ECUDA, HEOM_ESTATE = 0, -1, -2, -3, -4
+_STATUS = {0: "HEOM_OK", -1: "HEOM_EINVAL", -2: "HEOM_ENOMEM", -3: "HEOM_ECUDA", -4: "HEOM_ESTATE"}
+
+# every symbol include/heom.h declares (tests check the library exports all of them)
+SYMBOLS = [
+    "heom_create", "heom_destroy", "heom_set_option", "heom_num_nodes", "heom_num_modes",
+    "heom_get_tables", "heom_get_coefficients", "heom_workspace_bytes", "heom_bind_workspace",
+    "heom_set_state", "heom_set_full_state", "heom_get_full_state", "heom_rhs", "heom_rk4_steps",
+    "heom_sync", "heom_populations", "heom_launch_count", "heom_kernel_time", "heom_kernel_name",
+    "heom_last_error",
+]
+
+_lib = None
+
+
+class HeomError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+def load_library():
+    """Load libheom_b200.so; fails loudly if it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_1803_03498_b200.build` "
+                          "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = C.CDLL(LIB_PATH)
+    P, dp = C.c_void_p, C.POINTER(C.c_double)
+    lib.heom_create.argtypes = [C.POINTER(P), C.c_int, dp, dp, dp, C.c_double, C.c_int, C.c_int, C.c_int]
+    lib.heom_destroy.argtypes = [P]
+    lib.heom_destroy.restype = None
+    lib.heom_set_option.argtypes = [P, C.c_char_p, C.c_int]
+    lib.heom_num_nodes.argtypes = [P]
+    lib.heom_num_nodes.restype = C.c_int64
+    lib.heom_num_modes.argtypes = [P]
+    lib.heom_get_tables.argtypes = [P, P, P, P]
+    lib.heom_get_coefficients.argtypes = [P, P, P, P, P]
+    lib.heom_workspace_bytes.argtypes = [P]
+    lib.heom_workspace_bytes.restype = C.c_size_t
+    lib.heom_bind_workspace.argtypes = [P, P, C.c_size_t, P]
+    lib.heom_set_state.argtypes = [P, P]
+    lib.heom_set_full_state.argtypes = [P, P]
+    lib.heom_get_full_state.argtypes = [P, P]
+    lib.heom_rhs.argtypes = [P, P]
+    lib.heom_rk4_steps.argtypes = [P, C.c_double, C.c_int]
+    lib.heom_sync.argtypes = [P]
+    lib.heom_populations.argtypes = [P, P, P, P]
+    lib.heom_launch_count.argtypes = [P]
+    lib.heom_launch_count.restype = C.c_int64
+    lib.heom_kernel_time.argtypes = [P, P, P]
+    lib.heom_kernel_name.argtypes = [P]
+    lib.heom_kernel_name.restype = C.c_char_p
+    lib.heom_last_error.argtypes = [P]
+    lib.heom_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _dptr(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+class Heom:
+    """One truncated hierarchy bound to one GPU stream.  Mirrors include/heom.h one to one."""
+
+    def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, device=0, **options):
+        self._lib = load_library()
+        self._h = None
+        H = np.ascontiguousarray(H_cm, dtype=np.float64)
+        if H.ndim != 2 or H.shape[0] != H.shape[1]:
+            raise ValueError("H_cm must be square")
+        self.N = H.shape[0]
+        lam = np.ascontiguousarray(np.broadcast_to(lambda_cm, (self.N,)), dtype=np.float64)
+        nu = np.ascontiguousarray(np.broadcast_to(nu_per_fs, (self.N,)), dtype=np.float64)
+        h = C.c_void_p()
+        rc = self._lib.heom_create(C.byref(h), self.N, _dptr(H), _dptr(lam), _dptr(nu),
+                                   float(T_kelvin), int(K), int(D), int(device))
+        if rc != 0:
+            raise HeomError(rc, "heom_create rejected its arguments")
+        self._h = h
+        self.K, self.D, self.device = int(K), int(D), int(device)
+        self.nodes = int(self._lib.heom_num_nodes(h))
+        self.W = int(self._lib.heom_num_modes(h))
+        self._workspace = None
+        self._stream = None
+        for k, v in options.items():
+            self.set_option(k, v)
+
+    # -- plumbing -------------------------------------------------------------------------
+    def _ck(self, rc):
+        if rc != 0:
+            raise HeomError(rc, self._lib.heom_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.heom_destroy(self._h)
+            self._h = None
+        self._workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_option(self, name, value):
+        self._ck(self._lib.heom_set_option(self._h, name.encode(), int(value)))
+
+    # -- host tables ----------------------------------------------------------------------
+    def tables(self):
+        t = np.empty((self.nodes, self.W), dtype=np.uint8)
+        p = np.empty((self.nodes, self.W), dtype=np.int32)
+        m = np.empty((self.nodes, self.W), dtype=np.int32)
+        self._ck(self._lib.heom_get_tables(self._h, t.ctypes.data, p.ctypes.data, m.ctypes.data))
+        return t, p, m
+
+    def coefficients(self):
+        g = np.empty(self.W); cr = np.empty(self.W); ci = np.empty(self.W); d = np.empty(self.N)
+        self._ck(self._lib.heom_get_coefficients(self._h, g.ctypes.data, cr.ctypes.data,
+                                                 ci.ctypes.data, d.ctypes.data))
+        return g, cr, ci, d
+
+    # -- device workspace -----------------------------------------------------------------
+    def workspace_bytes(self):
+        return int(self._lib.heom_workspace_bytes(self._h))
+
+    def bind(self, stream=None):
+        """Allocate the workspace as a torch tensor on `device` and bind it (PyTorch = memory + stream)."""
+        import torch
+        if not torch.cuda.is_available():
+            raise HeomError(HEOM_ECUDA, "no CUDA device: the HEOM path has no CPU fallback")
+        dev = torch.device("cuda", self.device)
+        nbytes = self.workspace_bytes()
+        self._workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
+        ptr = (self._workspace.data_ptr() + 255) // 256 * 256
+        self._stream = stream if stream is not None else torch.cuda.current_stream(dev)
+        self._ck(self._lib.heom_bind_workspace(self._h, ptr, nbytes, self._stream.cuda_stream))
+        return self
+
+    def bind_raw(self, dev_ptr, nbytes, cuda_stream=0):
+        self._ck(self._lib.heom_bind_workspace(self._h, dev_ptr, nbytes, cuda_stream))
+
+    # -- state ----------------------------------------------------------------------------
+    def set_state(self, sigma0):
+        s = np.ascontiguousarray(sigma0, dtype=np.complex128)
+        if s.shape != (self.N, self.N):
+            raise ValueError("sigma0 must be N x N")
+        self._ck(self._lib.heom_set_state(self._h, s.ctypes.data))
+
+    def set_full_state(self, sigma):
+        s = np.ascontiguousarray(sigma, dtype=np.complex128)
+        if s.shape != (self.nodes, self.N, self.N):
+            raise ValueError("sigma must be [nodes][N][N]")
+        self._ck(self._lib.heom_set_full_state(self._h, s.ctypes.data))
+
+    def get_full_state(self, out=None):
+        if out is None:
+            out = np.empty((self.nodes, self.N, self.N), dtype=np.complex128)
+        self._ck(self._lib.heom_get_full_state(self._h, out.ctypes.data))
+        return out
+
+    def rhs(self, out=None):
+        if out is None:
+            out = np.empty((self.nodes, self.N, self.N), dtype=np.complex128)
+        self._ck(self._lib.heom_rhs(self._h, out.ctypes.data))
+        return out
+
+    def rk4_steps(self, dt_fs, nsteps):
+        self._ck(self._lib.heom_rk4_steps(self._h, float(dt_fs), int(nsteps)))
+
+    def sync(self):
+        self._ck(self._lib.heom_sync(self._h))
+
+    def populations(self):
+        pop = np.empty(self.N)
+        tr = C.c_double(), C.c_double()
+        self._ck(self._lib.heom_populations(self._h, pop.ctypes.data, C.addressof(tr[0]),
+                                            C.addressof(tr[1])))
+        return pop, complex(tr[0].value, tr[1].value)
+
+    # -- introspection --------------------------------------------------------------------
+    def launch_count(self):
+        return int(self._lib.heom_launch_count(self._h))
+
+    def kernel_time(self):
+        ms, n = C.c_double(), C.c_int64()
+        self._ck(self._lib.heom_kernel_time(self._h, C.addressof(ms), C.addressof(n)))
+        return ms.value, n.value
+
+    def kernel_name(self):
+        return self._lib.heom_kernel_name(self._h).decode()

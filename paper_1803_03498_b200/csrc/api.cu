@@ -1,0 +1,426 @@
+// api.cu -- the C ABI of include/heom.h: argument checking, workspace layout, stream-ordered
+// launches.  Every step of the hot path runs in the kernels; nothing here computes on the host
+// beyond the one-time hierarchy/coefficient build.
+#include "../../include/heom.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "hierarchy.hpp"
+#include "kernels.cuh"
+
+using namespace heom;
+
+struct heom_ctx {
+  Hierarchy h;
+  Coefficients c;
+  std::vector<double> H;      // [N][N]
+  std::vector<double> Tterm;  // [N][N]
+  int device = 0;
+  int order = 1;
+  int kernel = 1;
+  int timing = 0;
+  bool hierarchy_built = false;
+  int built_order = -1;
+  std::string err;
+  // workspace
+  bool bound = false;
+  bool have_state = false;
+  cudaStream_t stream = nullptr;
+  int stride = 0;  // complex elements per node
+  size_t state_bytes = 0;
+  double2 *y = nullptr, *acc = nullptr, *xa = nullptr, *xb = nullptr;
+  int32_t *d_plus = nullptr, *d_minus = nullptr, *d_slot = nullptr;
+  uint8_t* d_tuples = nullptr;
+  double *d_damp = nullptr, *d_H = nullptr, *d_T = nullptr, *d_ap = nullptr, *d_amx = nullptr,
+         *d_amo = nullptr, *d_scratch = nullptr;
+  double* h_pinned = nullptr;  // small pinned staging (sigma_0 / populations)
+  int64_t launches = 0;
+  // per-launch timing
+  std::vector<cudaEvent_t> ev;  // pairs
+  size_t ev_used = 0;
+};
+
+namespace {
+
+size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+heom_status fail(heom_ctx* c, heom_status s, const std::string& msg) {
+  if (c) c->err = msg;
+  return s;
+}
+heom_status cuda_fail(heom_ctx* c, cudaError_t e, const char* where) {
+  return fail(c, HEOM_ECUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define CU(call)                                                   \
+  do {                                                             \
+    cudaError_t e_ = (call);                                       \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);       \
+  } while (0)
+
+bool ensure_hierarchy(heom_ctx* c) {
+  if (c->hierarchy_built && c->built_order == c->order) return true;
+  std::string err;
+  if (!build_hierarchy(c->h.N, c->h.K, c->h.D, c->order, c->h, err)) { c->err = err; return false; }
+  c->hierarchy_built = true;
+  c->built_order = c->order;
+  return true;
+}
+
+int node_stride(int N) { return N * N; }
+
+struct Layout {
+  size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, total;
+};
+
+Layout layout_of(const heom_ctx* c) {
+  Layout L{};
+  const size_t nodes = (size_t)c->h.nodes, W = (size_t)c->h.W, N = (size_t)c->h.N, D1 = (size_t)c->h.D + 1;
+  L.state = align_up(nodes * (size_t)node_stride((int)N) * sizeof(double2));
+  size_t o = 0;
+  L.off_y = o; o += L.state;
+  L.off_acc = o; o += L.state;
+  L.off_xa = o; o += L.state;
+  L.off_xb = o; o += L.state;
+  L.off_plus = o; o += align_up(nodes * W * 4);
+  L.off_minus = o; o += align_up(nodes * W * 4);
+  L.off_slot = o; o += align_up(nodes * 4);
+  L.off_tuples = o; o += align_up(nodes * W);
+  L.off_damp = o; o += align_up(nodes * 8);
+  L.off_H = o; o += align_up(N * N * 8);
+  L.off_T = o; o += align_up(N * N * 8);
+  L.off_ap = o; o += align_up(W * D1 * 8);
+  L.off_amx = o; o += align_up(W * D1 * 8);
+  L.off_amo = o; o += align_up(W * D1 * 8);
+  L.off_scratch = o; o += align_up((N + 2) * 8);
+  L.total = o;
+  return L;
+}
+
+RhsParams base_params(const heom_ctx* c) {
+  RhsParams p{};
+  p.N = c->h.N; p.M = c->h.M; p.W = c->h.W; p.D = c->h.D; p.nodes = (int)c->h.nodes;
+  p.stride = c->stride;
+  p.inv_hbar = 1.0 / kHbar;
+  p.H = c->d_H; p.Tterm = c->d_T; p.damp = c->d_damp;
+  p.plus = c->d_plus; p.minus = c->d_minus; p.tuples = c->d_tuples;
+  p.a_plus = c->d_ap; p.a_minus_x = c->d_amx; p.a_minus_o = c->d_amo;
+  return p;
+}
+
+heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (ctx->timing) {
+    if (ctx->ev_used + 2 > ctx->ev.size()) {
+      for (int q = 0; q < 2; ++q) {
+        cudaEvent_t e;
+        CU(cudaEventCreate(&e));
+        ctx->ev.push_back(e);
+      }
+    }
+    e0 = ctx->ev[ctx->ev_used]; e1 = ctx->ev[ctx->ev_used + 1];
+    ctx->ev_used += 2;
+    CU(cudaEventRecord(e0, ctx->stream));
+  }
+  CU(launch_rhs_generic(p, ctx->stream));
+  ctx->launches += 1;
+  if (ctx->timing) CU(cudaEventRecord(e1, ctx->stream));
+  return HEOM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+heom_status heom_create(heom_ctx** out, int n_sites, const double* H_cm, const double* lambda_cm,
+                        const double* nu_per_fs, double T_kelvin, int K, int D, int device) {
+  if (!out) return HEOM_EINVAL;
+  *out = nullptr;
+  if (!H_cm || !lambda_cm || !nu_per_fs || n_sites < 1 || K < 0 || D < 0 || D > 255 || device < 0)
+    return HEOM_EINVAL;
+  for (int i = 0; i < n_sites; ++i)
+    for (int j = 0; j < n_sites; ++j) {
+      const double a = H_cm[(size_t)i * n_sites + j], b = H_cm[(size_t)j * n_sites + i];
+      if (!std::isfinite(a) || a != b) return HEOM_EINVAL;
+    }
+  heom_ctx* c = new (std::nothrow) heom_ctx();
+  if (!c) return HEOM_ENOMEM;
+  c->device = device;
+  c->h.N = n_sites; c->h.K = K; c->h.M = K + 1; c->h.W = n_sites * (K + 1); c->h.D = D;
+  std::string err;
+  if (!build_coefficients(n_sites, K, D, lambda_cm, nu_per_fs, T_kelvin, c->c, err)) {
+    delete c;
+    return HEOM_EINVAL;
+  }
+  c->H.assign(H_cm, H_cm + (size_t)n_sites * n_sites);
+  c->Tterm.assign((size_t)n_sites * n_sites, 0.0);
+  for (int i = 0; i < n_sites; ++i)
+    for (int j = 0; j < n_sites; ++j)
+      if (i != j) c->Tterm[(size_t)i * n_sites + j] = c->c.delta[i] + c->c.delta[j];  // Eq. 14 + 24
+  if (!ensure_hierarchy(c)) {
+    const bool oom = c->err.find("memory") != std::string::npos;
+    delete c;
+    return oom ? HEOM_ENOMEM : HEOM_EINVAL;
+  }
+  *out = c;
+  return HEOM_OK;
+}
+
+void heom_destroy(heom_ctx* c) {
+  if (!c) return;
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  if (c->h_pinned) cudaFreeHost(c->h_pinned);
+  delete c;
+}
+
+heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
+  if (!ctx || !name) return HEOM_EINVAL;
+  const std::string s(name);
+  if (s == "timing") { ctx->timing = value ? 1 : 0; return HEOM_OK; }
+  if (ctx->bound) return fail(ctx, HEOM_ESTATE, "option must be set before heom_bind_workspace");
+  if (s == "order") {
+    if (value != 0 && value != 1) return fail(ctx, HEOM_EINVAL, "order must be 0 or 1");
+    ctx->order = value;
+    return HEOM_OK;
+  }
+  if (s == "kernel") {
+    if (value < 0 || value > 1) return fail(ctx, HEOM_EINVAL, "unknown kernel variant");
+    ctx->kernel = value;
+    return HEOM_OK;
+  }
+  return fail(ctx, HEOM_EINVAL, "unknown option");
+}
+
+int64_t heom_num_nodes(const heom_ctx* c) { return c ? c->h.nodes : -1; }
+int heom_num_modes(const heom_ctx* c) { return c ? c->h.W : -1; }
+
+heom_status heom_get_tables(const heom_ctx* c, uint8_t* tuples, int32_t* plus, int32_t* minus) {
+  if (!c) return HEOM_EINVAL;
+  if (tuples) std::memcpy(tuples, c->h.tuples.data(), c->h.tuples.size());
+  if (plus) std::memcpy(plus, c->h.plus.data(), c->h.plus.size() * sizeof(int32_t));
+  if (minus) std::memcpy(minus, c->h.minus.data(), c->h.minus.size() * sizeof(int32_t));
+  return HEOM_OK;
+}
+
+heom_status heom_get_coefficients(const heom_ctx* c, double* gamma, double* c_re, double* c_im,
+                                  double* delta) {
+  if (!c) return HEOM_EINVAL;
+  const size_t W = (size_t)c->h.W;
+  if (gamma) std::memcpy(gamma, c->c.gamma.data(), W * 8);
+  if (c_re) std::memcpy(c_re, c->c.c_re.data(), W * 8);
+  if (c_im) std::memcpy(c_im, c->c.c_im.data(), W * 8);
+  if (delta) std::memcpy(delta, c->c.delta.data(), (size_t)c->h.N * 8);
+  return HEOM_OK;
+}
+
+size_t heom_workspace_bytes(const heom_ctx* c) { return c ? layout_of(c).total : 0; }
+
+}  // extern "C"
+
+extern "C" {
+
+heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void* cuda_stream) {
+  if (!ctx || !dev_ptr) return HEOM_EINVAL;
+  if (((uintptr_t)dev_ptr & 255u) != 0) return fail(ctx, HEOM_EINVAL, "workspace must be 256-byte aligned");
+  if (rhs_generic_smem(ctx->h.N) == 0)
+    return fail(ctx, HEOM_EINVAL, "n_sites > 96 is not supported by this build");
+  if (!ensure_hierarchy(ctx)) return HEOM_EINVAL;
+  const Layout L = layout_of(ctx);
+  if (bytes < L.total) return fail(ctx, HEOM_ENOMEM, "workspace smaller than heom_workspace_bytes()");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev <= ctx->device)
+    return fail(ctx, HEOM_ECUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
+  CU(cudaSetDevice(ctx->device));
+  ctx->stream = (cudaStream_t)cuda_stream;
+  ctx->stride = node_stride(ctx->h.N);
+  ctx->state_bytes = L.state;
+  char* base = (char*)dev_ptr;
+  ctx->y = (double2*)(base + L.off_y);
+  ctx->acc = (double2*)(base + L.off_acc);
+  ctx->xa = (double2*)(base + L.off_xa);
+  ctx->xb = (double2*)(base + L.off_xb);
+  ctx->d_plus = (int32_t*)(base + L.off_plus);
+  ctx->d_minus = (int32_t*)(base + L.off_minus);
+  ctx->d_slot = (int32_t*)(base + L.off_slot);
+  ctx->d_tuples = (uint8_t*)(base + L.off_tuples);
+  ctx->d_damp = (double*)(base + L.off_damp);
+  ctx->d_H = (double*)(base + L.off_H);
+  ctx->d_T = (double*)(base + L.off_T);
+  ctx->d_ap = (double*)(base + L.off_ap);
+  ctx->d_amx = (double*)(base + L.off_amx);
+  ctx->d_amo = (double*)(base + L.off_amo);
+  ctx->d_scratch = (double*)(base + L.off_scratch);
+  if (!ctx->h_pinned) CU(cudaMallocHost((void**)&ctx->h_pinned, ((size_t)ctx->h.N * ctx->h.N * 2 + 8) * 8));
+
+  // Device tables in STORAGE-slot order: row slot_of[u] holds the slots of u's neighbours.
+  const Hierarchy& h = ctx->h;
+  const size_t nodes = (size_t)h.nodes, W = (size_t)h.W;
+  try {
+    std::vector<int32_t> tp(nodes * W), tm(nodes * W);
+    std::vector<uint8_t> tt(nodes * W);
+    std::vector<double> damp(nodes);
+#pragma omp parallel for schedule(static)
+    for (int64_t u = 0; u < (int64_t)nodes; ++u) {
+      const size_t s = (size_t)h.slot_of[(size_t)u];
+      double d = 0.0;
+      for (size_t l = 0; l < W; ++l) {
+        const int32_t a = h.plus[(size_t)u * W + l], b = h.minus[(size_t)u * W + l];
+        tp[s * W + l] = a < 0 ? -1 : h.slot_of[(size_t)a];
+        tm[s * W + l] = b < 0 ? -1 : h.slot_of[(size_t)b];
+        const uint8_t n = h.tuples[(size_t)u * W + l];
+        tt[s * W + l] = n;
+        d += (double)n * ctx->c.gamma[l];  // Eq. 13
+      }
+      damp[s] = d;
+    }
+    CU(cudaMemcpy(ctx->d_plus, tp.data(), nodes * W * 4, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_minus, tm.data(), nodes * W * 4, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_tuples, tt.data(), nodes * W, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_damp, damp.data(), nodes * 8, cudaMemcpyHostToDevice));
+  } catch (const std::bad_alloc&) {
+    return fail(ctx, HEOM_ENOMEM, "out of host memory while staging the device tables");
+  }
+  const size_t NN = (size_t)h.N * h.N, WD = W * ((size_t)h.D + 1);
+  CU(cudaMemcpy(ctx->d_slot, h.slot_of.data(), nodes * 4, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(ctx->d_H, ctx->H.data(), NN * 8, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(ctx->d_T, ctx->Tterm.data(), NN * 8, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(ctx->d_ap, ctx->c.a_plus.data(), WD * 8, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(ctx->d_amx, ctx->c.a_minus_x.data(), WD * 8, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(ctx->d_amo, ctx->c.a_minus_o.data(), WD * 8, cudaMemcpyHostToDevice));
+  ctx->bound = true;
+  ctx->have_state = false;
+  return HEOM_OK;
+}
+
+heom_status heom_set_state(heom_ctx* ctx, const double* sigma0) {
+  if (!ctx || !sigma0) return HEOM_EINVAL;
+  if (!ctx->bound) return fail(ctx, HEOM_ESTATE, "no workspace bound");
+  const size_t NN = (size_t)ctx->h.N * ctx->h.N;
+  for (size_t e = 0; e < 2 * NN; ++e)
+    if (!std::isfinite(sigma0[e])) return fail(ctx, HEOM_EINVAL, "sigma0 has a non-finite entry");
+  CU(cudaStreamSynchronize(ctx->stream));  // the pinned staging buffer may still be in flight
+  std::memcpy(ctx->h_pinned, sigma0, NN * 16);
+  CU(cudaMemsetAsync(ctx->y, 0, ctx->state_bytes, ctx->stream));
+  CU(cudaMemcpyAsync(ctx->y + (size_t)ctx->h.slot_of[0] * ctx->stride, ctx->h_pinned, NN * 16,
+                     cudaMemcpyHostToDevice, ctx->stream));
+  ctx->have_state = true;
+  return HEOM_OK;
+}
+
+heom_status heom_set_full_state(heom_ctx* ctx, const double* sigma) {
+  if (!ctx || !sigma) return HEOM_EINVAL;
+  if (!ctx->bound) return fail(ctx, HEOM_ESTATE, "no workspace bound");
+  const size_t NN = (size_t)ctx->h.N * ctx->h.N, nodes = (size_t)ctx->h.nodes;
+  // stage in xa (pinned order, unpadded), then permute into y on the device
+  CU(cudaMemcpyAsync(ctx->xa, sigma, nodes * NN * 16, cudaMemcpyHostToDevice, ctx->stream));
+  CU(launch_permute(ctx->xa, ctx->y, ctx->d_slot, (int)nodes, (int)NN, ctx->stride, 1, ctx->stream));
+  ctx->launches += 1;
+  CU(cudaStreamSynchronize(ctx->stream));
+  ctx->have_state = true;
+  return HEOM_OK;
+}
+
+static heom_status read_back(heom_ctx* ctx, const double2* dev_state, double2* scratch, double* host) {
+  const size_t NN = (size_t)ctx->h.N * ctx->h.N, nodes = (size_t)ctx->h.nodes;
+  CU(launch_permute(dev_state, scratch, ctx->d_slot, (int)nodes, (int)NN, ctx->stride, 0, ctx->stream));
+  ctx->launches += 1;
+  CU(cudaMemcpyAsync(host, scratch, nodes * NN * 16, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  return HEOM_OK;
+}
+
+heom_status heom_get_full_state(heom_ctx* ctx, double* sigma) {
+  if (!ctx || !sigma) return HEOM_EINVAL;
+  if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
+  return read_back(ctx, ctx->y, ctx->xa, sigma);
+}
+
+heom_status heom_rhs(heom_ctx* ctx, double* dsigma) {
+  if (!ctx || !dsigma) return HEOM_EINVAL;
+  if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
+  RhsParams p = base_params(ctx);
+  p.x = ctx->y; p.rhs_only = 1; p.out_acc = ctx->xa;
+  heom_status s = launch_rhs(ctx, p);
+  if (s != HEOM_OK) return s;
+  return read_back(ctx, ctx->xa, ctx->xb, dsigma);
+}
+
+/* Classical RK4 (R6) with the stage combinations fused into the RHS epilogue (4 buffers):
+ *   stage 1: k1 = f(y);   xa = y + dt/2 k1;  acc = y + dt/6 k1
+ *   stage 2: k2 = f(xa);  xb = y + dt/2 k2;  acc += dt/3 k2
+ *   stage 3: k3 = f(xb);  xa = y + dt   k3;  acc += dt/3 k3
+ *   stage 4: k4 = f(xa);  y  = acc + dt/6 k4                                        */
+heom_status heom_rk4_steps(heom_ctx* ctx, double dt, int nsteps) {
+  if (!ctx || nsteps < 0 || !std::isfinite(dt)) return HEOM_EINVAL;
+  if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
+  RhsParams p = base_params(ctx);
+  p.rhs_only = 0;
+  for (int step = 0; step < nsteps; ++step) {
+    heom_status s;
+    p.x = ctx->y; p.y = ctx->y; p.acc_in = ctx->y; p.out_x = ctx->xa; p.out_acc = ctx->acc;
+    p.ax = dt / 2.0; p.bx = dt / 6.0;
+    if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+    p.x = ctx->xa; p.acc_in = ctx->acc; p.out_x = ctx->xb; p.out_acc = ctx->acc;
+    p.ax = dt / 2.0; p.bx = dt / 3.0;
+    if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+    p.x = ctx->xb; p.out_x = ctx->xa; p.ax = dt; p.bx = dt / 3.0;
+    if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+    p.x = ctx->xa; p.out_x = nullptr; p.out_acc = ctx->y; p.bx = dt / 6.0;
+    if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+  }
+  return HEOM_OK;
+}
+
+heom_status heom_sync(heom_ctx* ctx) {
+  if (!ctx) return HEOM_EINVAL;
+  if (!ctx->bound) return fail(ctx, HEOM_ESTATE, "no workspace bound");
+  CU(cudaStreamSynchronize(ctx->stream));
+  return HEOM_OK;
+}
+
+heom_status heom_populations(heom_ctx* ctx, double* pop, double* trace_re, double* trace_im) {
+  if (!ctx) return HEOM_EINVAL;
+  if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
+  const int N = ctx->h.N;
+  CU(launch_populations(ctx->y + (size_t)ctx->h.slot_of[0] * ctx->stride, N, ctx->d_scratch, ctx->stream));
+  ctx->launches += 1;
+  CU(cudaMemcpyAsync(ctx->h_pinned, ctx->d_scratch, (size_t)(N + 2) * 8, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  if (pop) std::memcpy(pop, ctx->h_pinned, (size_t)N * 8);
+  if (trace_re) *trace_re = ctx->h_pinned[N];
+  if (trace_im) *trace_im = ctx->h_pinned[N + 1];
+  return HEOM_OK;
+}
+
+int64_t heom_launch_count(const heom_ctx* c) { return c ? c->launches : -1; }
+
+heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches) {
+  if (!ctx) return HEOM_EINVAL;
+  if (!ctx->bound) return fail(ctx, HEOM_ESTATE, "no workspace bound");
+  CU(cudaStreamSynchronize(ctx->stream));
+  double tot = 0.0;
+  for (size_t q = 0; q + 1 < ctx->ev_used; q += 2) {
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, ctx->ev[q], ctx->ev[q + 1]));
+    tot += ms;
+  }
+  if (total_ms) *total_ms = tot;
+  if (launches) *launches = (int64_t)(ctx->ev_used / 2);
+  ctx->ev_used = 0;
+  return HEOM_OK;
+}
+
+const char* heom_kernel_name(const heom_ctx* c) {
+  (void)c;
+  return "rhs_generic_kernel";
+}
+
+const char* heom_last_error(const heom_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+}  // extern "C"

@@ -1,0 +1,179 @@
+// hierarchy.cpp -- see hierarchy.hpp.  Host only, integer + a little fp64.
+#include "hierarchy.hpp"
+
+#include <cmath>
+#include <limits>
+
+namespace heom {
+namespace {
+
+// Pascal triangle choose(a, b) for a <= amax, b <= bmax, saturating at INT64_MAX.
+struct Binomials {
+  int amax, bmax;
+  std::vector<int64_t> v;
+  Binomials(int amax_, int bmax_) : amax(amax_), bmax(bmax_), v((size_t)(amax_ + 1) * (bmax_ + 1), 0) {
+    const int64_t SAT = std::numeric_limits<int64_t>::max();
+    for (int a = 0; a <= amax; ++a) {
+      at(a, 0) = 1;
+      for (int b = 1; b <= bmax && b <= a; ++b) {
+        const int64_t x = at(a - 1, b - 1), y = (b <= a - 1) ? at(a - 1, b) : 0;
+        at(a, b) = (x > SAT - y) ? SAT : x + y;
+      }
+    }
+  }
+  int64_t& at(int a, int b) { return v[(size_t)a * (bmax + 1) + b]; }
+  // C(a, b) with b possibly > a or negative a
+  int64_t operator()(int a, int b) const {
+    if (a < 0 || b < 0 || b > a) return 0;
+    return v[(size_t)a * (bmax + 1) + b];
+  }
+};
+
+// Rank of tuple n (level L) in the pinned order:
+//   u = C(L-1+W, W) + sum_{l=0}^{W-2} C(t_{l+1} - 1 + m_l, m_l),  m_l = W-l-1,
+//   t_{l+1} = sum_{l' > l} n_{l'};  C(x-1+m, m) evaluated as C(x-1+m, x-1), x <= D.
+inline int64_t pinned_rank(const uint8_t* n, int W, int L, const Binomials& C) {
+  int64_t u = (L >= 1) ? C(L - 1 + W, L - 1) : 0;
+  int t = L;  // suffix sum starting at l
+  for (int l = 0; l + 1 < W; ++l) {
+    t -= n[l];  // now t = t_{l+1}
+    if (t == 0) break;
+    u += C(t - 1 + (W - l - 1), t - 1);
+  }
+  return u;
+}
+
+// Rank in plain ascending lexicographic order over all tuples with sum <= D:
+//   slot = sum_l sum_{v < n_l} C(R_l - v + m_l, m_l),  R_l = D - sum_{l'<l} n_{l'}.
+inline int64_t lex_rank(const uint8_t* n, int W, int D, const Binomials& C) {
+  int64_t s = 0;
+  int R = D;
+  for (int l = 0; l < W; ++l) {
+    const int m = W - l - 1;
+    for (int v = 0; v < n[l]; ++v) s += C(R - v + m, R - v);
+    R -= n[l];
+  }
+  return s;
+}
+
+}  // namespace
+
+bool build_hierarchy(int N, int K, int D, int order, Hierarchy& h, std::string& err) {
+  if (N < 1 || K < 0 || D < 0 || D > 255) { err = "invalid N, K or D"; return false; }
+  if (order != 0 && order != 1) { err = "unknown storage order"; return false; }
+  const int M = K + 1;
+  if ((int64_t)N * M > 100000) { err = "tuple length too large"; return false; }
+  const int W = N * M;
+  Binomials C(W + D + 1, D + 1);
+  const int64_t nodes = C(W + D, D);
+  if (nodes <= 0 || nodes > 2147483647LL) { err = "hierarchy has more than 2^31-1 nodes"; return false; }
+  h.N = N; h.K = K; h.M = M; h.W = W; h.D = D; h.nodes = nodes;
+  try {
+    h.tuples.assign((size_t)nodes * W, 0);
+    h.plus.assign((size_t)nodes * W, -1);
+    h.minus.assign((size_t)nodes * W, -1);
+    h.slot_of.assign((size_t)nodes, 0);
+    h.node_at.assign((size_t)nodes, 0);
+  } catch (const std::bad_alloc&) { err = "out of host memory for the hierarchy tables"; return false; }
+
+  // Enumerate in the pinned order with the descending-lexicographic successor:
+  // rightmost p < W-1 with n_p > 0: n_p -= 1, n_{p+1} = n_{W-1} + 1, n_{W-1} = 0 (if p+1 != W-1).
+  {
+    std::vector<uint8_t> n((size_t)W, 0);
+    int64_t u = 0;
+    for (int L = 0; L <= D; ++L) {
+      for (int l = 0; l < W; ++l) n[l] = 0;
+      n[0] = (uint8_t)L;
+      for (;;) {
+        uint8_t* dst = &h.tuples[(size_t)u * W];
+        for (int l = 0; l < W; ++l) dst[l] = n[l];
+        ++u;
+        int p = W - 2;
+        while (p >= 0 && n[p] == 0) --p;
+        if (p < 0) break;
+        const int r = n[W - 1];
+        n[W - 1] = 0;
+        n[p] -= 1;
+        n[p + 1] = (uint8_t)(r + 1);
+      }
+    }
+    if (u != nodes) { err = "internal error: enumeration count mismatch"; return false; }
+  }
+
+  // Links through the closed-form rank of n +- e_l (P:90 validity rules).
+#pragma omp parallel
+  {
+    std::vector<uint8_t> n((size_t)W);
+#pragma omp for schedule(static)
+    for (int64_t u = 0; u < nodes; ++u) {
+      int L = 0;
+      for (int l = 0; l < W; ++l) { n[l] = h.tuples[(size_t)u * W + l]; L += n[l]; }
+      for (int l = 0; l < W; ++l) {
+        if (L < D) {
+          n[l] += 1;
+          h.plus[(size_t)u * W + l] = (int32_t)pinned_rank(n.data(), W, L + 1, C);
+          n[l] -= 1;
+        }
+        if (n[l] > 0) {
+          n[l] -= 1;
+          h.minus[(size_t)u * W + l] = (int32_t)pinned_rank(n.data(), W, L - 1, C);
+          n[l] += 1;
+        }
+      }
+      h.slot_of[(size_t)u] = (order == 0) ? (int32_t)u : (int32_t)lex_rank(n.data(), W, D, C);
+    }
+  }
+  for (int64_t u = 0; u < nodes; ++u) h.node_at[(size_t)h.slot_of[(size_t)u]] = (int32_t)u;
+  return true;
+}
+
+bool build_coefficients(int N, int K, int D, const double* lambda_cm, const double* nu_per_fs,
+                        double T_kelvin, Coefficients& c, std::string& err) {
+  if (!(T_kelvin > 0.0) || !std::isfinite(T_kelvin)) { err = "T_kelvin must be > 0"; return false; }
+  const int M = K + 1, W = N * M;
+  const double two_pi = 6.283185307179586476925286766559;
+  c.beta_hbar = kHbar / (kBoltz * T_kelvin);
+  c.gamma.assign(W, 0.0); c.c_re.assign(W, 0.0); c.c_im.assign(W, 0.0); c.delta.assign(N, 0.0);
+  c.a_plus.assign((size_t)W * (D + 1), 0.0);
+  c.a_minus_x.assign((size_t)W * (D + 1), 0.0);
+  c.a_minus_o.assign((size_t)W * (D + 1), 0.0);
+  for (int b = 0; b < N; ++b) {
+    const double lam = lambda_cm[b], nu = nu_per_fs[b];
+    if (!(lam >= 0.0) || !std::isfinite(lam)) { err = "lambda_cm must be >= 0"; return false; }
+    if (!(nu > 0.0) || !std::isfinite(nu)) { err = "nu_per_fs must be > 0"; return false; }
+    const double lh = lam / kHbar;  // lambda_b / hbar
+    double series = 0.0;            // sum_k Re c(b,k) / gamma(b,k)
+    for (int k = 0; k < M; ++k) {
+      const int l = b * M + k;
+      double g, cre, cim = 0.0;
+      if (k == 0) {
+        g = nu;
+        const double x = 0.5 * c.beta_hbar * nu;
+        const double sn = std::sin(x), cs = std::cos(x);
+        if (lh != 0.0 && sn == 0.0) { err = "cot(beta hbar nu/2) is singular"; return false; }
+        cre = (lh == 0.0) ? 0.0 : lh * nu * (cs / sn);
+        cim = -lh * nu;
+      } else {
+        g = two_pi * (double)k / c.beta_hbar;
+        const double den = c.beta_hbar * (g * g - nu * nu);
+        if (lh != 0.0 && den == 0.0) { err = "Matsubara frequency equals the Drude rate"; return false; }
+        cre = (lh == 0.0) ? 0.0 : 4.0 * lh * nu * g / den;
+      }
+      if (!std::isfinite(cre)) { err = "non-finite coefficient"; return false; }
+      c.gamma[l] = g; c.c_re[l] = cre; c.c_im[l] = cim;
+      series += cre / g;
+      const double s = std::fabs(cre);
+      const double sgn = (cre > 0.0) ? 1.0 : ((cre < 0.0) ? -1.0 : 0.0);
+      for (int n = 0; n <= D; ++n) {
+        c.a_plus[(size_t)l * (D + 1) + n] = std::sqrt(((double)n + 1.0) * s);
+        c.a_minus_x[(size_t)l * (D + 1) + n] = sgn * std::sqrt((double)n * s);
+        c.a_minus_o[(size_t)l * (D + 1) + n] =
+            (k == 0 && s > 0.0) ? std::sqrt((double)n / s) * (lh * nu) : 0.0;
+      }
+    }
+    c.delta[b] = 2.0 * lh / (c.beta_hbar * nu) - series;
+  }
+  return true;
+}
+
+}  // namespace heom

@@ -1,0 +1,47 @@
+// kernels.cuh -- launch interface between the C ABI (api.cu) and the sm_100a kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace heom {
+
+// Everything one RHS evaluation needs.  All pointers DEVICE.  Node index = storage slot.
+struct RhsParams {
+  int N;            // sites
+  int M;            // modes per bath (K+1)
+  int W;            // N*M
+  int D;            // depth
+  int nodes;        // number of nodes
+  int stride;       // complex elements per node in a state buffer (>= N*N)
+  double inv_hbar;  // 1/hbar, fs^-1 per cm^-1
+  const double* H;          // [N][N] cm^-1
+  const double* Tterm;      // [N][N]  (1-delta_ij)(Delta_i+Delta_j)            Eq. 14 + 24
+  const double* damp;       // [nodes] sum_l n_l gamma_l                         Eq. 13
+  const int32_t* plus;      // [nodes][W] slot of n+e_l or -1
+  const int32_t* minus;     // [nodes][W] slot of n-e_l or -1
+  const uint8_t* tuples;    // [nodes][W]
+  const double* a_plus;     // [W][D+1]                                          Eq. 35
+  const double* a_minus_x;  // [W][D+1]                                          Eq. 36, V^x part
+  const double* a_minus_o;  // [W][D+1]                                          Eq. 36, V^o part
+  // state buffers (complex128 as double2)
+  const double2* x;       // stage input: the state the Liouvillian is applied to (gathered)
+  const double2* y;       // step-start state (may be null when not needed)
+  const double2* acc_in;  // running RK4 sum to extend (may alias y)
+  double2* out_x;         // next stage input  = y + ax*k      (null: not written)
+  double2* out_acc;       // acc_in + bx*k     (or, in RHS-only mode, k itself)
+  double ax, bx;
+  int rhs_only;           // 1: out_acc = k, nothing else read or written
+};
+
+// Generic kernel: any N <= 96, one thread per matrix element.
+cudaError_t launch_rhs_generic(const RhsParams& p, cudaStream_t s);
+// Shared-memory bytes the generic kernel needs (0 if N is unsupported).
+size_t rhs_generic_smem(int N);
+
+// dst[slot_of[u]*dst_stride + e] = src[u*NN + e]  (to_device=1) or the inverse (to_device=0)
+cudaError_t launch_permute(const double2* src, double2* dst, const int32_t* slot_of, int nodes,
+                           int NN, int stride, int to_device, cudaStream_t s);
+// out[0..N-1] = Re sigma_0[i][i]; out[N], out[N+1] = trace (re, im)
+cudaError_t launch_populations(const double2* node0, int N, double* out, cudaStream_t s);
+
+}  // namespace heom

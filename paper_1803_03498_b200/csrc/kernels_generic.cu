@@ -1,0 +1,195 @@
+// kernels_generic.cu -- generic sm_100a kernel for the HEOM right-hand side with the
+// RK4 stage combination fused into its epilogue, plus the small helper kernels.
+//
+// One thread per matrix element (i,j) of a node; a CTA owns G consecutive nodes
+// whose sigma tiles it stages in shared memory (coalesced 16 B loads) together
+// with H, so the commutator (Eq. 12) runs out of shared memory.  The couplings to
+// sigma_{n +- e_l} (Eq. 15-17 with the masks Eq. 23-25) touch element (i,j) only
+// through the modes of bath i (row part) and bath j (column part), so each thread
+// walks 2M links instead of W.
+#include "kernels.cuh"
+
+namespace heom {
+namespace {
+
+constexpr int kThreads = 256;
+
+__host__ __device__ inline int nodes_per_cta(int N) {
+  const int NN = N * N;
+  return NN >= kThreads ? 1 : (kThreads + NN - 1) / NN;
+}
+
+__device__ __forceinline__ double2 ldg2(const double2* p) { return __ldg(p); }
+
+__global__ void __launch_bounds__(kThreads)
+rhs_generic_kernel(const RhsParams p) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int N = p.N, NN = N * N, M = p.M, W = p.W, D1 = p.D + 1;
+  const int G = nodes_per_cta(N);
+  double* sH = reinterpret_cast<double*>(smem_raw);                 // [N][N]
+  double2* sS = reinterpret_cast<double2*>(sH + ((NN + 1) & ~1));   // [G][NN]
+
+  const int s0 = blockIdx.x * G;
+  const int g_here = min(G, p.nodes - s0);
+  for (int e = threadIdx.x; e < NN; e += kThreads) sH[e] = p.H[e];
+  for (int e = threadIdx.x; e < g_here * NN; e += kThreads) {
+    const int g = e / NN, q = e - g * NN;
+    sS[e] = p.x[(size_t)(s0 + g) * p.stride + q];
+  }
+  __syncthreads();
+
+  for (int e = threadIdx.x; e < g_here * NN; e += kThreads) {
+    const int g = e / NN, q = e - g * NN;
+    const int i = q / N, j = q - i * N;
+    const int s = s0 + g;
+    const double2* sig = sS + g * NN;
+
+    // Eq. 12: -(i/hbar)(H sigma - sigma H), H real
+    double cr = 0.0, ci = 0.0;
+    for (int m = 0; m < N; ++m) {
+      const double him = sH[i * N + m], hmj = sH[m * N + j];
+      const double2 a = sig[m * N + j], b = sig[i * N + m];
+      cr = fma(him, a.x, cr); ci = fma(him, a.y, ci);
+      cr = fma(-hmj, b.x, cr); ci = fma(-hmj, b.y, ci);
+    }
+    double kr = ci * p.inv_hbar, ki = -cr * p.inv_hbar;
+
+    // Eq. 13 + Eq. 14 (mask Eq. 24)
+    const double2 own = sig[q];
+    const double dd = p.damp[s] + p.Tterm[q];
+    kr = fma(-dd, own.x, kr); ki = fma(-dd, own.y, ki);
+
+    const int32_t* pl = p.plus + (size_t)s * W;
+    const int32_t* mi = p.minus + (size_t)s * W;
+    const uint8_t* tu = p.tuples + (size_t)s * W;
+    if (i != j) {
+      // bath b = i: V^x = +1, V^o = 1
+      for (int k = 0; k < M; ++k) {
+        const int l = i * M + k;
+        const int n = tu[l];
+        const int up = pl[l], dn = mi[l];
+        if (up >= 0) {  // Eq. 15/35: + i a+ sigma^+
+          const double a = p.a_plus[l * D1 + n];
+          const double2 v = ldg2(p.x + (size_t)up * p.stride + q);
+          kr = fma(-a, v.y, kr); ki = fma(a, v.x, ki);
+        }
+        if (dn >= 0) {  // Eq. 16-17/36: (i a-x + a-o) sigma^-
+          const double ax = p.a_minus_x[l * D1 + n], ao = p.a_minus_o[l * D1 + n];
+          const double2 v = ldg2(p.x + (size_t)dn * p.stride + q);
+          kr = fma(ao, v.x, kr); kr = fma(-ax, v.y, kr);
+          ki = fma(ao, v.y, ki); ki = fma(ax, v.x, ki);
+        }
+      }
+      // bath b = j: V^x = -1, V^o = 1
+      for (int k = 0; k < M; ++k) {
+        const int l = j * M + k;
+        const int n = tu[l];
+        const int up = pl[l], dn = mi[l];
+        if (up >= 0) {
+          const double a = p.a_plus[l * D1 + n];
+          const double2 v = ldg2(p.x + (size_t)up * p.stride + q);
+          kr = fma(a, v.y, kr); ki = fma(-a, v.x, ki);
+        }
+        if (dn >= 0) {
+          const double ax = p.a_minus_x[l * D1 + n], ao = p.a_minus_o[l * D1 + n];
+          const double2 v = ldg2(p.x + (size_t)dn * p.stride + q);
+          kr = fma(ao, v.x, kr); kr = fma(ax, v.y, kr);
+          ki = fma(ao, v.y, ki); ki = fma(-ax, v.x, ki);
+        }
+      }
+    } else {
+      // diagonal: V^x = 0, V^o = 2 (bath b = i = j only)
+      for (int k = 0; k < M; ++k) {
+        const int l = i * M + k;
+        const int dn = mi[l];
+        if (dn >= 0) {
+          const double ao = 2.0 * p.a_minus_o[l * D1 + tu[l]];
+          const double2 v = ldg2(p.x + (size_t)dn * p.stride + q);
+          kr = fma(ao, v.x, kr); ki = fma(ao, v.y, ki);
+        }
+      }
+    }
+
+    // fused RK4 stage epilogue
+    const size_t off = (size_t)s * p.stride + q;
+    if (p.rhs_only) {
+      p.out_acc[off] = make_double2(kr, ki);
+    } else {
+      if (p.out_x) {
+        const double2 yv = p.y[off];
+        p.out_x[off] = make_double2(fma(p.ax, kr, yv.x), fma(p.ax, ki, yv.y));
+      }
+      const double2 av = p.acc_in[off];
+      p.out_acc[off] = make_double2(fma(p.bx, kr, av.x), fma(p.bx, ki, av.y));
+    }
+  }
+}
+
+__global__ void permute_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
+                               const int32_t* __restrict__ slot_of, int nodes, int NN, int stride,
+                               int to_device) {
+  const size_t total = (size_t)nodes * NN;
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < total;
+       e += (size_t)gridDim.x * blockDim.x) {
+    const int u = (int)(e / NN), q = (int)(e - (size_t)u * NN);
+    const size_t dev = (size_t)slot_of[u] * stride + q;
+    if (to_device) dst[dev] = src[e];
+    else dst[e] = src[dev];
+  }
+}
+
+__global__ void populations_kernel(const double2* __restrict__ node0, int N, double* __restrict__ out) {
+  // one warp; lanes stride over the diagonal, shuffle-reduce the trace (Eq. 26)
+  double tr = 0.0, ti = 0.0;
+  for (int i = threadIdx.x; i < N; i += 32) {
+    const double2 d = node0[(size_t)i * N + i];
+    out[i] = d.x;
+    tr += d.x; ti += d.y;
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    tr += __shfl_xor_sync(0xffffffffu, tr, o);
+    ti += __shfl_xor_sync(0xffffffffu, ti, o);
+  }
+  if (threadIdx.x == 0) { out[N] = tr; out[N + 1] = ti; }
+}
+
+}  // namespace
+
+size_t rhs_generic_smem(int N) {
+  if (N < 1 || N > 96) return 0;
+  const size_t NN = (size_t)N * N;
+  return ((NN + 1) & ~(size_t)1) * sizeof(double) + (size_t)nodes_per_cta(N) * NN * sizeof(double2);
+}
+
+cudaError_t launch_rhs_generic(const RhsParams& p, cudaStream_t s) {
+  const size_t smem = rhs_generic_smem(p.N);
+  if (smem == 0) return cudaErrorInvalidValue;
+  static size_t configured = 0;
+  if (smem > 48 * 1024 && smem > configured) {
+    cudaError_t e = cudaFuncSetAttribute(rhs_generic_kernel,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = smem;
+  }
+  const int G = nodes_per_cta(p.N);
+  const int grid = (p.nodes + G - 1) / G;
+  rhs_generic_kernel<<<grid, kThreads, smem, s>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_permute(const double2* src, double2* dst, const int32_t* slot_of, int nodes,
+                           int NN, int stride, int to_device, cudaStream_t s) {
+  const size_t total = (size_t)nodes * NN;
+  int grid = (int)((total + 255) / 256);
+  if (grid > 148 * 16) grid = 148 * 16;
+  if (grid < 1) grid = 1;
+  permute_kernel<<<grid, 256, 0, s>>>(src, dst, slot_of, nodes, NN, stride, to_device);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_populations(const double2* node0, int N, double* out, cudaStream_t s) {
+  populations_kernel<<<1, 32, 0, s>>>(node0, N, out);
+  return cudaGetLastError();
+}
+
+}  // namespace heom

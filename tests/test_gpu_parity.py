@@ -1,0 +1,183 @@
+"""-m gpu: the CUDA path, called through the C ABI, against the CPU oracle, element by element
+on the same seeded inputs.
+
+Bars (BASELINE.json north_star): index tables bit-exact; states within 1e-10 max-abs relative
+to max|sigma| after the RK4 run; a single RHS evaluation within 1e-13 relative to max|k|
+(both sides fp64; they differ only in summation order and fma contraction).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import workloads
+from oracle.oracle import Oracle
+
+pytestmark = pytest.mark.gpu
+
+RHS_TOL = 1e-13
+STATE_TOL = 1e-10
+
+
+def _pair(w, **opts):
+    from paper_1803_03498_b200 import Heom
+    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D)
+    g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, **opts).bind()
+    return o, g
+
+
+def _small(N, K, D, T=300.0, seed=0, lam=None, inv_nu=None, name="small"):
+    rng = np.random.default_rng(1000 + seed)
+    H = rng.normal(0.0, 80.0, (N, N)); H = (H + H.T) / 2
+    return workloads.Workload(name, H, 35.0 if lam is None else lam, 50.0 if inv_nu is None else inv_nu,
+                              T, K, D, 0.5, 50)
+
+
+def rel_err(a, b):
+    return np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300)
+
+
+SHAPES = [(2, 1, 4), (7, 1, 3), (14, 0, 3), (3, 2, 4), (1, 0, 5), (5, 0, 0), (96, 0, 1), (33, 1, 1),
+          (7, 1, 5), (16, 0, 2)]
+
+
+@pytest.mark.parametrize("N,K,D", SHAPES)
+@pytest.mark.parametrize("order", [0, 1])
+def test_rhs_parity_random_state(N, K, D, order):
+    """One RHS evaluation on a dense non-Hermitian random state: exercises every term."""
+    w = _small(N, K, D, T=77.0 if K >= 2 else 300.0, seed=N + K + D)
+    o, g = _pair(w, order=order)
+    for a, b in zip(g.tables(), o.tables()):
+        assert np.array_equal(a, b)
+    st = workloads.random_state(o.nodes, N, seed=17 + N)
+    o.set_full_state(st); g.set_full_state(st)
+    assert np.array_equal(g.get_full_state(), st)          # I/O permutation round trip is exact
+    ref, got = o.rhs(), g.rhs()
+    assert rel_err(got, ref) < RHS_TOL
+    assert np.array_equal(g.get_full_state(), st)          # heom_rhs leaves the state alone
+
+
+def test_dimer_1000_steps():
+    """BASELINE config 1 in full."""
+    w = workloads.dimer()
+    o, g = _pair(w)
+    o.set_state(w.sigma0()); g.set_state(w.sigma0())
+    o.rk4_steps(w.dt_fs, w.steps); g.rk4_steps(w.dt_fs, w.steps)
+    ref, got = o.get_full_state(), g.get_full_state()
+    assert rel_err(got, ref) < STATE_TOL
+    pop, tr = g.populations()
+    assert np.allclose(pop, np.diag(ref[0]).real, atol=1e-12)
+    assert abs(tr - 1.0) < 1e-12
+    # golden regression fixture written from the oracle alone
+    gold = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "dimer_trajectory.txt"))
+    assert abs(got[0][0, 0].real - gold[-1, 1]) < 1e-12
+
+
+@pytest.mark.parametrize("name,D,steps", [("cfg2", 4, 300), ("cfg3", 5, 100), ("cfg4", 4, 200),
+                                          ("cfg5", 1, 50), ("cfg5", 2, 10)])
+@pytest.mark.parametrize("order", [0, 1])
+def test_rk4_parity_reduced_depth(name, D, steps, order):
+    """The BASELINE configs at reduced depth (sizes the oracle finishes in seconds; several CTAs
+    and a ragged last CTA), full RK4 runs, every node compared."""
+    w = workloads.get(name).with_(D=D)
+    o, g = _pair(w, order=order)
+    o.set_state(w.sigma0()); g.set_state(w.sigma0())
+    o.rk4_steps(w.dt_fs, steps); g.rk4_steps(w.dt_fs, steps)
+    ref, got = o.get_full_state(), g.get_full_state()
+    assert rel_err(got, ref) < STATE_TOL
+    pop, tr = g.populations()
+    assert abs(tr - 1.0) < 1e-11 and np.all(pop > -1e-9)
+    # Hermiticity of every ADO is preserved by the kernels too
+    assert np.max(np.abs(got - np.conj(np.swapaxes(got, 1, 2)))) < 1e-13 * np.abs(got).max()
+
+
+def test_nonhermitian_initial_state_propagation():
+    """Linear-absorption-like input: sigma_0(0) = mu rho is not Hermitian."""
+    w = _small(4, 1, 4, seed=3)
+    o, g = _pair(w)
+    rng = np.random.default_rng(5)
+    s0 = rng.standard_normal((4, 4)) + 1j * rng.standard_normal((4, 4))
+    o.set_state(s0); g.set_state(s0)
+    o.rk4_steps(0.5, 200); g.rk4_steps(0.5, 200)
+    assert rel_err(g.get_full_state(), o.get_full_state()) < STATE_TOL
+
+
+def test_lambda_zero_and_depth_zero_degenerate_cases():
+    w = _small(3, 1, 3, seed=9, lam=0.0)
+    o, g = _pair(w)
+    rho = workloads.random_density(3, 2)
+    o.set_state(rho); g.set_state(rho)
+    o.rk4_steps(0.5, 100); g.rk4_steps(0.5, 100)
+    got = g.get_full_state()
+    assert np.all(got[1:] == 0)
+    assert rel_err(got, o.get_full_state()) < STATE_TOL
+    w0 = _small(6, 2, 0, seed=4)            # D = 0: a single node, Liouville + terminator only
+    o, g = _pair(w0)
+    rho = workloads.random_density(6, 3)
+    o.set_state(rho); g.set_state(rho)
+    o.rk4_steps(0.5, 100); g.rk4_steps(0.5, 100)
+    assert g.nodes == 1 and rel_err(g.get_full_state(), o.get_full_state()) < STATE_TOL
+    g.rk4_steps(0.5, 0)                     # zero steps is a no-op
+
+
+@pytest.mark.parametrize("name,steps", [("cfg2", 20), ("cfg4", 5)])
+def test_full_size_configs(name, steps):
+    """BASELINE configs 2 and 4 at FULL size, in the launch configuration bench.py times:
+    (i) one RHS evaluation on a dense random state, compared on sampled nodes the oracle
+    computes one by one; (ii) a short RK4 run from sigma_0 = |1><1| compared on every node;
+    (iii) invariants at the end (trace, Hermiticity)."""
+    w = workloads.get(name)
+    o, g = _pair(w)
+    assert g.nodes == w.nodes
+    st = workloads.random_state(o.nodes, w.N, seed=23)
+    o.set_full_state(st); g.set_full_state(st)
+    rng = np.random.default_rng(3)
+    ids = np.unique(np.concatenate([[0, 1, o.nodes - 1, o.nodes // 2], rng.integers(0, o.nodes, 4000)]))
+    got = g.rhs()
+    ref = o.rhs_nodes(ids)
+    assert np.max(np.abs(got[ids] - ref)) / np.max(np.abs(ref)) < RHS_TOL
+    del st, got
+    o.set_state(w.sigma0()); g.set_state(w.sigma0())
+    o.rk4_steps(w.dt_fs, steps); g.rk4_steps(w.dt_fs, steps)
+    ref, got = o.get_full_state(), g.get_full_state()
+    assert rel_err(got, ref) < STATE_TOL
+    pop, tr = g.populations()
+    assert abs(tr - 1.0) < 1e-12
+    assert np.max(np.abs(got - np.conj(np.swapaxes(got, 1, 2)))) < 1e-14
+
+
+@pytest.mark.skipif(os.environ.get("HEOM_FULL", "0") != "1", reason="set HEOM_FULL=1 (needs ~60 GB host RAM)")
+@pytest.mark.parametrize("name", ["cfg3", "cfg5"])
+def test_full_size_large_configs_sampled_rhs(name):
+    """Configs 3 and 5 at full size: RHS on sampled nodes + invariants after a few steps."""
+    w = workloads.get(name)
+    o, g = _pair(w)
+    st = workloads.random_state(o.nodes, w.N, seed=29)
+    o.set_full_state(st); g.set_full_state(st)
+    del st
+    rng = np.random.default_rng(4)
+    n_s = 2000 if name == "cfg3" else 64
+    ids = np.unique(np.concatenate([[0, 1, o.nodes - 1], rng.integers(0, o.nodes, n_s)]))
+    ref = o.rhs_nodes(ids)
+    got = g.rhs()
+    assert np.max(np.abs(got[ids] - ref)) / np.max(np.abs(ref)) < RHS_TOL
+    del got
+    g.set_state(w.sigma0())
+    g.rk4_steps(w.dt_fs, 3)
+    pop, tr = g.populations()
+    assert abs(tr - 1.0) < 1e-12
+
+
+def test_call_order_errors_on_gpu():
+    from paper_1803_03498_b200 import Heom, HeomError
+    w = workloads.dimer()
+    g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D).bind()
+    with pytest.raises(HeomError) as e:
+        g.rk4_steps(1.0, 1)                 # no state yet
+    assert e.value.status == -4
+    with pytest.raises(HeomError):
+        g.set_state(np.full((2, 2), np.nan))
+    g.set_state(w.sigma0())
+    n0 = g.launch_count()
+    g.rk4_steps(1.0, 3)
+    assert g.launch_count() - n0 == 12      # 4 fused stage kernels per step, nothing else
