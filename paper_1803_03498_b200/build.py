@@ -37,6 +37,8 @@ def deps():
 def build(force: bool = False, verbose: bool = False, extra=()) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(map(os.path.getmtime, deps())):
         return LIB
+    if os.environ.get("HEOM_DEBUG"):
+        extra = list(extra) + ["-DHEOM_DEBUG"]
     cmd = [nvcc_path()] + NVCC_FLAGS + list(extra) + ["-I", INCLUDE, "-o", LIB] + sources() + ["-lgomp"]
     if verbose:
         cmd.insert(1, "-Xptxas")

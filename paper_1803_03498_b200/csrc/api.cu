@@ -34,7 +34,9 @@ struct heom_ctx {
   int stride = 0;  // complex elements per node
   size_t state_bytes = 0;
   double2 *y = nullptr, *acc = nullptr, *xa = nullptr, *xb = nullptr;
-  int32_t *d_plus = nullptr, *d_minus = nullptr, *d_slot = nullptr;
+  int32_t *d_plus = nullptr, *d_minus = nullptr, *d_slot = nullptr, *d_links = nullptr;
+  int lrow = 0;
+  bool use_rows = false;
   uint8_t* d_tuples = nullptr;
   double *d_damp = nullptr, *d_H = nullptr, *d_T = nullptr, *d_ap = nullptr, *d_amx = nullptr,
          *d_amo = nullptr, *d_scratch = nullptr;
@@ -72,10 +74,12 @@ bool ensure_hierarchy(heom_ctx* c) {
 }
 
 int node_stride(int N) { return N * N; }
+// int32 entries per row of the combined link table: plus[W], minus[W], W tuple bytes, padded to 16 B
+int links_row(int W) { return (2 * W + (W + 3) / 4 + 3) / 4 * 4; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, total;
 };
 
 Layout layout_of(const heom_ctx* c) {
@@ -98,6 +102,7 @@ Layout layout_of(const heom_ctx* c) {
   L.off_amx = o; o += align_up(W * D1 * 8);
   L.off_amo = o; o += align_up(W * D1 * 8);
   L.off_scratch = o; o += align_up((N + 2) * 8);
+  L.off_links = o; o += align_up(nodes * (size_t)links_row((int)W) * 4);
   L.total = o;
   return L;
 }
@@ -127,7 +132,8 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
     ctx->ev_used += 2;
     CU(cudaEventRecord(e0, ctx->stream));
   }
-  CU(launch_rhs_generic(p, ctx->stream));
+  if (ctx->use_rows) CU(launch_rhs_rows(p, ctx->d_links, ctx->lrow, ctx->H.data(), ctx->stream));
+  else CU(launch_rhs_generic(p, ctx->stream));
   ctx->launches += 1;
   if (ctx->timing) CU(cudaEventRecord(e1, ctx->stream));
   return HEOM_OK;
@@ -256,6 +262,9 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->d_amx = (double*)(base + L.off_amx);
   ctx->d_amo = (double*)(base + L.off_amo);
   ctx->d_scratch = (double*)(base + L.off_scratch);
+  ctx->d_links = (int32_t*)(base + L.off_links);
+  ctx->lrow = links_row(ctx->h.W);
+  ctx->use_rows = ctx->kernel == 1 && rows_supported(ctx->h.N, ctx->h.W, ctx->h.D);
   if (!ctx->h_pinned) CU(cudaMallocHost((void**)&ctx->h_pinned, ((size_t)ctx->h.N * ctx->h.N * 2 + 8) * 8));
 
   // Device tables in STORAGE-slot order: row slot_of[u] holds the slots of u's neighbours.
@@ -283,6 +292,18 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
     CU(cudaMemcpy(ctx->d_minus, tm.data(), nodes * W * 4, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(ctx->d_tuples, tt.data(), nodes * W, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(ctx->d_damp, damp.data(), nodes * 8, cudaMemcpyHostToDevice));
+    if (ctx->use_rows) {
+      const size_t lrow = (size_t)ctx->lrow;
+      std::vector<int32_t> lk(nodes * lrow, 0);
+#pragma omp parallel for schedule(static)
+      for (int64_t s = 0; s < (int64_t)nodes; ++s) {
+        int32_t* row = &lk[(size_t)s * lrow];
+        std::memcpy(row, &tp[(size_t)s * W], W * 4);
+        std::memcpy(row + W, &tm[(size_t)s * W], W * 4);
+        std::memcpy(row + 2 * W, &tt[(size_t)s * W], W);
+      }
+      CU(cudaMemcpy(ctx->d_links, lk.data(), nodes * lrow * 4, cudaMemcpyHostToDevice));
+    }
   } catch (const std::bad_alloc&) {
     return fail(ctx, HEOM_ENOMEM, "out of host memory while staging the device tables");
   }
@@ -417,8 +438,7 @@ heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches)
 }
 
 const char* heom_kernel_name(const heom_ctx* c) {
-  (void)c;
-  return "rhs_generic_kernel";
+  return (c && c->use_rows) ? "rhs_rows_kernel" : "rhs_generic_kernel";
 }
 
 const char* heom_last_error(const heom_ctx* c) { return c ? c->err.c_str() : "null context"; }

@@ -38,6 +38,12 @@ cudaError_t launch_rhs_generic(const RhsParams& p, cudaStream_t s);
 // Shared-memory bytes the generic kernel needs (0 if N is unsupported).
 size_t rhs_generic_smem(int N);
 
+// Row-per-thread kernel for 2 <= N <= 16 (kernels_rows.cu).  links: DEVICE [nodes][lrow] int32 =
+// plus[W], minus[W], then the tuple bytes; H_host: HOST [N][N] (travels in the kernel parameters).
+bool rows_supported(int N, int W, int D);
+cudaError_t launch_rhs_rows(const RhsParams& p, const int32_t* links, int lrow, const double* H_host,
+                            cudaStream_t s);
+
 // dst[slot_of[u]*dst_stride + e] = src[u*NN + e]  (to_device=1) or the inverse (to_device=0)
 cudaError_t launch_permute(const double2* src, double2* dst, const int32_t* slot_of, int nodes,
                            int NN, int stride, int to_device, cudaStream_t s);

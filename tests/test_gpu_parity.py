@@ -38,15 +38,15 @@ def rel_err(a, b):
 
 
 SHAPES = [(2, 1, 4), (7, 1, 3), (14, 0, 3), (3, 2, 4), (1, 0, 5), (5, 0, 0), (96, 0, 1), (33, 1, 1),
-          (7, 1, 5), (16, 0, 2)]
+          (7, 1, 5), (16, 0, 2), (4, 0, 6), (6, 1, 3), (9, 0, 3), (11, 1, 2), (13, 0, 2), (15, 0, 2)]
 
 
 @pytest.mark.parametrize("N,K,D", SHAPES)
-@pytest.mark.parametrize("order", [0, 1])
-def test_rhs_parity_random_state(N, K, D, order):
+@pytest.mark.parametrize("order,kernel", [(0, 1), (1, 1), (1, 0)])
+def test_rhs_parity_random_state(N, K, D, order, kernel):
     """One RHS evaluation on a dense non-Hermitian random state: exercises every term."""
     w = _small(N, K, D, T=77.0 if K >= 2 else 300.0, seed=N + K + D)
-    o, g = _pair(w, order=order)
+    o, g = _pair(w, order=order, kernel=kernel)
     for a, b in zip(g.tables(), o.tables()):
         assert np.array_equal(a, b)
     st = workloads.random_state(o.nodes, N, seed=17 + N)
@@ -75,12 +75,12 @@ def test_dimer_1000_steps():
 
 @pytest.mark.parametrize("name,D,steps", [("cfg2", 4, 300), ("cfg3", 5, 100), ("cfg4", 4, 200),
                                           ("cfg5", 1, 50), ("cfg5", 2, 10)])
-@pytest.mark.parametrize("order", [0, 1])
-def test_rk4_parity_reduced_depth(name, D, steps, order):
+@pytest.mark.parametrize("order,kernel", [(0, 1), (1, 1), (1, 0)])
+def test_rk4_parity_reduced_depth(name, D, steps, order, kernel):
     """The BASELINE configs at reduced depth (sizes the oracle finishes in seconds; several CTAs
     and a ragged last CTA), full RK4 runs, every node compared."""
     w = workloads.get(name).with_(D=D)
-    o, g = _pair(w, order=order)
+    o, g = _pair(w, order=order, kernel=kernel)
     o.set_state(w.sigma0()); g.set_state(w.sigma0())
     o.rk4_steps(w.dt_fs, steps); g.rk4_steps(w.dt_fs, steps)
     ref, got = o.get_full_state(), g.get_full_state()
