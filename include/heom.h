@@ -66,7 +66,11 @@ void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
  *             lexicographic (default 1)
  *   "kernel"  0 = generic element-per-thread kernel, 1 = auto (specialised
  *             kernels where available; default)
- *   "timing"  1 = bracket every RHS launch with CUDA events (heom_kernel_time) */
+ *   "timing"  1 = bracket every RHS launch with CUDA events (heom_kernel_time)
+ *   "hermitian" 1 (default) = when heom_set_state / heom_set_full_state find the state
+ *             EXACTLY Hermitian (every node equals its conjugate transpose bit for bit), use
+ *             the row-gather kernel that keeps it exactly Hermitian; 0 = always the general
+ *             kernel.  "timing" and "hermitian" may be changed at any time. */
 heom_status heom_set_option(heom_ctx* ctx, const char* name, int value);
 
 int64_t heom_num_nodes(const heom_ctx* ctx); /* Eq. 9: C(W+D, D) */

@@ -37,6 +37,13 @@ struct heom_ctx {
   int32_t *d_plus = nullptr, *d_minus = nullptr, *d_slot = nullptr, *d_links = nullptr;
   int lrow = 0;
   bool use_rows = false;
+  // Hermitian fast path (kernels_herm.cu)
+  int herm_opt = 1;          // option "hermitian": 1 = use it when the state is exactly Hermitian
+  bool use_herm = false;     // kernel available for this shape
+  bool state_hermitian = false;
+  int32_t* d_linksH = nullptr;
+  double* d_coefH = nullptr;
+  int lrowH = 0;
   uint8_t* d_tuples = nullptr;
   double *d_damp = nullptr, *d_H = nullptr, *d_T = nullptr, *d_ap = nullptr, *d_amx = nullptr,
          *d_amo = nullptr, *d_scratch = nullptr;
@@ -79,7 +86,7 @@ int links_row(int W) { return (2 * W + (W + 3) / 4 + 3) / 4 * 4; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, total;
 };
 
 Layout layout_of(const heom_ctx* c) {
@@ -103,6 +110,8 @@ Layout layout_of(const heom_ctx* c) {
   L.off_amo = o; o += align_up(W * D1 * 8);
   L.off_scratch = o; o += align_up((N + 2) * 8);
   L.off_links = o; o += align_up(nodes * (size_t)links_row((int)W) * 4);
+  L.off_linksH = o; o += align_up(nodes * (size_t)herm_links_row((int)N, c->h.M) * 4);
+  L.off_coefH = o; o += align_up(W * D1 * 32);
   L.total = o;
   return L;
 }
@@ -132,7 +141,9 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
     ctx->ev_used += 2;
     CU(cudaEventRecord(e0, ctx->stream));
   }
-  if (ctx->use_rows) CU(launch_rhs_rows(p, ctx->d_links, ctx->lrow, ctx->H.data(), ctx->stream));
+  if (ctx->use_herm && ctx->herm_opt && ctx->state_hermitian)
+    CU(launch_rhs_herm(p, ctx->d_linksH, ctx->lrowH, ctx->d_coefH, ctx->H.data(), ctx->c.delta.data(), ctx->stream));
+  else if (ctx->use_rows) CU(launch_rhs_rows(p, ctx->d_links, ctx->lrow, ctx->H.data(), ctx->stream));
   else CU(launch_rhs_generic(p, ctx->stream));
   ctx->launches += 1;
   if (ctx->timing) CU(cudaEventRecord(e1, ctx->stream));
@@ -188,6 +199,7 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
   if (!ctx || !name) return HEOM_EINVAL;
   const std::string s(name);
   if (s == "timing") { ctx->timing = value ? 1 : 0; return HEOM_OK; }
+  if (s == "hermitian") { ctx->herm_opt = value ? 1 : 0; return HEOM_OK; }
   if (ctx->bound) return fail(ctx, HEOM_ESTATE, "option must be set before heom_bind_workspace");
   if (s == "order") {
     if (value != 0 && value != 1) return fail(ctx, HEOM_EINVAL, "order must be 0 or 1");
@@ -264,7 +276,11 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->d_scratch = (double*)(base + L.off_scratch);
   ctx->d_links = (int32_t*)(base + L.off_links);
   ctx->lrow = links_row(ctx->h.W);
-  ctx->use_rows = ctx->kernel == 1 && rows_supported(ctx->h.N, ctx->h.W, ctx->h.D);
+  ctx->use_rows = ctx->kernel == 1 && rows_supported(ctx->h.N, ctx->h.W, ctx->h.D, ctx->lrow);
+  ctx->d_linksH = (int32_t*)(base + L.off_linksH);
+  ctx->d_coefH = (double*)(base + L.off_coefH);
+  ctx->lrowH = herm_links_row(ctx->h.N, ctx->h.M);
+  ctx->use_herm = ctx->kernel == 1 && herm_supported(ctx->h.N, ctx->h.W, ctx->h.D);
   if (!ctx->h_pinned) CU(cudaMallocHost((void**)&ctx->h_pinned, ((size_t)ctx->h.N * ctx->h.N * 2 + 8) * 8));
 
   // Device tables in STORAGE-slot order: row slot_of[u] holds the slots of u's neighbours.
@@ -304,6 +320,20 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
       }
       CU(cudaMemcpy(ctx->d_links, lk.data(), nodes * lrow * 4, cudaMemcpyHostToDevice));
     }
+    if (ctx->use_herm) {
+      const size_t lrow = (size_t)ctx->lrowH;
+      std::vector<int32_t> lk(nodes * lrow, 0);
+#pragma omp parallel for schedule(static)
+      for (int64_t s = 0; s < (int64_t)nodes; ++s)
+        herm_pack_links(h.N, h.M, &tp[(size_t)s * W], &tm[(size_t)s * W], &tt[(size_t)s * W], &lk[(size_t)s * lrow]);
+      CU(cudaMemcpy(ctx->d_linksH, lk.data(), nodes * lrow * 4, cudaMemcpyHostToDevice));
+      const size_t D1 = (size_t)h.D + 1;
+      std::vector<double> cf(W * D1 * 4, 0.0);
+      for (size_t q = 0; q < W * D1; ++q) {
+        cf[4 * q] = ctx->c.a_plus[q]; cf[4 * q + 1] = ctx->c.a_minus_x[q]; cf[4 * q + 2] = ctx->c.a_minus_o[q];
+      }
+      CU(cudaMemcpy(ctx->d_coefH, cf.data(), W * D1 * 32, cudaMemcpyHostToDevice));
+    }
   } catch (const std::bad_alloc&) {
     return fail(ctx, HEOM_ENOMEM, "out of host memory while staging the device tables");
   }
@@ -325,6 +355,17 @@ heom_status heom_set_state(heom_ctx* ctx, const double* sigma0) {
   const size_t NN = (size_t)ctx->h.N * ctx->h.N;
   for (size_t e = 0; e < 2 * NN; ++e)
     if (!std::isfinite(sigma0[e])) return fail(ctx, HEOM_EINVAL, "sigma0 has a non-finite entry");
+  {
+    const int N = ctx->h.N;
+    bool herm = true;
+    for (int i = 0; i < N && herm; ++i)
+      for (int j = i; j < N; ++j) {
+        const double ar = sigma0[2 * (i * N + j)], ai = sigma0[2 * (i * N + j) + 1];
+        const double br = sigma0[2 * (j * N + i)], bi = sigma0[2 * (j * N + i) + 1];
+        if (ar != br || ai != -bi) { herm = false; break; }
+      }
+    ctx->state_hermitian = herm;
+  }
   CU(cudaStreamSynchronize(ctx->stream));  // the pinned staging buffer may still be in flight
   std::memcpy(ctx->h_pinned, sigma0, NN * 16);
   CU(cudaMemsetAsync(ctx->y, 0, ctx->state_bytes, ctx->stream));
@@ -338,6 +379,19 @@ heom_status heom_set_full_state(heom_ctx* ctx, const double* sigma) {
   if (!ctx || !sigma) return HEOM_EINVAL;
   if (!ctx->bound) return fail(ctx, HEOM_ESTATE, "no workspace bound");
   const size_t NN = (size_t)ctx->h.N * ctx->h.N, nodes = (size_t)ctx->h.nodes;
+  {
+    // exact Hermiticity of every node selects the row-gather kernel (checked, never assumed)
+    const int N = ctx->h.N;
+    int bad = 0;
+#pragma omp parallel for schedule(static) reduction(| : bad)
+    for (int64_t u = 0; u < (int64_t)nodes; ++u) {
+      const double* a = sigma + (size_t)u * NN * 2;
+      for (int i = 0; i < N; ++i)
+        for (int j = i; j < N; ++j)
+          if (a[2 * (i * N + j)] != a[2 * (j * N + i)] || a[2 * (i * N + j) + 1] != -a[2 * (j * N + i) + 1]) bad |= 1;
+    }
+    ctx->state_hermitian = !bad;
+  }
   // stage in xa (pinned order, unpadded), then permute into y on the device
   CU(cudaMemcpyAsync(ctx->xa, sigma, nodes * NN * 16, cudaMemcpyHostToDevice, ctx->stream));
   CU(launch_permute(ctx->xa, ctx->y, ctx->d_slot, (int)nodes, (int)NN, ctx->stride, 1, ctx->stream));
@@ -438,7 +492,9 @@ heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches)
 }
 
 const char* heom_kernel_name(const heom_ctx* c) {
-  return (c && c->use_rows) ? "rhs_rows_kernel" : "rhs_generic_kernel";
+  if (!c) return "none";
+  if (c->use_herm && c->herm_opt && c->state_hermitian) return "rhs_herm_kernel";
+  return c->use_rows ? "rhs_rows_kernel" : "rhs_generic_kernel";
 }
 
 const char* heom_last_error(const heom_ctx* c) { return c ? c->err.c_str() : "null context"; }

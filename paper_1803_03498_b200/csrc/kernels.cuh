@@ -40,9 +40,19 @@ size_t rhs_generic_smem(int N);
 
 // Row-per-thread kernel for 2 <= N <= 16 (kernels_rows.cu).  links: DEVICE [nodes][lrow] int32 =
 // plus[W], minus[W], then the tuple bytes; H_host: HOST [N][N] (travels in the kernel parameters).
-bool rows_supported(int N, int W, int D);
+bool rows_supported(int N, int W, int D, int lrow);
 cudaError_t launch_rhs_rows(const RhsParams& p, const int32_t* links, int lrow, const double* H_host,
                             cudaStream_t s);
+
+// Hermitian-state kernel for 2 <= N <= 16 (kernels_herm.cu).  links: DEVICE [nodes][lrow] int32 in the
+// grouped layout written by herm_pack_links (per mode index kk: plus[N pad 4], minus[N pad 4], tuple
+// bytes [N pad 8]); coef: DEVICE [W][D+1][4] doubles = a+, a-x, a-o, 0.  H_host, delta_host: HOST.
+int herm_links_row(int N, int M);   // ints per row (multiple of 4), 0 if unsupported
+bool herm_supported(int N, int W, int D);
+void herm_pack_links(int N, int M, const int32_t* plus, const int32_t* minus, const uint8_t* tuple,
+                     int32_t* row);  // HOST: one node's row from its plus/minus/tuple entries [W]
+cudaError_t launch_rhs_herm(const RhsParams& p, const int32_t* links, int lrow, const double* coef,
+                            const double* H_host, const double* delta_host, cudaStream_t s);
 
 // dst[slot_of[u]*dst_stride + e] = src[u*NN + e]  (to_device=1) or the inverse (to_device=0)
 cudaError_t launch_permute(const double2* src, double2* dst, const int32_t* slot_of, int nodes,

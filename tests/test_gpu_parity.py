@@ -57,6 +57,27 @@ def test_rhs_parity_random_state(N, K, D, order, kernel):
     assert np.array_equal(g.get_full_state(), st)          # heom_rhs leaves the state alone
 
 
+@pytest.mark.parametrize("N,K,D", [(2, 1, 4), (7, 1, 4), (14, 0, 3), (3, 2, 4), (5, 0, 0), (16, 0, 2), (4, 0, 6),
+                                   (6, 1, 3), (9, 0, 3), (11, 1, 2), (13, 0, 2), (8, 2, 2)])
+@pytest.mark.parametrize("order", [0, 1])
+def test_rhs_parity_hermitian_state(N, K, D, order):
+    """Dense HERMITIAN random state: takes the row-gather kernel (kernels_herm.cu); the result must
+    match the oracle and be exactly Hermitian."""
+    w = _small(N, K, D, T=77.0 if K >= 2 else 300.0, seed=2 * N + K + D)
+    o, g = _pair(w, order=order)
+    st = workloads.random_state(o.nodes, N, seed=31 + N, hermitian=True)
+    o.set_full_state(st); g.set_full_state(st)
+    assert g.kernel_name() == "rhs_herm_kernel"
+    ref, got = o.rhs(), g.rhs()
+    assert rel_err(got, ref) < RHS_TOL
+    assert np.array_equal(got, np.conj(np.swapaxes(got, 1, 2)))
+    # a non-Hermitian state on the same context falls back to the general kernel
+    st2 = workloads.random_state(o.nodes, N, seed=32 + N)
+    o.set_full_state(st2); g.set_full_state(st2)
+    assert g.kernel_name() == "rhs_rows_kernel"
+    assert rel_err(g.rhs(), o.rhs()) < RHS_TOL
+
+
 def test_dimer_1000_steps():
     """BASELINE config 1 in full."""
     w = workloads.dimer()
@@ -75,20 +96,23 @@ def test_dimer_1000_steps():
 
 @pytest.mark.parametrize("name,D,steps", [("cfg2", 4, 300), ("cfg3", 5, 100), ("cfg4", 4, 200),
                                           ("cfg5", 1, 50), ("cfg5", 2, 10)])
-@pytest.mark.parametrize("order,kernel", [(0, 1), (1, 1), (1, 0)])
-def test_rk4_parity_reduced_depth(name, D, steps, order, kernel):
+@pytest.mark.parametrize("order,kernel,herm", [(0, 1, 1), (1, 1, 1), (1, 1, 0), (1, 0, 0)])
+def test_rk4_parity_reduced_depth(name, D, steps, order, kernel, herm):
     """The BASELINE configs at reduced depth (sizes the oracle finishes in seconds; several CTAs
     and a ragged last CTA), full RK4 runs, every node compared."""
     w = workloads.get(name).with_(D=D)
-    o, g = _pair(w, order=order, kernel=kernel)
+    o, g = _pair(w, order=order, kernel=kernel, hermitian=herm)
     o.set_state(w.sigma0()); g.set_state(w.sigma0())
     o.rk4_steps(w.dt_fs, steps); g.rk4_steps(w.dt_fs, steps)
     ref, got = o.get_full_state(), g.get_full_state()
     assert rel_err(got, ref) < STATE_TOL
     pop, tr = g.populations()
     assert abs(tr - 1.0) < 1e-11 and np.all(pop > -1e-9)
-    # Hermiticity of every ADO is preserved by the kernels too
-    assert np.max(np.abs(got - np.conj(np.swapaxes(got, 1, 2)))) < 1e-13 * np.abs(got).max()
+    # Hermiticity of every ADO is preserved by the kernels too (exactly, on the Hermitian path)
+    asym = np.max(np.abs(got - np.conj(np.swapaxes(got, 1, 2))))
+    assert asym < 1e-13 * np.abs(got).max()
+    if g.kernel_name() == "rhs_herm_kernel":
+        assert asym == 0.0
 
 
 def test_nonhermitian_initial_state_propagation():
@@ -144,6 +168,13 @@ def test_full_size_configs(name, steps):
     pop, tr = g.populations()
     assert abs(tr - 1.0) < 1e-12
     assert np.max(np.abs(got - np.conj(np.swapaxes(got, 1, 2)))) < 1e-14
+    # Hermitian dense state at full size through the row-gather kernel, sampled nodes
+    st = workloads.random_state(o.nodes, w.N, seed=24, hermitian=True)
+    o.set_full_state(st); g.set_full_state(st)
+    assert g.kernel_name() == "rhs_herm_kernel"
+    got = g.rhs()
+    ref = o.rhs_nodes(ids)
+    assert np.max(np.abs(got[ids] - ref)) / np.max(np.abs(ref)) < RHS_TOL
 
 
 @pytest.mark.skipif(os.environ.get("HEOM_FULL", "0") != "1", reason="set HEOM_FULL=1 (needs ~60 GB host RAM)")
