@@ -45,49 +45,87 @@ struct HermParams {
   double delta[N];
 };
 
-__device__ __forceinline__ void prefetch_l2h(const void* ptr) {
-  asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
+// ---- TMA bulk copy (global -> shared, completion on an mbarrier) and friends ------------------
+__device__ __forceinline__ unsigned smem_u32(const void* ptr) {
+  return (unsigned)__cvta_generic_to_shared(ptr);
+}
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes,
+                                         unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src_gmem, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src_gmem), "r"(bytes) : "memory");
+}
+// 16-byte load from a generic address (shared tile or global state), executed only when `on`;
+// returns 0 otherwise.  Keeps the gather loop straight-line so the loads of a batch overlap.
+__device__ __forceinline__ double2 ld_if(const double2* ptr, bool on) {
+  double2 r;
+  asm("{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, %3, 0;\n"
+      "mov.f64 %0, 0d0000000000000000;\n"
+      "mov.f64 %1, 0d0000000000000000;\n"
+      "@p ld.v2.f64 {%0, %1}, [%2];\n"
+      "}\n" : "=d"(r.x), "=d"(r.y) : "l"(ptr), "r"((int)on));
+  return r;
 }
 
 template <int N>
 __global__ void __launch_bounds__(HermCfg<N>::THREADS, HermCfg<N>::MINB)
 rhs_herm_kernel(const __grid_constant__ HermParams<N> P) {
   using C = HermCfg<N>;
-  constexpr int NN = C::NN, G = C::G, T = C::T, WARPS = C::WARPS, THREADS = C::THREADS;
+  constexpr int NN = C::NN, G = C::G, T = C::T, WARPS = C::WARPS;
   constexpr int NP4 = C::NP4, NB8 = C::NB8;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   const RhsParams& p = P.p;
   const int W = p.W, M = p.M, D1 = p.D + 1, lrow = P.lrow;
   double2* sX = reinterpret_cast<double2*>(smem_raw);            // [T][NN]
   double2* sK = sX + T * NN;                                     // [WARPS][G][NN]
   double2* sC = sK + WARPS * G * NN;                             // [W*D1][2] double2 = 4 doubles
   int32_t* sL = reinterpret_cast<int32_t*>(sC + 2 * W * D1);     // [T][lrow]
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(sL + T * lrow);
 
   const int t0 = blockIdx.x * T;
   const int tcount = min(T, p.nodes - t0);
-  {
-    const double2* src = p.x + (size_t)t0 * p.stride;
-    for (int e = threadIdx.x; e < tcount * NN; e += THREADS) sX[e] = src[e];
-    const int4* lsrc = reinterpret_cast<const int4*>(P.links + (size_t)t0 * lrow);
-    int4* ldst = reinterpret_cast<int4*>(sL);
-    for (int e = threadIdx.x; e < tcount * (lrow >> 2); e += THREADS) ldst[e] = lsrc[e];
-    const double2* csrc = reinterpret_cast<const double2*>(P.coef);
-    for (int e = threadIdx.x; e < 2 * W * D1; e += THREADS) sC[e] = csrc[e];
+  // One thread arms the mbarrier and issues three bulk copies (sigma tile, link rows, coupling
+  // factors) plus L2 prefetches of the y / acc ranges the epilogue will stream.
+  if (threadIdx.x == 0) mbar_init(bar, 1);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const unsigned bx = (unsigned)tcount * NN * 16, bl = (unsigned)tcount * lrow * 4, bc = (unsigned)W * D1 * 32;
+    mbar_expect_tx(bar, bx + bl + bc);
+    bulk_g2s(sX, p.x + (size_t)t0 * p.stride, bx, bar);
+    bulk_g2s(sL, P.links + (size_t)t0 * lrow, bl, bar);
+    bulk_g2s(sC, P.coef, bc, bar);
     if (!p.rhs_only) {
-      const size_t off = (size_t)t0 * p.stride;
-      const int lines = (tcount * NN * 16 + 127) >> 7;
-      for (int e = threadIdx.x; e < lines; e += THREADS) {
-        prefetch_l2h(reinterpret_cast<const char*>(p.acc_in + off) + ((size_t)e << 7));
-        if (p.out_x) prefetch_l2h(reinterpret_cast<const char*>(p.y + off) + ((size_t)e << 7));
-      }
+      bulk_prefetch_l2(p.acc_in + (size_t)t0 * p.stride, bx);
+      if (p.out_x) bulk_prefetch_l2(p.y + (size_t)t0 * p.stride, bx);
     }
   }
-  __syncthreads();
-
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane / N, j = lane - g * N;
   double2* myK = sK + warp * (G * NN);
   const double my_delta = P.delta[j];
+  mbar_wait(bar, 0);
 
   for (int pass = 0; pass < C::PASSES; ++pass) {
     const int first = (pass * WARPS + warp) * G;
@@ -99,75 +137,91 @@ rhs_herm_kernel(const __grid_constant__ HermParams<N> P) {
     const int s = t0 + tl;
     const double2* sig = sX + (size_t)tl * NN;
 
-    // ---- Z = -(i/hbar) H sigma, column j ------------------------------------------------------
-    double2 col[N], z[N];
+    // ---- Z = -(i/hbar) H sigma - (d_u + T)/2 o sigma, column j ------------------------------------
+    // (Z + Z^dagger then carries the full damping/terminator term, Eq. 13-14, exactly symmetrically)
+    double2 z[N];
+    {
+      double2 col[N];
 #pragma unroll
-    for (int m = 0; m < N; ++m) col[m] = sig[m * N + j];
+      for (int m = 0; m < N; ++m) col[m] = sig[m * N + j];
+      const double dd = p.damp[s];
 #pragma unroll
-    for (int b = 0; b < N; ++b) {
-      double zr = 0.0, zi = 0.0;
+      for (int b = 0; b < N; ++b) {
+        double zr = 0.0, zi = 0.0;
 #pragma unroll
-      for (int m = 0; m < N; ++m) { zr = fma(P.H[b * N + m], col[m].x, zr); zi = fma(P.H[b * N + m], col[m].y, zi); }
-      z[b] = make_double2(zi * p.inv_hbar, -zr * p.inv_hbar);
+        for (int m = 0; m < N; ++m) { zr = fma(P.H[b * N + m], col[m].x, zr); zi = fma(P.H[b * N + m], col[m].y, zi); }
+        const double hd = -0.5 * (dd + ((b == j) ? 0.0 : P.delta[b] + my_delta));
+        z[b].x = fma(hd, col[b].x, zi * p.inv_hbar);
+        z[b].y = fma(hd, col[b].y, -zr * p.inv_hbar);
+      }
     }
 
     // ---- couplings: row b of sigma_{u +- e_l}, element j (Eq. 15-17 / 35-36, Eq. 23, 25) -------
-    auto nb = [&](int idx) -> const double2* {
+    const double2* xg = p.x;
+    const int stride = p.stride;
+    auto nb = [&](int idx, int off) -> const double2* {
       const unsigned loc = (unsigned)(idx - t0);
-      return loc < (unsigned)tcount ? sX + (size_t)loc * NN : p.x + (size_t)idx * p.stride;
+      return (loc < (unsigned)tcount ? sX + (size_t)loc * NN : xg + (size_t)idx * stride) + off;
     };
     for (int kk = 0; kk < M; ++kk) {
       const int32_t* grp = sL + tl * lrow + kk * C::GROUP;
-      int up[NP4], dn[NP4];
       unsigned nbytes[NB8 / 4];
-#pragma unroll
-      for (int q = 0; q < NP4 / 4; ++q) {
-        const int4 a = reinterpret_cast<const int4*>(grp)[q];
-        const int4 c = reinterpret_cast<const int4*>(grp + NP4)[q];
-        up[4 * q] = a.x; up[4 * q + 1] = a.y; up[4 * q + 2] = a.z; up[4 * q + 3] = a.w;
-        dn[4 * q] = c.x; dn[4 * q + 1] = c.y; dn[4 * q + 2] = c.z; dn[4 * q + 3] = c.w;
-      }
 #pragma unroll
       for (int q = 0; q < NB8 / 8; ++q) {
         const uint2 t = reinterpret_cast<const uint2*>(grp + 2 * NP4)[q];
         nbytes[2 * q] = t.x; nbytes[2 * q + 1] = t.y;
       }
-      double2 wu[N], wd[N], c01[N], c23[N];
+      {  // "+" links: i a+ sigma^+[b][j]
+        int up[NP4];
 #pragma unroll
-      for (int b = 0; b < N; ++b) {
-        const int n = (nbytes[b >> 2] >> (8 * (b & 3))) & 0xff;
-        const double2* rec = sC + 2 * ((b * M + kk) * D1 + n);
-        c01[b] = rec[0];   // a+, a-x
-        c23[b] = rec[1];   // a-o, 0
-        wu[b] = make_double2(0.0, 0.0);
-        wd[b] = make_double2(0.0, 0.0);
-        if (up[b] >= 0) wu[b] = nb(up[b])[b * N + j];
-        if (dn[b] >= 0) wd[b] = nb(dn[b])[b * N + j];
+        for (int q = 0; q < NP4 / 4; ++q) {
+          const int4 a = reinterpret_cast<const int4*>(grp)[q];
+          up[4 * q] = a.x; up[4 * q + 1] = a.y; up[4 * q + 2] = a.z; up[4 * q + 3] = a.w;
+        }
+        double2 w[N];
+#pragma unroll
+        for (int b = 0; b < N; ++b) w[b] = ld_if(nb(up[b], b * N + j), up[b] >= 0);
+#pragma unroll
+        for (int b = 0; b < N; ++b) {
+          const int n = (nbytes[b >> 2] >> (8 * (b & 3))) & 0xff;
+          const double a = sC[2 * ((b * M + kk) * D1 + n)].x;
+          z[b].x = fma(-a, w[b].y, z[b].x); z[b].y = fma(a, w[b].x, z[b].y);
+        }
       }
+      {  // "-" links: (i a-x + a-o) sigma^-[b][j]
+        int dn[NP4];
 #pragma unroll
-      for (int b = 0; b < N; ++b) {
-        const double a = c01[b].x, ax = c01[b].y, ao = c23[b].x;
-        z[b].x = fma(-a, wu[b].y, z[b].x); z[b].y = fma(a, wu[b].x, z[b].y);
-        z[b].x = fma(ao, wd[b].x, fma(-ax, wd[b].y, z[b].x));
-        z[b].y = fma(ao, wd[b].y, fma(ax, wd[b].x, z[b].y));
+        for (int q = 0; q < NP4 / 4; ++q) {
+          const int4 c = reinterpret_cast<const int4*>(grp + NP4)[q];
+          dn[4 * q] = c.x; dn[4 * q + 1] = c.y; dn[4 * q + 2] = c.z; dn[4 * q + 3] = c.w;
+        }
+        double2 w[N];
+#pragma unroll
+        for (int b = 0; b < N; ++b) w[b] = ld_if(nb(dn[b], b * N + j), dn[b] >= 0);
+#pragma unroll
+        for (int b = 0; b < N; ++b) {
+          const int n = (nbytes[b >> 2] >> (8 * (b & 3))) & 0xff;
+          const double2* rec = sC + 2 * ((b * M + kk) * D1 + n);
+          const double ax = rec[0].y, ao = rec[1].x;
+          z[b].x = fma(ao, w[b].x, fma(-ax, w[b].y, z[b].x));
+          z[b].y = fma(ao, w[b].y, fma(ax, w[b].x, z[b].y));
+        }
       }
     }
 
-    // ---- k = Z + Z^dagger - (d_u + T) o sigma, column j ------------------------------------------
+    // ---- k = Z + Z^dagger, column j -------------------------------------------------------------
     __syncwarp();
     if (active) {
 #pragma unroll
       for (int b = 0; b < N; ++b) myK[g * NN + b * N + j] = z[b];
     }
     __syncwarp();
-    const double dd = p.damp[s];
     double2 k[N];
 #pragma unroll
     for (int i = 0; i < N; ++i) {
       const double2 zt = myK[gg * NN + j * N + i];               // Z[j][i]
-      const double dt = dd + ((i == j) ? 0.0 : P.delta[i] + my_delta);   // Eq. 13 + Eq. 14/24
-      k[i].x = fma(-dt, col[i].x, z[i].x + zt.x);
-      k[i].y = fma(-dt, col[i].y, z[i].y - zt.y);
+      k[i].x = z[i].x + zt.x;
+      k[i].y = z[i].y - zt.y;
     }
     __syncwarp();
     if (active) {
@@ -211,7 +265,7 @@ template <int N>
 size_t herm_smem(int W, int D, int lrow) {
   using C = HermCfg<N>;
   return (size_t)(C::T + C::WARPS * C::G) * C::NN * sizeof(double2) + (size_t)W * (D + 1) * 32 +
-         (size_t)C::T * lrow * sizeof(int32_t);
+         (size_t)C::T * lrow * sizeof(int32_t) + 16;
 }
 
 template <int N>
