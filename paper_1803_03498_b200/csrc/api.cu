@@ -44,6 +44,12 @@ struct heom_ctx {
   int32_t* d_linksH = nullptr;
   double* d_coefH = nullptr;
   int lrowH = 0;
+  // persistent pipelined Hermitian kernel (kernels_hpipe.cu)
+  bool use_hpipe = false;
+  int32_t* d_linksP = nullptr;
+  int lrowP = 0;
+  int warps_per_cta = 0;     // option "warps_per_cta": 0 = as many as fit
+  int sms = 148;
   uint8_t* d_tuples = nullptr;
   double *d_damp = nullptr, *d_H = nullptr, *d_T = nullptr, *d_ap = nullptr, *d_amx = nullptr,
          *d_amo = nullptr, *d_scratch = nullptr;
@@ -86,7 +92,7 @@ int links_row(int W) { return (2 * W + (W + 3) / 4 + 3) / 4 * 4; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, off_linksP, total;
 };
 
 Layout layout_of(const heom_ctx* c) {
@@ -102,7 +108,7 @@ Layout layout_of(const heom_ctx* c) {
   L.off_minus = o; o += align_up(nodes * W * 4);
   L.off_slot = o; o += align_up(nodes * 4);
   L.off_tuples = o; o += align_up(nodes * W);
-  L.off_damp = o; o += align_up(nodes * 8);
+  L.off_damp = o; o += align_up((nodes + 1) * 8);
   L.off_H = o; o += align_up(N * N * 8);
   L.off_T = o; o += align_up(N * N * 8);
   L.off_ap = o; o += align_up(W * D1 * 8);
@@ -112,6 +118,7 @@ Layout layout_of(const heom_ctx* c) {
   L.off_links = o; o += align_up(nodes * (size_t)links_row((int)W) * 4);
   L.off_linksH = o; o += align_up(nodes * (size_t)herm_links_row((int)N, c->h.M) * 4);
   L.off_coefH = o; o += align_up(W * D1 * 32);
+  L.off_linksP = o; o += align_up(nodes * (size_t)hpipe_links_row((int)N, c->h.M) * 4);
   L.total = o;
   return L;
 }
@@ -141,7 +148,10 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
     ctx->ev_used += 2;
     CU(cudaEventRecord(e0, ctx->stream));
   }
-  if (ctx->use_herm && ctx->herm_opt && ctx->state_hermitian)
+  if (ctx->use_hpipe && ctx->herm_opt && ctx->state_hermitian)
+    CU(launch_rhs_hpipe(p, ctx->d_linksP, ctx->lrowP, ctx->d_coefH, ctx->H.data(), ctx->c.delta.data(),
+                        ctx->warps_per_cta, ctx->sms, ctx->stream));
+  else if (ctx->use_herm && ctx->herm_opt && ctx->state_hermitian)
     CU(launch_rhs_herm(p, ctx->d_linksH, ctx->lrowH, ctx->d_coefH, ctx->H.data(), ctx->c.delta.data(), ctx->stream));
   else if (ctx->use_rows) CU(launch_rhs_rows(p, ctx->d_links, ctx->lrow, ctx->H.data(), ctx->stream));
   else CU(launch_rhs_generic(p, ctx->stream));
@@ -200,6 +210,11 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
   const std::string s(name);
   if (s == "timing") { ctx->timing = value ? 1 : 0; return HEOM_OK; }
   if (s == "hermitian") { ctx->herm_opt = value ? 1 : 0; return HEOM_OK; }
+  if (s == "warps_per_cta") {
+    if (value < 0 || value > 32) return fail(ctx, HEOM_EINVAL, "warps_per_cta must be 0..32");
+    ctx->warps_per_cta = value;
+    return HEOM_OK;
+  }
   if (ctx->bound) return fail(ctx, HEOM_ESTATE, "option must be set before heom_bind_workspace");
   if (s == "order") {
     if (value != 0 && value != 1) return fail(ctx, HEOM_EINVAL, "order must be 0 or 1");
@@ -207,7 +222,7 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
     return HEOM_OK;
   }
   if (s == "kernel") {
-    if (value < 0 || value > 1) return fail(ctx, HEOM_EINVAL, "unknown kernel variant");
+    if (value < 0 || value > 2) return fail(ctx, HEOM_EINVAL, "unknown kernel variant");
     ctx->kernel = value;
     return HEOM_OK;
   }
@@ -276,11 +291,19 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->d_scratch = (double*)(base + L.off_scratch);
   ctx->d_links = (int32_t*)(base + L.off_links);
   ctx->lrow = links_row(ctx->h.W);
-  ctx->use_rows = ctx->kernel == 1 && rows_supported(ctx->h.N, ctx->h.W, ctx->h.D, ctx->lrow);
+  ctx->use_rows = ctx->kernel >= 1 && rows_supported(ctx->h.N, ctx->h.W, ctx->h.D, ctx->lrow);
   ctx->d_linksH = (int32_t*)(base + L.off_linksH);
   ctx->d_coefH = (double*)(base + L.off_coefH);
   ctx->lrowH = herm_links_row(ctx->h.N, ctx->h.M);
-  ctx->use_herm = ctx->kernel == 1 && herm_supported(ctx->h.N, ctx->h.W, ctx->h.D);
+  ctx->use_herm = ctx->kernel >= 1 && herm_supported(ctx->h.N, ctx->h.W, ctx->h.D);
+  ctx->d_linksP = (int32_t*)(base + L.off_linksP);
+  ctx->lrowP = hpipe_links_row(ctx->h.N, ctx->h.M);
+  ctx->use_hpipe = ctx->kernel == 1 && hpipe_supported(ctx->h.N, ctx->h.W, ctx->h.D, (long long)ctx->h.nodes);
+  {
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, ctx->device));
+    ctx->sms = prop.multiProcessorCount;
+  }
   if (!ctx->h_pinned) CU(cudaMallocHost((void**)&ctx->h_pinned, ((size_t)ctx->h.N * ctx->h.N * 2 + 8) * 8));
 
   // Device tables in STORAGE-slot order: row slot_of[u] holds the slots of u's neighbours.
@@ -307,6 +330,7 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
     CU(cudaMemcpy(ctx->d_plus, tp.data(), nodes * W * 4, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(ctx->d_minus, tm.data(), nodes * W * 4, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(ctx->d_tuples, tt.data(), nodes * W, cudaMemcpyHostToDevice));
+    CU(cudaMemset(ctx->d_damp + nodes, 0, 8));
     CU(cudaMemcpy(ctx->d_damp, damp.data(), nodes * 8, cudaMemcpyHostToDevice));
     if (ctx->use_rows) {
       const size_t lrow = (size_t)ctx->lrow;
@@ -320,6 +344,22 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
       }
       CU(cudaMemcpy(ctx->d_links, lk.data(), nodes * lrow * 4, cudaMemcpyHostToDevice));
     }
+    if (ctx->use_hpipe) {
+      const size_t lrow = (size_t)ctx->lrowP;
+      std::vector<int32_t> lk(nodes * lrow, 0);
+#pragma omp parallel for schedule(static)
+      for (int64_t s = 0; s < (int64_t)nodes; ++s)
+        hpipe_pack_links(h.N, h.M, h.D, &tp[(size_t)s * W], &tm[(size_t)s * W], &tt[(size_t)s * W], damp[(size_t)s], &lk[(size_t)s * lrow]);
+      CU(cudaMemcpy(ctx->d_linksP, lk.data(), nodes * lrow * 4, cudaMemcpyHostToDevice));
+    }
+    if (ctx->use_herm || ctx->use_hpipe) {
+      const size_t D1 = (size_t)h.D + 1;
+      std::vector<double> cf(W * D1 * 4, 0.0);
+      for (size_t q = 0; q < W * D1; ++q) {
+        cf[4 * q] = ctx->c.a_plus[q]; cf[4 * q + 1] = ctx->c.a_minus_x[q]; cf[4 * q + 2] = ctx->c.a_minus_o[q];
+      }
+      CU(cudaMemcpy(ctx->d_coefH, cf.data(), W * D1 * 32, cudaMemcpyHostToDevice));
+    }
     if (ctx->use_herm) {
       const size_t lrow = (size_t)ctx->lrowH;
       std::vector<int32_t> lk(nodes * lrow, 0);
@@ -327,12 +367,6 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
       for (int64_t s = 0; s < (int64_t)nodes; ++s)
         herm_pack_links(h.N, h.M, &tp[(size_t)s * W], &tm[(size_t)s * W], &tt[(size_t)s * W], &lk[(size_t)s * lrow]);
       CU(cudaMemcpy(ctx->d_linksH, lk.data(), nodes * lrow * 4, cudaMemcpyHostToDevice));
-      const size_t D1 = (size_t)h.D + 1;
-      std::vector<double> cf(W * D1 * 4, 0.0);
-      for (size_t q = 0; q < W * D1; ++q) {
-        cf[4 * q] = ctx->c.a_plus[q]; cf[4 * q + 1] = ctx->c.a_minus_x[q]; cf[4 * q + 2] = ctx->c.a_minus_o[q];
-      }
-      CU(cudaMemcpy(ctx->d_coefH, cf.data(), W * D1 * 32, cudaMemcpyHostToDevice));
     }
   } catch (const std::bad_alloc&) {
     return fail(ctx, HEOM_ENOMEM, "out of host memory while staging the device tables");
@@ -493,6 +527,7 @@ heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches)
 
 const char* heom_kernel_name(const heom_ctx* c) {
   if (!c) return "none";
+  if (c->use_hpipe && c->herm_opt && c->state_hermitian) return "rhs_hpipe_kernel";
   if (c->use_herm && c->herm_opt && c->state_hermitian) return "rhs_herm_kernel";
   return c->use_rows ? "rhs_rows_kernel" : "rhs_generic_kernel";
 }

@@ -1,0 +1,444 @@
+// kernels_hpipe.cu -- persistent, software-pipelined sm_100a kernel for HERMITIAN hierarchy states,
+// 2 <= N <= 16: the HEOM right-hand side (Eq. 12-17 with Eq. 23-25, 35-36) with the RK4 stage
+// combination fused into its epilogue.
+//
+// Arithmetic (as kernels_herm.cu): the hierarchical Liouvillian maps Hermitian ADOs to Hermitian ADOs,
+// so with   Z = -(i/hbar) H sigma_u - (d_u + T)/2 o sigma_u
+//               + sum_l [ i a+ P_b sigma_{u+e_l} + (i a-x + a-o) P_b sigma_{u-e_l} ]      (P_b keeps row b)
+// the right-hand side is k_u = Z + Z^dagger and only ROWS of neighbours are read.  Lane (g,j) owns
+// column j of node g of its warp (G = 32/N nodes per warp pass).  Element (j,i) is produced by exactly
+// the conjugate operations of element (i,j): the state stays bit-exactly Hermitian.
+//
+// Machine mapping -- every byte that streams goes through the TMA, only the gathers are plain loads:
+//   * one CTA per SM with few, register-rich warps; every WARP is an independent worker looping over
+//     groups of G consecutive storage slots with a grid-wide stride, with a private ring of S = 3
+//     shared-memory slots {XA, ML}, two AC buffers and a private transposition scratch;
+//   * lane 0 is the warp's producer: cp.async.bulk (global -> shared, completion on the slot's
+//     mbarrier) brings the stage input x and the nodes' meta rows (neighbour element offsets,
+//     coupling-record offsets, damping rate) 1.5 passes ahead of the arithmetic; the running sum acc
+//     goes into one of two AC buffers half a pass ahead (bulk-prefetched into L2 before that);
+//   * once a pass has its sigma columns in registers the XA region is dead and the step-start state y
+//     is bulk-loaded into it (second mbarrier) while the warp does the commutator and the gathers;
+//   * all 2*M*N neighbour-row loads of a pass are issued back to back (one L2/DRAM round trip per
+//     pass), predicated, from pre-multiplied element offsets (one IMAD.WIDE + one LDG per link);
+//   * the epilogue updates XA (next stage input) and AC (running sum) in place in shared memory and
+//     lane 0 writes them back with cp.async.bulk (shared -> global, bulk async-group).
+#include "kernels.cuh"
+
+namespace heom {
+namespace {
+
+template <int N>
+struct PipeCfg {
+  static constexpr int NN = N * N;
+  static constexpr int G = 32 / N;                    // nodes per warp pass
+  static constexpr int S = 2;                         // ring slots per warp
+  static constexpr int MAXW = (N <= 8) ? 12 : 6;      // warps per CTA (fewer if shared memory is short)
+  static constexpr int SMEM_BUDGET = 224 * 1024;
+  static constexpr int KB = (16 / N) > 0 ? (16 / N) : 1;   // mode indices kk per gather batch (<= 32 loads)
+  static constexpr int NP4 = (N + 3) / 4 * 4;         // ints per index group
+  static constexpr int NB8 = (N + 7) / 8 * 8;         // coupling-record offsets (uint16) per group
+  static constexpr int GROUP = (2 * NP4 + NB8 / 2 + 3) / 4 * 4;
+};
+
+template <int N>
+struct PipeParams {
+  RhsParams p;
+  const int32_t* links;   // [nodes][lrow]: per mode index kk: plus offsets[NP4], minus offsets[NP4], uint16
+                          // byte offsets of the (l, n_l) coupling records [NB8]; then d_u (double), padding
+  const double* coef;     // [W][D+1][4] = a+, a-x, a-o, 0   (32-byte coupling records)
+  int lrow;               // ints per links row (multiple of 4)
+  int npass;              // groups of G nodes
+  int nwarps;             // warps per CTA
+  double H[N * N];        // H / hbar, fs^-1
+  double delta[N];
+};
+
+__device__ __forceinline__ unsigned smem_u32(const void* ptr) {
+  return (unsigned)__cvta_generic_to_shared(ptr);
+}
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes,
+                                         unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, unsigned bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+               ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src_gmem, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src_gmem), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// 16-byte read-only global load of base[off], executed only for off >= 0 (a valid link); otherwise the
+// destination keeps its old contents.
+__device__ __forceinline__ void ldg_link(double2& r, const double2* base, int off) {
+  asm volatile("{\n"
+      ".reg .pred p;\n"
+      ".reg .b64 a;\n"
+      "setp.ge.s32 p, %3, 0;\n"
+      "mad.wide.s32 a, %3, 16, %2;\n"
+      "@p ld.global.nc.v2.f64 {%0, %1}, [a];\n"
+      "}\n" : "+d"(r.x), "+d"(r.y) : "l"(base), "r"(off));
+}
+
+template <int N>
+__global__ void __launch_bounds__(PipeCfg<N>::MAXW * 32, 1)
+rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
+  using C = PipeCfg<N>;
+  constexpr int NN = C::NN, G = C::G, S = C::S, KB = C::KB;
+  constexpr int NP4 = C::NP4, NB8 = C::NB8, GROUP = C::GROUP;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const RhsParams& p = P.p;
+  const int W = p.W, M = p.M, D1 = p.D + 1, lrow = P.lrow, CW = P.nwarps;
+  // shared memory per warp: S slots of {XA [G][NN] double2, ML [G][lrow] int32} and 2 AC buffers [G][NN]
+  // double2 (the one not holding this pass's running sum is the transposition scratch); then two
+  // copies of the coupling records (the second with a+ = 0, for nodes on the top level), a null meta
+  // row and the mbarriers
+  constexpr int XB = G * NN * 16;
+  const int slot_bytes = XB + G * lrow * 4;
+  const int warp_bytes = S * slot_bytes + 2 * XB;
+  const int tbl_bytes = W * D1 * 32;
+  unsigned char* sC = smem_raw + CW * warp_bytes;                             // [W*D1] records
+  unsigned char* sCz = sC + tbl_bytes;                                        // same, a+ zeroed
+  int32_t* sNull = reinterpret_cast<int32_t*>(sCz + tbl_bytes);               // [lrow]
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(sNull + lrow);
+
+  for (int e = threadIdx.x; e < W * D1; e += blockDim.x) {
+    const double2 r0 = reinterpret_cast<const double2*>(P.coef)[2 * e], r1 = reinterpret_cast<const double2*>(P.coef)[2 * e + 1];
+    reinterpret_cast<double2*>(sC)[2 * e] = r0; reinterpret_cast<double2*>(sC)[2 * e + 1] = r1;
+    reinterpret_cast<double2*>(sCz)[2 * e] = make_double2(0.0, r0.y); reinterpret_cast<double2*>(sCz)[2 * e + 1] = r1;
+  }
+  // a null meta row: every link invalid, record offsets 0 (results of such lanes are never stored)
+  for (int e = threadIdx.x; e < lrow; e += blockDim.x) sNull[e] = (e < M * GROUP && (e % GROUP) < 2 * NP4) ? -1 : 0;
+  constexpr int NBAR = 2 * S + 2;                     // per warp: barX[S], barY[S], barA[2]
+  if (threadIdx.x == 0) {
+    for (int q = 0; q < CW * NBAR; ++q) mbar_init(bars + q, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  unsigned char* ring = smem_raw + warp * warp_bytes;
+  unsigned char* acbuf = ring + S * slot_bytes;       // 2 AC buffers
+  unsigned long long* barX = bars + warp * NBAR;      // x + meta rows landed
+  unsigned long long* barY = barX + S;                // y landed (in the XA region)
+  unsigned long long* barA = barY + S;                // acc landed (in an AC buffer)
+  const int npass = P.npass;
+  const int stride = gridDim.x * CW;
+  const int q0 = blockIdx.x * CW + warp;
+
+  const bool rhs_only = p.rhs_only != 0;
+  const bool y_is_x = (p.y == p.x), acc_is_x = (p.acc_in == p.x);
+  const bool need_A = !rhs_only && !acc_is_x;
+  const bool need_Y = !rhs_only && p.out_x != nullptr && !y_is_x;
+  const bool write_x = !rhs_only && p.out_x != nullptr;
+
+  // lane 0 of every warp is its own producer
+  auto issue_x = [&](int q, int slot) {               // stage input + meta rows of pass q -> ring slot
+    const int n0 = q * G;
+    const int ncnt = min(G, p.nodes - n0);
+    unsigned char* dst = ring + slot * slot_bytes;
+    const unsigned bx = (unsigned)ncnt * NN * 16, bl = (unsigned)ncnt * lrow * 4;
+    mbar_expect_tx(barX + slot, bx + bl);
+    bulk_g2s(dst, p.x + (size_t)n0 * NN, bx, barX + slot);
+    bulk_g2s(dst + XB, P.links + (size_t)n0 * lrow, bl, barX + slot);
+    if (need_A) bulk_prefetch_l2(p.acc_in + (size_t)n0 * NN, bx);
+    if (need_Y) bulk_prefetch_l2(p.y + (size_t)n0 * NN, bx);
+  };
+  auto issue_a = [&](int q, int buf) {                // running sum of pass q -> AC buffer
+    const int n0 = q * G;
+    const unsigned bx = (unsigned)min(G, p.nodes - n0) * NN * 16;
+    mbar_expect_tx(barA + buf, bx);
+    bulk_g2s(acbuf + buf * XB, p.acc_in + (size_t)n0 * NN, bx, barA + buf);
+  };
+  if (lane == 0) {
+    if (q0 < npass) { issue_x(q0, 0); if (need_A) issue_a(q0, 0); }
+  }
+
+  const int g = lane / N, j = lane - g * N;
+  const bool lane_used = lane < G * N;
+  const double my_delta = P.delta[j];
+  const double2* xj = p.x + j;
+
+  int s = 0, ab = 0;                                  // ring slot and AC buffer of this pass
+  unsigned ph = 0, pha = 0;                           // their mbarrier phases
+  for (int q = q0; q < npass; q += stride) {
+    const int n0 = q * G;
+    const int ncnt = min(G, p.nodes - n0);
+    unsigned char* slot = ring + s * slot_bytes;
+    double2* sXA = reinterpret_cast<double2*>(slot);
+    double2* sAC = reinterpret_cast<double2*>(acbuf + ab * XB);
+    double2* scr = reinterpret_cast<double2*>(acbuf + (ab ^ 1) * XB);
+    const int32_t* sL = reinterpret_cast<const int32_t*>(slot + XB);
+    mbar_wait(barX + s, ph);
+
+    const bool active = lane_used && (g < ncnt);
+    const int tl = active ? g : 0;                  // idle lanes shadow the pass's first node
+    const double2* sig = sXA + tl * NN;
+    const int32_t* lk = active ? sL + tl * lrow : sNull;
+
+    // ---- Z = -(i/hbar) H sigma - (d_u + T)/2 o sigma, column j (Eq. 12-14) ----------------------
+    double2 z[N];
+    {
+      double2 col[N];
+#pragma unroll
+      for (int m = 0; m < N; ++m) col[m] = sig[m * N + j];
+      if (need_Y) {
+        // the sigma columns are in registers: XA is dead, stream the step-start state y into it
+        fence_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+          const unsigned bx = (unsigned)ncnt * NN * 16;
+          mbar_expect_tx(barY + s, bx);
+          bulk_g2s(sXA, p.y + (size_t)n0 * NN, bx, barY + s);
+        }
+      }
+      const double mhd = -0.5 * *reinterpret_cast<const double*>(lk + M * GROUP);   // -d_u/2 (Eq. 13)
+#pragma unroll
+      for (int b = 0; b < N; ++b) {
+        double zr = 0.0, zi = 0.0;                  // (H/hbar) sigma, element (b, j)
+#pragma unroll
+        for (int m = 0; m < N; ++m) { zr = fma(P.H[b * N + m], col[m].x, zr); zi = fma(P.H[b * N + m], col[m].y, zi); }
+        const double hd = (b == j) ? mhd : fma(-0.5, P.delta[b] + my_delta, mhd);   // Eq. 14 with Eq. 24
+        z[b].x = fma(hd, col[b].x, zi);             // -i (zr + i zi) = zi - i zr
+        z[b].y = fma(hd, col[b].y, -zr);
+      }
+    }
+
+    // ---- couplings: row b of sigma_{u +- e_l}, element j (Eq. 15-17 / 35-36, Eq. 23, 25) -------
+    // "+" links of a node are all valid (level < D) or all invalid: the top level reads its records
+    // from the copy with a+ = 0.  An invalid "-" link has n = 0 and therefore zero factors.  Either
+    // way a skipped load may leave stale finite data in w[].
+    const unsigned char* tbl = (lk[0] >= 0) ? sC : sCz;
+    bool refilled = false;
+    for (int kk0 = 0; kk0 < M; kk0 += KB) {
+      double2 w[2 * KB * N];
+#pragma unroll
+      for (int b = 0; b < 2 * KB * N; ++b) w[b] = make_double2(0.0, 0.0);
+#pragma unroll
+      for (int kb = 0; kb < KB; ++kb) {
+        const int kk = kk0 + kb;
+        if (kk < M) {
+          const int32_t* grp = lk + kk * GROUP;
+          int up[NP4], dn[NP4];
+#pragma unroll
+          for (int t = 0; t < NP4 / 4; ++t) {
+            const int4 a = reinterpret_cast<const int4*>(grp)[t];
+            up[4 * t] = a.x; up[4 * t + 1] = a.y; up[4 * t + 2] = a.z; up[4 * t + 3] = a.w;
+            const int4 c = reinterpret_cast<const int4*>(grp + NP4)[t];
+            dn[4 * t] = c.x; dn[4 * t + 1] = c.y; dn[4 * t + 2] = c.z; dn[4 * t + 3] = c.w;
+          }
+#pragma unroll
+          for (int b = 0; b < N; ++b) {
+            ldg_link(w[(2 * kb) * N + b], xj + b * N, up[b]);
+            ldg_link(w[(2 * kb + 1) * N + b], xj + b * N, dn[b]);
+          }
+        }
+      }
+      if (!refilled) {
+        // with the gathers in flight: the write-back of the previous pass has left shared memory, so
+        // its ring slot can take the next pass
+        refilled = true;
+        if (lane == 0) {
+          bulk_wait_read0();
+          if (q + stride < npass) issue_x(q + stride, s ^ 1);
+        }
+      }
+#pragma unroll
+      for (int kb = 0; kb < KB; ++kb) {
+        const int kk = kk0 + kb;
+        if (kk < M) {
+          const int32_t* grp = lk + kk * GROUP;
+          unsigned rw[NB8 / 2];
+#pragma unroll
+          for (int t = 0; t < NB8 / 8; ++t) {
+            const uint4 v = reinterpret_cast<const uint4*>(grp + 2 * NP4)[t];
+            rw[4 * t] = v.x; rw[4 * t + 1] = v.y; rw[4 * t + 2] = v.z; rw[4 * t + 3] = v.w;
+          }
+#pragma unroll
+          for (int b = 0; b < N; ++b) {
+            const unsigned ro = (b & 1) ? (rw[b >> 1] >> 16) : (rw[b >> 1] & 0xffffu);
+            const double2 r0 = *reinterpret_cast<const double2*>(tbl + ro);          // a+, a-x
+            const double ao = *reinterpret_cast<const double*>(tbl + ro + 16);       // a-o
+            const double2 wu = w[(2 * kb) * N + b], wd = w[(2 * kb + 1) * N + b];
+            z[b].x = fma(-r0.x, wu.y, z[b].x); z[b].y = fma(r0.x, wu.x, z[b].y);               // i a+ sigma^+
+            z[b].x = fma(ao, wd.x, fma(-r0.y, wd.y, z[b].x));                                  // (i a-x + a-o) sigma^-
+            z[b].y = fma(ao, wd.y, fma(r0.y, wd.x, z[b].y));
+          }
+        }
+      }
+    }
+
+    // ---- k = Z + Z^dagger, column j, through the warp's scratch ---------------------------------
+    __syncwarp();
+    if (active) {
+#pragma unroll
+      for (int b = 0; b < N; ++b) scr[g * NN + b * N + j] = z[b];
+    }
+    __syncwarp();
+    double2 k[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+      const double2 zt = scr[tl * NN + j * N + i];                 // Z[j][i]
+      k[i].x = z[i].x + zt.x;
+      k[i].y = z[i].y - zt.y;
+    }
+    if (need_A && q + stride < npass) {
+      // the scratch is free again: bring the next pass's running sum (already in L2) into it
+      fence_async_smem();
+      __syncwarp();
+      if (lane == 0) issue_a(q + stride, ab ^ 1);
+    }
+
+    // ---- fused RK4 stage epilogue, in place in shared memory ------------------------------------
+    if (need_Y) mbar_wait(barY + s, ph);
+    if (need_A) mbar_wait(barA + ab, pha);
+    if (active) {
+      double2* xa = sXA + g * NN + j;
+      double2* ac = sAC + g * NN + j;
+      if (rhs_only) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) ac[i * N] = k[i];
+      } else {
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+          const double2 yv = xa[i * N];             // y (stage 1: y = x, still in XA)
+          const double2 av = acc_is_x ? yv : ac[i * N];
+          if (write_x) xa[i * N] = make_double2(fma(p.ax, k[i].x, yv.x), fma(p.ax, k[i].y, yv.y));
+          ac[i * N] = make_double2(fma(p.bx, k[i].x, av.x), fma(p.bx, k[i].y, av.y));
+        }
+      }
+    }
+    fence_async_smem();
+    __syncwarp();
+    if (lane == 0) {
+      const unsigned bx = (unsigned)ncnt * NN * 16;
+      if (write_x) bulk_s2g(p.out_x + (size_t)n0 * NN, sXA, bx);
+      bulk_s2g(p.out_acc + (size_t)n0 * NN, sAC, bx);
+      bulk_commit();
+    }
+    if ((s ^= 1) == 0) ph ^= 1u;
+    if ((ab ^= 1) == 0) pha ^= 1u;
+  }
+  if (lane == 0) bulk_wait_all();
+}
+
+template <int N>
+size_t hpipe_smem(int W, int D, int lrow, int warps) {
+  using C = PipeCfg<N>;
+  const size_t xb = (size_t)C::G * C::NN * 16;
+  return (size_t)warps * (C::S * (xb + (size_t)C::G * lrow * 4) + 2 * xb) + 2 * (size_t)W * (D + 1) * 32 +
+         (size_t)lrow * 4 + (size_t)warps * (2 * C::S + 2) * 8;
+}
+// warps per CTA: as many as fit into the shared-memory budget (0 if not even one fits)
+template <int N>
+int hpipe_warps(int W, int D, int lrow) {
+  using C = PipeCfg<N>;
+  int w = C::MAXW;
+  while (w >= 1 && hpipe_smem<N>(W, D, lrow, w) > (size_t)C::SMEM_BUDGET) --w;
+  return w;
+}
+
+template <int N>
+cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, const double* coef,
+                           const double* H_host, const double* delta_host, int warps, int sms,
+                           cudaStream_t s) {
+  using C = PipeCfg<N>;
+  PipeParams<N> P;
+  P.p = p; P.links = links; P.coef = coef; P.lrow = lrow;
+  P.npass = (p.nodes + C::G - 1) / C::G;
+  const int wmax = hpipe_warps<N>(p.W, p.D, lrow);
+  if (wmax < 1) return cudaErrorInvalidValue;
+  P.nwarps = (warps > 0 && warps < wmax) ? warps : wmax;
+  for (int e = 0; e < N * N; ++e) P.H[e] = H_host[e] * p.inv_hbar;
+  for (int e = 0; e < N; ++e) P.delta[e] = delta_host[e];
+  const size_t smem = hpipe_smem<N>(p.W, p.D, lrow, P.nwarps);
+  static size_t configured = 0;
+  if (smem > configured) {
+    cudaError_t e = cudaFuncSetAttribute(rhs_hpipe_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = smem;
+  }
+  int grid = sms;
+  if (grid > (P.npass + P.nwarps - 1) / P.nwarps) grid = (P.npass + P.nwarps - 1) / P.nwarps;
+  if (grid < 1) grid = 1;
+  rhs_hpipe_kernel<N><<<grid, P.nwarps * 32, smem, s>>>(P);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+#define HEOM_HPIPE_ALL(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
+
+int hpipe_links_row(int N, int M) {
+  if (N < 2 || N > 16) return 0;
+  const int np4 = (N + 3) / 4 * 4, nb8 = (N + 7) / 8 * 8;
+  return M * ((2 * np4 + nb8 / 2 + 3) / 4 * 4) + 4;
+}
+
+bool hpipe_supported(int N, int W, int D, long long nodes) {
+  const int M = W / (N > 0 ? N : 1);
+  const int lrow = hpipe_links_row(N, M);
+  if (lrow == 0) return false;
+  if (nodes * (long long)N * N >= 2147483647LL) return false;   // element offsets are int32
+  if ((long long)W * (D + 1) * 32 > 65535) return false;        // record offsets are uint16
+  switch (N) {
+#define HEOM_HPIPE_CASE(n) case n: return hpipe_warps<n>(W, D, lrow) >= 2;
+    HEOM_HPIPE_ALL(HEOM_HPIPE_CASE)
+#undef HEOM_HPIPE_CASE
+    default: return false;
+  }
+}
+
+void hpipe_pack_links(int N, int M, int D, const int32_t* plus, const int32_t* minus, const uint8_t* tuple,
+                      double damp, int32_t* row) {
+  const int np4 = (N + 3) / 4 * 4, nb8 = (N + 7) / 8 * 8, group = (2 * np4 + nb8 / 2 + 3) / 4 * 4;
+  const int NN = N * N;
+  for (int kk = 0; kk < M; ++kk) {
+    int32_t* grp = row + kk * group;
+    uint16_t* rec = reinterpret_cast<uint16_t*>(grp + 2 * np4);   // byte offset of record (l, n_l), l = b*M + kk
+    for (int b = 0; b < np4; ++b) {
+      const int32_t up = (b < N) ? plus[b * M + kk] : -1, dn = (b < N) ? minus[b * M + kk] : -1;
+      grp[b] = up < 0 ? -1 : up * NN;               // pre-multiplied element offset of the neighbour
+      grp[np4 + b] = dn < 0 ? -1 : dn * NN;
+    }
+    for (int b = 0; b < nb8; ++b)
+      rec[b] = (b < N) ? (uint16_t)((((b * M + kk) * (D + 1)) + tuple[b * M + kk]) * 32) : 0;
+  }
+  double* tail = reinterpret_cast<double*>(row + M * group);    // 16-byte tail: d_u (Eq. 13), padding
+  tail[0] = damp; tail[1] = 0.0;
+}
+
+cudaError_t launch_rhs_hpipe(const RhsParams& p, const int32_t* links, int lrow, const double* coef,
+                             const double* H_host, const double* delta_host, int warps, int sms,
+                             cudaStream_t s) {
+  switch (p.N) {
+#define HEOM_HPIPE_CASE(n) case n: return launch_hpipe_t<n>(p, links, lrow, coef, H_host, delta_host, warps, sms, s);
+    HEOM_HPIPE_ALL(HEOM_HPIPE_CASE)
+#undef HEOM_HPIPE_CASE
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace heom
