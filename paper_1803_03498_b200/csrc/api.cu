@@ -49,6 +49,7 @@ struct heom_ctx {
   int32_t* d_linksP = nullptr;
   int lrowP = 0;
   int warps_per_cta = 0;     // option "warps_per_cta": 0 = as many as fit
+  int l2_fetch = 0;          // option "l2_fetch": cudaLimitMaxL2FetchGranularity in bytes, 0 = leave the default
   int sms = 148;
   uint8_t* d_tuples = nullptr;
   double *d_damp = nullptr, *d_H = nullptr, *d_T = nullptr, *d_ap = nullptr, *d_amx = nullptr,
@@ -149,8 +150,9 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
     CU(cudaEventRecord(e0, ctx->stream));
   }
   if (ctx->use_hpipe && ctx->herm_opt && ctx->state_hermitian)
-    CU(launch_rhs_hpipe(p, ctx->d_linksP, ctx->lrowP, ctx->d_coefH, ctx->H.data(), ctx->c.delta.data(),
-                        ctx->warps_per_cta, ctx->sms, ctx->stream));
+    CU(launch_rhs_hpipe(p, ctx->d_linksP, ctx->lrowP, ctx->c.a_plus.data(), ctx->c.a_minus_x.data(),
+                        ctx->c.a_minus_o.data(), ctx->H.data(), ctx->c.delta.data(), ctx->warps_per_cta,
+                        ctx->sms, ctx->stream));
   else if (ctx->use_herm && ctx->herm_opt && ctx->state_hermitian)
     CU(launch_rhs_herm(p, ctx->d_linksH, ctx->lrowH, ctx->d_coefH, ctx->H.data(), ctx->c.delta.data(), ctx->stream));
   else if (ctx->use_rows) CU(launch_rhs_rows(p, ctx->d_links, ctx->lrow, ctx->H.data(), ctx->stream));
@@ -210,6 +212,11 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
   const std::string s(name);
   if (s == "timing") { ctx->timing = value ? 1 : 0; return HEOM_OK; }
   if (s == "hermitian") { ctx->herm_opt = value ? 1 : 0; return HEOM_OK; }
+  if (s == "l2_fetch") {
+    if (value != 0 && value != 32 && value != 64 && value != 128) return fail(ctx, HEOM_EINVAL, "l2_fetch must be 0, 32, 64 or 128");
+    ctx->l2_fetch = value;
+    return HEOM_OK;
+  }
   if (s == "warps_per_cta") {
     if (value < 0 || value > 32) return fail(ctx, HEOM_EINVAL, "warps_per_cta must be 0..32");
     ctx->warps_per_cta = value;
@@ -270,6 +277,7 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   if (e != cudaSuccess || ndev <= ctx->device)
     return fail(ctx, HEOM_ECUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
   CU(cudaSetDevice(ctx->device));
+  if (ctx->l2_fetch) CU(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)ctx->l2_fetch));
   ctx->stream = (cudaStream_t)cuda_stream;
   ctx->stride = node_stride(ctx->h.N);
   ctx->state_bytes = L.state;

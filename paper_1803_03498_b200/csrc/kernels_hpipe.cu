@@ -6,52 +6,73 @@
 // so with   Z = -(i/hbar) H sigma_u - (d_u + T)/2 o sigma_u
 //               + sum_l [ i a+ P_b sigma_{u+e_l} + (i a-x + a-o) P_b sigma_{u-e_l} ]      (P_b keeps row b)
 // the right-hand side is k_u = Z + Z^dagger and only ROWS of neighbours are read.  Lane (g,j) owns
-// column j of node g of its warp (G = 32/N nodes per warp pass).  Element (j,i) is produced by exactly
+// column j of node g of its warp; a node takes LP = 2, 4, 8 or 16 lanes (the power of two >= N), so a
+// warp pass covers G = 32/LP nodes.  Element (j,i) is produced by exactly
 // the conjugate operations of element (i,j): the state stays bit-exactly Hermitian.
+// The coupling factors of Eq. 35-36 are formed as sqrt(n) * c_l: (sqrt(n), sqrt(n+1)) from a small
+// shared-memory table (one 16-byte load per link pair) and the per-mode constants c_l from the
+// constant bank.
 //
 // Machine mapping -- every byte that streams goes through the TMA, only the gathers are plain loads:
-//   * one CTA per SM with few, register-rich warps; every WARP is an independent worker looping over
-//     groups of G consecutive storage slots with a grid-wide stride, with a private ring of S = 3
-//     shared-memory slots {XA, ML}, two AC buffers and a private transposition scratch;
+//   * one CTA per SM; every WARP is an independent worker looping over groups of G consecutive storage
+//     slots with a grid-wide stride, with a private ring of S = 2 shared-memory slots {XA, ML} and two
+//     AC buffers (the one not holding this pass's running sum is the transposition scratch);
 //   * lane 0 is the warp's producer: cp.async.bulk (global -> shared, completion on the slot's
 //     mbarrier) brings the stage input x and the nodes' meta rows (neighbour element offsets,
-//     coupling-record offsets, damping rate) 1.5 passes ahead of the arithmetic; the running sum acc
-//     goes into one of two AC buffers half a pass ahead (bulk-prefetched into L2 before that);
-//   * once a pass has its sigma columns in registers the XA region is dead and the step-start state y
-//     is bulk-loaded into it (second mbarrier) while the warp does the commutator and the gathers;
+//     occupation records, damping rate) one pass ahead; the running sum acc follows half a pass ahead
+//     (bulk-prefetched into L2 before that); once a pass has its sigma columns in registers the XA
+//     region is dead and the step-start state y is bulk-loaded into it;
+//   * a quarter-warp never spans two nodes (LP lanes per node) and the scratch uses a row stride == 1
+//     (mod 8) elements, so the column reads, the transposition and the epilogue are free of bank
+//     conflicts -- the LSU data pipe, not DRAM, limits this kernel otherwise;
 //   * all 2*M*N neighbour-row loads of a pass are issued back to back (one L2/DRAM round trip per
 //     pass), predicated, from pre-multiplied element offsets (one IMAD.WIDE + one LDG per link);
 //   * the epilogue updates XA (next stage input) and AC (running sum) in place in shared memory and
 //     lane 0 writes them back with cp.async.bulk (shared -> global, bulk async-group).
 #include "kernels.cuh"
 
+#include <cmath>
+
 namespace heom {
 namespace {
+
+constexpr int kMaxModes = 64;   // W of the constant-bank coupling tables
+constexpr int kMaxSqrt = 64;    // occupation numbers 0..D+1 < kMaxSqrt
 
 template <int N>
 struct PipeCfg {
   static constexpr int NN = N * N;
-  static constexpr int G = 32 / N;                    // nodes per warp pass
+  static constexpr int LP = (N <= 2) ? 2 : (N <= 4) ? 4 : (N <= 8) ? 8 : 16;   // lanes per node
+  static constexpr int G = 32 / LP;                   // nodes per warp pass
   static constexpr int S = 2;                         // ring slots per warp
   static constexpr int MAXW = (N <= 8) ? 12 : 6;      // warps per CTA (fewer if shared memory is short)
   static constexpr int SMEM_BUDGET = 224 * 1024;
   static constexpr int KB = (16 / N) > 0 ? (16 / N) : 1;   // mode indices kk per gather batch (<= 32 loads)
   static constexpr int NP4 = (N + 3) / 4 * 4;         // ints per index group
-  static constexpr int NB8 = (N + 7) / 8 * 8;         // coupling-record offsets (uint16) per group
+  static constexpr int NB8 = (N + 7) / 8 * 8;         // occupation records (uint16) per group
   static constexpr int GROUP = (2 * NP4 + NB8 / 2 + 3) / 4 * 4;
+  static constexpr int PS = NN;                       // shared-memory node stride (double2 elements): dense
+  // transposition scratch: row stride == 1 (mod 8) elements
+  static constexpr int RS = (N >= 5) ? ((N - 1 + 7) / 8 * 8 + 1) : N;
+  static constexpr int SZ = (N - 1) * RS + N;
+  static constexpr int XB = G * PS * 16;              // bytes of an XA region
+  static constexpr int AB = G * SZ * 16;              // bytes of an AC buffer (also the scratch)
 };
 
 template <int N>
 struct PipeParams {
   RhsParams p;
   const int32_t* links;   // [nodes][lrow]: per mode index kk: plus offsets[NP4], minus offsets[NP4], uint16
-                          // byte offsets of the (l, n_l) coupling records [NB8]; then d_u (double), padding
-  const double* coef;     // [W][D+1][4] = a+, a-x, a-o, 0   (32-byte coupling records)
+                          // occupation records [NB8] = 16 (2 n_l + [the "+" link exists]), the byte offset
+                          // into the sqrt table; then d_u (double), padding
   int lrow;               // ints per links row (multiple of 4)
   int npass;              // groups of G nodes
   int nwarps;             // warps per CTA
   double H[N * N];        // H / hbar, fs^-1
   double delta[N];
+  double cP[kMaxModes];   // sqrt(s_l)                      a+(l,n)  = sqrt(n+1) cP[l]     (Eq. 35)
+  double cX[kMaxModes];   // sgn(Re c_l) sqrt(s_l)          a-x(l,n) = sqrt(n) cX[l]       (Eq. 36, V^x part)
+  double cO[kMaxModes];   // delta_k0 (lambda nu/hbar)/sqrt(s_l)   a-o(l,n) = sqrt(n) cO[l] (Eq. 36, V^o part)
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* ptr) {
@@ -74,62 +95,66 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
       "WAIT_DONE:\n"
       "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes,
-                                         unsigned long long* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+// L2 eviction priorities: the streams (y, acc, the written buffers) are read or written once per launch
+// -> evict_first; the stage input x is re-read by the neighbour gathers -> evict_last.
+__device__ __forceinline__ unsigned long long policy_evict_first() {
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
 }
-__device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, unsigned bytes) {
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-               ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes) : "memory");
+__device__ __forceinline__ unsigned long long policy_evict_last() {
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes,
+                                         unsigned long long* bar, unsigned long long pol) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+               ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, unsigned bytes, unsigned long long pol) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+               ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-__device__ __forceinline__ void bulk_prefetch_l2(const void* src_gmem, unsigned bytes) {
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src_gmem), "r"(bytes) : "memory");
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src_gmem, unsigned bytes, unsigned long long pol) {
+  asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(src_gmem), "r"(bytes), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // 16-byte read-only global load of base[off], executed only for off >= 0 (a valid link); otherwise the
 // destination keeps its old contents.
-__device__ __forceinline__ void ldg_link(double2& r, const double2* base, int off) {
+__device__ __forceinline__ void ldg_link(double2& r, const double2* base, int off, unsigned long long pol) {
   asm volatile("{\n"
       ".reg .pred p;\n"
       ".reg .b64 a;\n"
       "setp.ge.s32 p, %3, 0;\n"
       "mad.wide.s32 a, %3, 16, %2;\n"
-      "@p ld.global.nc.v2.f64 {%0, %1}, [a];\n"
-      "}\n" : "+d"(r.x), "+d"(r.y) : "l"(base), "r"(off));
+      "@p ld.global.nc.L2::cache_hint.v2.f64 {%0, %1}, [a], %4;\n"
+      "}\n" : "+d"(r.x), "+d"(r.y) : "l"(base), "r"(off), "l"(pol));
 }
 
 template <int N>
 __global__ void __launch_bounds__(PipeCfg<N>::MAXW * 32, 1)
 rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   using C = PipeCfg<N>;
-  constexpr int NN = C::NN, G = C::G, S = C::S, KB = C::KB;
-  constexpr int NP4 = C::NP4, NB8 = C::NB8, GROUP = C::GROUP;
+  constexpr int NN = C::NN, G = C::G, S = C::S, KB = C::KB, PS = C::PS, RS = C::RS, SZ = C::SZ;
+  constexpr int NP4 = C::NP4, NB8 = C::NB8, GROUP = C::GROUP, XB = C::XB, AB = C::AB;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const RhsParams& p = P.p;
-  const int W = p.W, M = p.M, D1 = p.D + 1, lrow = P.lrow, CW = P.nwarps;
-  // shared memory per warp: S slots of {XA [G][NN] double2, ML [G][lrow] int32} and 2 AC buffers [G][NN]
-  // double2 (the one not holding this pass's running sum is the transposition scratch); then two
-  // copies of the coupling records (the second with a+ = 0, for nodes on the top level), a null meta
-  // row and the mbarriers
-  constexpr int XB = G * NN * 16;
+  const int M = p.M, lrow = P.lrow, CW = P.nwarps;
+  // shared memory per warp: S slots of {XA [G][PS] double2, ML [G][lrow] int32} and 2 AC buffers; then a
+  // null meta row, the sqrt table [n][up] = (sqrt(n), up ? sqrt(n+1) : 0) and the mbarriers
   const int slot_bytes = XB + G * lrow * 4;
-  const int warp_bytes = S * slot_bytes + 2 * XB;
-  const int tbl_bytes = W * D1 * 32;
-  unsigned char* sC = smem_raw + CW * warp_bytes;                             // [W*D1] records
-  unsigned char* sCz = sC + tbl_bytes;                                        // same, a+ zeroed
-  int32_t* sNull = reinterpret_cast<int32_t*>(sCz + tbl_bytes);               // [lrow]
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(sNull + lrow);
+  const int warp_bytes = S * slot_bytes + 2 * AB;
+  int32_t* sNull = reinterpret_cast<int32_t*>(smem_raw + CW * warp_bytes);    // [lrow]
+  double2* sSQ = reinterpret_cast<double2*>(sNull + lrow);                    // [kMaxSqrt][2]
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(sSQ + 2 * kMaxSqrt);
+  for (int e = threadIdx.x; e < 2 * kMaxSqrt; e += blockDim.x)
+    sSQ[e] = make_double2(sqrt((double)(e >> 1)), (e & 1) ? sqrt((double)((e >> 1) + 1)) : 0.0);
 
-  for (int e = threadIdx.x; e < W * D1; e += blockDim.x) {
-    const double2 r0 = reinterpret_cast<const double2*>(P.coef)[2 * e], r1 = reinterpret_cast<const double2*>(P.coef)[2 * e + 1];
-    reinterpret_cast<double2*>(sC)[2 * e] = r0; reinterpret_cast<double2*>(sC)[2 * e + 1] = r1;
-    reinterpret_cast<double2*>(sCz)[2 * e] = make_double2(0.0, r0.y); reinterpret_cast<double2*>(sCz)[2 * e + 1] = r1;
-  }
-  // a null meta row: every link invalid, record offsets 0 (results of such lanes are never stored)
+  // a null meta row: every link invalid, every occupation record 0 (all coupling factors vanish)
   for (int e = threadIdx.x; e < lrow; e += blockDim.x) sNull[e] = (e < M * GROUP && (e % GROUP) < 2 * NP4) ? -1 : 0;
   constexpr int NBAR = 2 * S + 2;                     // per warp: barX[S], barY[S], barA[2]
   if (threadIdx.x == 0) {
@@ -153,31 +178,36 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   const bool need_A = !rhs_only && !acc_is_x;
   const bool need_Y = !rhs_only && p.out_x != nullptr && !y_is_x;
   const bool write_x = !rhs_only && p.out_x != nullptr;
+  const bool producer = lane == 0;
+  const unsigned long long pol_stream = policy_evict_first(), pol_keep = policy_evict_last();
 
-  // lane 0 of every warp is its own producer
+  // ---- producer side (lane 0 only) -------------------------------------------------------------
   auto issue_x = [&](int q, int slot) {               // stage input + meta rows of pass q -> ring slot
     const int n0 = q * G;
     const int ncnt = min(G, p.nodes - n0);
     unsigned char* dst = ring + slot * slot_bytes;
     const unsigned bx = (unsigned)ncnt * NN * 16, bl = (unsigned)ncnt * lrow * 4;
     mbar_expect_tx(barX + slot, bx + bl);
-    bulk_g2s(dst, p.x + (size_t)n0 * NN, bx, barX + slot);
-    bulk_g2s(dst + XB, P.links + (size_t)n0 * lrow, bl, barX + slot);
-    if (need_A) bulk_prefetch_l2(p.acc_in + (size_t)n0 * NN, bx);
-    if (need_Y) bulk_prefetch_l2(p.y + (size_t)n0 * NN, bx);
+    bulk_g2s(dst, p.x + (size_t)n0 * NN, bx, barX + slot, pol_keep);
+    bulk_g2s(dst + XB, P.links + (size_t)n0 * lrow, bl, barX + slot, pol_stream);
+    if (need_A) bulk_prefetch_l2(p.acc_in + (size_t)n0 * NN, bx, pol_stream);
+    if (need_Y) bulk_prefetch_l2(p.y + (size_t)n0 * NN, bx, pol_stream);
   };
   auto issue_a = [&](int q, int buf) {                // running sum of pass q -> AC buffer
     const int n0 = q * G;
     const unsigned bx = (unsigned)min(G, p.nodes - n0) * NN * 16;
     mbar_expect_tx(barA + buf, bx);
-    bulk_g2s(acbuf + buf * XB, p.acc_in + (size_t)n0 * NN, bx, barA + buf);
+    bulk_g2s(acbuf + buf * AB, p.acc_in + (size_t)n0 * NN, bx, barA + buf, pol_stream);
   };
-  if (lane == 0) {
-    if (q0 < npass) { issue_x(q0, 0); if (need_A) issue_a(q0, 0); }
+  if (producer && q0 < npass) {
+    issue_x(q0, 0);
+    if (need_A) issue_a(q0, 0);
   }
 
-  const int g = lane / N, j = lane - g * N;
-  const bool lane_used = lane < G * N;
+  constexpr int LP = C::LP;
+  const int g = lane / LP;
+  const bool lane_used = (lane % LP) < N;
+  const int j = lane_used ? lane % LP : 0;            // idle lanes shadow column 0 of their node
   const double my_delta = P.delta[j];
   const double2* xj = p.x + j;
 
@@ -188,14 +218,14 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     const int ncnt = min(G, p.nodes - n0);
     unsigned char* slot = ring + s * slot_bytes;
     double2* sXA = reinterpret_cast<double2*>(slot);
-    double2* sAC = reinterpret_cast<double2*>(acbuf + ab * XB);
-    double2* scr = reinterpret_cast<double2*>(acbuf + (ab ^ 1) * XB);
+    double2* sAC = reinterpret_cast<double2*>(acbuf + ab * AB);
+    double2* scr = reinterpret_cast<double2*>(acbuf + (ab ^ 1) * AB);
     const int32_t* sL = reinterpret_cast<const int32_t*>(slot + XB);
     mbar_wait(barX + s, ph);
 
     const bool active = lane_used && (g < ncnt);
     const int tl = active ? g : 0;                  // idle lanes shadow the pass's first node
-    const double2* sig = sXA + tl * NN;
+    const double2* sig = sXA + tl * PS;
     const int32_t* lk = active ? sL + tl * lrow : sNull;
 
     // ---- Z = -(i/hbar) H sigma - (d_u + T)/2 o sigma, column j (Eq. 12-14) ----------------------
@@ -211,7 +241,7 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
         if (lane == 0) {
           const unsigned bx = (unsigned)ncnt * NN * 16;
           mbar_expect_tx(barY + s, bx);
-          bulk_g2s(sXA, p.y + (size_t)n0 * NN, bx, barY + s);
+          bulk_g2s(sXA, p.y + (size_t)n0 * NN, bx, barY + s, pol_stream);
         }
       }
       const double mhd = -0.5 * *reinterpret_cast<const double*>(lk + M * GROUP);   // -d_u/2 (Eq. 13)
@@ -227,10 +257,8 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     }
 
     // ---- couplings: row b of sigma_{u +- e_l}, element j (Eq. 15-17 / 35-36, Eq. 23, 25) -------
-    // "+" links of a node are all valid (level < D) or all invalid: the top level reads its records
-    // from the copy with a+ = 0.  An invalid "-" link has n = 0 and therefore zero factors.  Either
-    // way a skipped load may leave stale finite data in w[].
-    const unsigned char* tbl = (lk[0] >= 0) ? sC : sCz;
+    // An invalid "-" link has n_l = 0, an invalid "+" link (top level) carries the record byte 0:
+    // both give a zero factor, so a skipped load contributes nothing.
     bool refilled = false;
     for (int kk0 = 0; kk0 < M; kk0 += KB) {
       double2 w[2 * KB * N];
@@ -251,8 +279,8 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
           }
 #pragma unroll
           for (int b = 0; b < N; ++b) {
-            ldg_link(w[(2 * kb) * N + b], xj + b * N, up[b]);
-            ldg_link(w[(2 * kb + 1) * N + b], xj + b * N, dn[b]);
+            ldg_link(w[(2 * kb) * N + b], xj + b * N, up[b], pol_keep);
+            ldg_link(w[(2 * kb + 1) * N + b], xj + b * N, dn[b], pol_keep);
           }
         }
       }
@@ -260,7 +288,7 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
         // with the gathers in flight: the write-back of the previous pass has left shared memory, so
         // its ring slot can take the next pass
         refilled = true;
-        if (lane == 0) {
+        if (producer) {
           bulk_wait_read0();
           if (q + stride < npass) issue_x(q + stride, s ^ 1);
         }
@@ -278,29 +306,30 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
           }
 #pragma unroll
           for (int b = 0; b < N; ++b) {
-            const unsigned ro = (b & 1) ? (rw[b >> 1] >> 16) : (rw[b >> 1] & 0xffffu);
-            const double2 r0 = *reinterpret_cast<const double2*>(tbl + ro);          // a+, a-x
-            const double ao = *reinterpret_cast<const double*>(tbl + ro + 16);       // a-o
+            const unsigned rec = (b & 1) ? (rw[b >> 1] >> 16) : (rw[b >> 1] & 0xffffu);
+            const double2 sq = *reinterpret_cast<const double2*>(reinterpret_cast<const unsigned char*>(sSQ) + rec);
+            const int l = b * M + kk;
+            const double a = sq.y * P.cP[l], ax = sq.x * P.cX[l], ao = sq.x * P.cO[l];   // sqrt(n+1)|0, sqrt(n)
             const double2 wu = w[(2 * kb) * N + b], wd = w[(2 * kb + 1) * N + b];
-            z[b].x = fma(-r0.x, wu.y, z[b].x); z[b].y = fma(r0.x, wu.x, z[b].y);               // i a+ sigma^+
-            z[b].x = fma(ao, wd.x, fma(-r0.y, wd.y, z[b].x));                                  // (i a-x + a-o) sigma^-
-            z[b].y = fma(ao, wd.y, fma(r0.y, wd.x, z[b].y));
+            z[b].x = fma(-a, wu.y, z[b].x); z[b].y = fma(a, wu.x, z[b].y);                     // i a+ sigma^+
+            z[b].x = fma(ao, wd.x, fma(-ax, wd.y, z[b].x));                                    // (i a-x + a-o) sigma^-
+            z[b].y = fma(ao, wd.y, fma(ax, wd.x, z[b].y));
           }
         }
       }
     }
 
-    // ---- k = Z + Z^dagger, column j, through the warp's scratch ---------------------------------
+    // ---- k = Z + Z^dagger, column j, through the scratch (conflict-free row stride RS) -----------
     __syncwarp();
     if (active) {
 #pragma unroll
-      for (int b = 0; b < N; ++b) scr[g * NN + b * N + j] = z[b];
+      for (int b = 0; b < N; ++b) scr[g * SZ + b * RS + j] = z[b];
     }
     __syncwarp();
     double2 k[N];
 #pragma unroll
     for (int i = 0; i < N; ++i) {
-      const double2 zt = scr[tl * NN + j * N + i];                 // Z[j][i]
+      const double2 zt = scr[tl * SZ + j * RS + i];                // Z[j][i]
       k[i].x = z[i].x + zt.x;
       k[i].y = z[i].y - zt.y;
     }
@@ -308,15 +337,15 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
       // the scratch is free again: bring the next pass's running sum (already in L2) into it
       fence_async_smem();
       __syncwarp();
-      if (lane == 0) issue_a(q + stride, ab ^ 1);
+      if (producer) issue_a(q + stride, ab ^ 1);
     }
 
     // ---- fused RK4 stage epilogue, in place in shared memory ------------------------------------
     if (need_Y) mbar_wait(barY + s, ph);
     if (need_A) mbar_wait(barA + ab, pha);
     if (active) {
-      double2* xa = sXA + g * NN + j;
-      double2* ac = sAC + g * NN + j;
+      double2* xa = sXA + g * PS + j;
+      double2* ac = sAC + g * PS + j;
       if (rhs_only) {
 #pragma unroll
         for (int i = 0; i < N; ++i) ac[i * N] = k[i];
@@ -334,46 +363,52 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     __syncwarp();
     if (lane == 0) {
       const unsigned bx = (unsigned)ncnt * NN * 16;
-      if (write_x) bulk_s2g(p.out_x + (size_t)n0 * NN, sXA, bx);
-      bulk_s2g(p.out_acc + (size_t)n0 * NN, sAC, bx);
+      if (write_x) bulk_s2g(p.out_x + (size_t)n0 * NN, sXA, bx, pol_stream);
+      bulk_s2g(p.out_acc + (size_t)n0 * NN, sAC, bx, pol_stream);
       bulk_commit();
     }
     if ((s ^= 1) == 0) ph ^= 1u;
     if ((ab ^= 1) == 0) pha ^= 1u;
   }
-  if (lane == 0) bulk_wait_all();
+  if (producer) bulk_wait_all();
 }
 
 template <int N>
-size_t hpipe_smem(int W, int D, int lrow, int warps) {
+size_t hpipe_smem(int lrow, int warps) {
   using C = PipeCfg<N>;
-  const size_t xb = (size_t)C::G * C::NN * 16;
-  return (size_t)warps * (C::S * (xb + (size_t)C::G * lrow * 4) + 2 * xb) + 2 * (size_t)W * (D + 1) * 32 +
-         (size_t)lrow * 4 + (size_t)warps * (2 * C::S + 2) * 8;
+  return (size_t)warps * (C::S * ((size_t)C::XB + (size_t)C::G * lrow * 4) + 2 * (size_t)C::AB) +
+         (size_t)lrow * 4 + 2 * kMaxSqrt * 16 + (size_t)warps * (2 * C::S + 2) * 8;
 }
 // warps per CTA: as many as fit into the shared-memory budget (0 if not even one fits)
 template <int N>
-int hpipe_warps(int W, int D, int lrow) {
+int hpipe_warps(int lrow) {
   using C = PipeCfg<N>;
   int w = C::MAXW;
-  while (w >= 1 && hpipe_smem<N>(W, D, lrow, w) > (size_t)C::SMEM_BUDGET) --w;
+  while (w >= 1 && hpipe_smem<N>(lrow, w) > (size_t)C::SMEM_BUDGET) --w;
   return w;
 }
 
 template <int N>
-cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, const double* coef,
-                           const double* H_host, const double* delta_host, int warps, int sms,
-                           cudaStream_t s) {
+cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, const double* a_plus,
+                           const double* a_minus_x, const double* a_minus_o, const double* H_host,
+                           const double* delta_host, int warps, int sms, cudaStream_t s) {
   using C = PipeCfg<N>;
   PipeParams<N> P;
-  P.p = p; P.links = links; P.coef = coef; P.lrow = lrow;
+  P.p = p; P.links = links; P.lrow = lrow;
   P.npass = (p.nodes + C::G - 1) / C::G;
-  const int wmax = hpipe_warps<N>(p.W, p.D, lrow);
+  const int wmax = hpipe_warps<N>(lrow);
   if (wmax < 1) return cudaErrorInvalidValue;
   P.nwarps = (warps > 0 && warps < wmax) ? warps : wmax;
   for (int e = 0; e < N * N; ++e) P.H[e] = H_host[e] * p.inv_hbar;
   for (int e = 0; e < N; ++e) P.delta[e] = delta_host[e];
-  const size_t smem = hpipe_smem<N>(p.W, p.D, lrow, P.nwarps);
+  const int D1 = p.D + 1;
+  for (int l = 0; l < kMaxModes; ++l) {
+    const bool on = l < p.W && p.D >= 1;
+    P.cP[l] = on ? a_plus[(size_t)l * D1] : 0.0;            // sqrt(1 * s_l)
+    P.cX[l] = on ? a_minus_x[(size_t)l * D1 + 1] : 0.0;     // sgn sqrt(1 * s_l)
+    P.cO[l] = on ? a_minus_o[(size_t)l * D1 + 1] : 0.0;     // sqrt(1 / s_l) lambda nu / hbar
+  }
+  const size_t smem = hpipe_smem<N>(lrow, P.nwarps);
   static size_t configured = 0;
   if (smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(rhs_hpipe_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -402,9 +437,9 @@ bool hpipe_supported(int N, int W, int D, long long nodes) {
   const int lrow = hpipe_links_row(N, M);
   if (lrow == 0) return false;
   if (nodes * (long long)N * N >= 2147483647LL) return false;   // element offsets are int32
-  if ((long long)W * (D + 1) * 32 > 65535) return false;        // record offsets are uint16
+  if (W > kMaxModes || D + 2 > kMaxSqrt) return false;          // constant-bank tables
   switch (N) {
-#define HEOM_HPIPE_CASE(n) case n: return hpipe_warps<n>(W, D, lrow) >= 2;
+#define HEOM_HPIPE_CASE(n) case n: return hpipe_warps<n>(lrow) >= 2;
     HEOM_HPIPE_ALL(HEOM_HPIPE_CASE)
 #undef HEOM_HPIPE_CASE
     default: return false;
@@ -415,26 +450,34 @@ void hpipe_pack_links(int N, int M, int D, const int32_t* plus, const int32_t* m
                       double damp, int32_t* row) {
   const int np4 = (N + 3) / 4 * 4, nb8 = (N + 7) / 8 * 8, group = (2 * np4 + nb8 / 2 + 3) / 4 * 4;
   const int NN = N * N;
+  (void)D;
   for (int kk = 0; kk < M; ++kk) {
     int32_t* grp = row + kk * group;
-    uint16_t* rec = reinterpret_cast<uint16_t*>(grp + 2 * np4);   // byte offset of record (l, n_l), l = b*M + kk
+    uint16_t* rec = reinterpret_cast<uint16_t*>(grp + 2 * np4);   // 16 (2 n_l + ["+" link exists])
     for (int b = 0; b < np4; ++b) {
       const int32_t up = (b < N) ? plus[b * M + kk] : -1, dn = (b < N) ? minus[b * M + kk] : -1;
       grp[b] = up < 0 ? -1 : up * NN;               // pre-multiplied element offset of the neighbour
       grp[np4 + b] = dn < 0 ? -1 : dn * NN;
     }
-    for (int b = 0; b < nb8; ++b)
-      rec[b] = (b < N) ? (uint16_t)((((b * M + kk) * (D + 1)) + tuple[b * M + kk]) * 32) : 0;
+    for (int b = 0; b < nb8; ++b) {
+      if (b < N) {
+        const unsigned n = tuple[b * M + kk];
+        rec[b] = (uint16_t)(16u * (2u * n + (plus[b * M + kk] >= 0 ? 1u : 0u)));
+      } else {
+        rec[b] = 0;
+      }
+    }
   }
   double* tail = reinterpret_cast<double*>(row + M * group);    // 16-byte tail: d_u (Eq. 13), padding
   tail[0] = damp; tail[1] = 0.0;
 }
 
-cudaError_t launch_rhs_hpipe(const RhsParams& p, const int32_t* links, int lrow, const double* coef,
-                             const double* H_host, const double* delta_host, int warps, int sms,
-                             cudaStream_t s) {
+cudaError_t launch_rhs_hpipe(const RhsParams& p, const int32_t* links, int lrow, const double* a_plus,
+                             const double* a_minus_x, const double* a_minus_o, const double* H_host,
+                             const double* delta_host, int warps, int sms, cudaStream_t s) {
   switch (p.N) {
-#define HEOM_HPIPE_CASE(n) case n: return launch_hpipe_t<n>(p, links, lrow, coef, H_host, delta_host, warps, sms, s);
+#define HEOM_HPIPE_CASE(n) \
+  case n: return launch_hpipe_t<n>(p, links, lrow, a_plus, a_minus_x, a_minus_o, H_host, delta_host, warps, sms, s);
     HEOM_HPIPE_ALL(HEOM_HPIPE_CASE)
 #undef HEOM_HPIPE_CASE
     default: return cudaErrorInvalidValue;
