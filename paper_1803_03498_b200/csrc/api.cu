@@ -49,6 +49,8 @@ struct heom_ctx {
   int32_t* d_linksP = nullptr;
   int lrowP = 0;
   int warps_per_cta = 0;     // option "warps_per_cta": 0 = as many as fit
+  unsigned long long* d_tickets = nullptr;   // work counter of the persistent kernel
+  unsigned long long ticket_base = 0;
   int l2_fetch = 0;          // option "l2_fetch": cudaLimitMaxL2FetchGranularity in bytes, 0 = leave the default
   int sms = 148;
   uint8_t* d_tuples = nullptr;
@@ -115,7 +117,7 @@ Layout layout_of(const heom_ctx* c) {
   L.off_ap = o; o += align_up(W * D1 * 8);
   L.off_amx = o; o += align_up(W * D1 * 8);
   L.off_amo = o; o += align_up(W * D1 * 8);
-  L.off_scratch = o; o += align_up((N + 2) * 8);
+  L.off_scratch = o; o += align_up((N + 2) * 8 + 128);
   L.off_links = o; o += align_up(nodes * (size_t)links_row((int)W) * 4);
   L.off_linksH = o; o += align_up(nodes * (size_t)herm_links_row((int)N, c->h.M) * 4);
   L.off_coefH = o; o += align_up(W * D1 * 32);
@@ -152,7 +154,7 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
   if (ctx->use_hpipe && ctx->herm_opt && ctx->state_hermitian)
     CU(launch_rhs_hpipe(p, ctx->d_linksP, ctx->lrowP, ctx->c.a_plus.data(), ctx->c.a_minus_x.data(),
                         ctx->c.a_minus_o.data(), ctx->H.data(), ctx->c.delta.data(), ctx->warps_per_cta,
-                        ctx->sms, ctx->stream));
+                        ctx->sms, ctx->d_tickets, &ctx->ticket_base, ctx->stream));
   else if (ctx->use_herm && ctx->herm_opt && ctx->state_hermitian)
     CU(launch_rhs_herm(p, ctx->d_linksH, ctx->lrowH, ctx->d_coefH, ctx->H.data(), ctx->c.delta.data(), ctx->stream));
   else if (ctx->use_rows) CU(launch_rhs_rows(p, ctx->d_links, ctx->lrow, ctx->H.data(), ctx->stream));
@@ -297,6 +299,9 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->d_amx = (double*)(base + L.off_amx);
   ctx->d_amo = (double*)(base + L.off_amo);
   ctx->d_scratch = (double*)(base + L.off_scratch);
+  ctx->d_tickets = (unsigned long long*)(base + L.off_scratch + (((size_t)ctx->h.N + 2) * 8 + 63) / 64 * 64);
+  ctx->ticket_base = 0;
+  CU(cudaMemset(ctx->d_tickets, 0, 8));
   ctx->d_links = (int32_t*)(base + L.off_links);
   ctx->lrow = links_row(ctx->h.W);
   ctx->use_rows = ctx->kernel >= 1 && rows_supported(ctx->h.N, ctx->h.W, ctx->h.D, ctx->lrow);

@@ -58,14 +58,16 @@ cudaError_t launch_rhs_herm(const RhsParams& p, const int32_t* links, int lrow, 
 // [nodes][lrow] int32 written by hpipe_pack_links (neighbour entries are element offsets slot*N*N, uint16
 // occupation records, and the row ends with the node's damping rate).  a_plus, a_minus_x, a_minus_o,
 // H_host, delta_host: HOST (the per-mode constants travel in the kernel parameters).  warps <= 0: as
-// many warps per CTA as shared memory allows; grid = one CTA per SM.
+// many warps per CTA as shared memory allows; grid = one CTA per SM.  tickets: DEVICE counter (zeroed once);
+// *ticket_base: HOST running total of the tickets drawn by earlier launches (updated here).
 int hpipe_links_row(int N, int M);
 bool hpipe_supported(int N, int W, int D, long long nodes);
 void hpipe_pack_links(int N, int M, int D, const int32_t* plus, const int32_t* minus, const uint8_t* tuple,
                       double damp, int32_t* row);
 cudaError_t launch_rhs_hpipe(const RhsParams& p, const int32_t* links, int lrow, const double* a_plus,
                              const double* a_minus_x, const double* a_minus_o, const double* H_host,
-                             const double* delta_host, int warps, int sms, cudaStream_t s);
+                             const double* delta_host, int warps, int sms, unsigned long long* tickets,
+                             unsigned long long* ticket_base, cudaStream_t s);
 
 // dst[slot_of[u]*dst_stride + e] = src[u*NN + e]  (to_device=1) or the inverse (to_device=0)
 cudaError_t launch_permute(const double2* src, double2* dst, const int32_t* slot_of, int nodes,

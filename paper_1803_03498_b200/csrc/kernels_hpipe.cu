@@ -14,9 +14,11 @@
 // constant bank.
 //
 // Machine mapping -- every byte that streams goes through the TMA, only the gathers are plain loads:
-//   * one CTA per SM; every WARP is an independent worker looping over groups of G consecutive storage
-//     slots with a grid-wide stride, with a private ring of S = 2 shared-memory slots {XA, ML} and two
-//     AC buffers (the one not holding this pass's running sum is the transposition scratch);
+//   * one CTA per SM; every WARP is an independent worker that draws groups of G consecutive storage
+//     slots from a global ticket counter (so the groups in flight always form one compact window of
+//     the state, which is what keeps the neighbour gathers in L2), with a private ring of S = 2
+//     shared-memory slots {XA, ML} and two AC buffers (the one not holding this pass's running sum is
+//     the transposition scratch);
 //   * lane 0 is the warp's producer: cp.async.bulk (global -> shared, completion on the slot's
 //     mbarrier) brings the stage input x and the nodes' meta rows (neighbour element offsets,
 //     occupation records, damping rate) one pass ahead; the running sum acc follows half a pass ahead
@@ -68,6 +70,8 @@ struct PipeParams {
   int lrow;               // ints per links row (multiple of 4)
   int npass;              // groups of G nodes
   int nwarps;             // warps per CTA
+  unsigned long long* tickets;   // DEVICE ticket counter; pass index = ticket - ticket_base
+  unsigned long long ticket_base;
   double H[N * N];        // H / hbar, fs^-1
   double delta[N];
   double cP[kMaxModes];   // sqrt(s_l)                      a+(l,n)  = sqrt(n+1) cP[l]     (Eq. 35)
@@ -170,8 +174,6 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   unsigned long long* barY = barX + S;                // y landed (in the XA region)
   unsigned long long* barA = barY + S;                // acc landed (in an AC buffer)
   const int npass = P.npass;
-  const int stride = gridDim.x * CW;
-  const int q0 = blockIdx.x * CW + warp;
 
   const bool rhs_only = p.rhs_only != 0;
   const bool y_is_x = (p.y == p.x), acc_is_x = (p.acc_in == p.x);
@@ -199,10 +201,20 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     mbar_expect_tx(barA + buf, bx);
     bulk_g2s(acbuf + buf * AB, p.acc_in + (size_t)n0 * NN, bx, barA + buf, pol_stream);
   };
-  if (producer && q0 < npass) {
-    issue_x(q0, 0);
-    if (need_A) issue_a(q0, 0);
+  // next group of this warp: one ticket per pass, drawn by lane 0 (values >= npass: no more work)
+  auto draw = [&]() -> int {
+    const unsigned long long t = atomicAdd(P.tickets, 1ULL) - P.ticket_base;
+    return t < (unsigned long long)npass ? (int)t : npass;
+  };
+  int q = 0;
+  if (producer) {
+    q = draw();
+    if (q < npass) {
+      issue_x(q, 0);
+      if (need_A) issue_a(q, 0);
+    }
   }
+  q = __shfl_sync(0xffffffffu, q, 0);
 
   constexpr int LP = C::LP;
   const int g = lane / LP;
@@ -213,7 +225,9 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
 
   int s = 0, ab = 0;                                  // ring slot and AC buffer of this pass
   unsigned ph = 0, pha = 0;                           // their mbarrier phases
-  for (int q = q0; q < npass; q += stride) {
+  while (q < npass) {
+    int qn = 0;                                     // the pass after this one
+    if (producer) qn = draw();
     const int n0 = q * G;
     const int ncnt = min(G, p.nodes - n0);
     unsigned char* slot = ring + s * slot_bytes;
@@ -290,8 +304,9 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
         refilled = true;
         if (producer) {
           bulk_wait_read0();
-          if (q + stride < npass) issue_x(q + stride, s ^ 1);
+          if (qn < npass) issue_x(qn, s ^ 1);
         }
+        qn = __shfl_sync(0xffffffffu, qn, 0);
       }
 #pragma unroll
       for (int kb = 0; kb < KB; ++kb) {
@@ -333,11 +348,11 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
       k[i].x = z[i].x + zt.x;
       k[i].y = z[i].y - zt.y;
     }
-    if (need_A && q + stride < npass) {
+    if (need_A && qn < npass) {
       // the scratch is free again: bring the next pass's running sum (already in L2) into it
       fence_async_smem();
       __syncwarp();
-      if (producer) issue_a(q + stride, ab ^ 1);
+      if (producer) issue_a(qn, ab ^ 1);
     }
 
     // ---- fused RK4 stage epilogue, in place in shared memory ------------------------------------
@@ -369,6 +384,7 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     }
     if ((s ^= 1) == 0) ph ^= 1u;
     if ((ab ^= 1) == 0) pha ^= 1u;
+    q = qn;
   }
   if (producer) bulk_wait_all();
 }
@@ -391,7 +407,8 @@ int hpipe_warps(int lrow) {
 template <int N>
 cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, const double* a_plus,
                            const double* a_minus_x, const double* a_minus_o, const double* H_host,
-                           const double* delta_host, int warps, int sms, cudaStream_t s) {
+                           const double* delta_host, int warps, int sms, unsigned long long* tickets,
+                           unsigned long long* ticket_base, cudaStream_t s) {
   using C = PipeCfg<N>;
   PipeParams<N> P;
   P.p = p; P.links = links; P.lrow = lrow;
@@ -418,6 +435,9 @@ cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, c
   int grid = sms;
   if (grid > (P.npass + P.nwarps - 1) / P.nwarps) grid = (P.npass + P.nwarps - 1) / P.nwarps;
   if (grid < 1) grid = 1;
+  P.tickets = tickets;
+  P.ticket_base = *ticket_base;
+  *ticket_base += (unsigned long long)P.npass + (unsigned long long)grid * P.nwarps;   // one failing draw per warp
   rhs_hpipe_kernel<N><<<grid, P.nwarps * 32, smem, s>>>(P);
   return cudaGetLastError();
 }
@@ -474,10 +494,11 @@ void hpipe_pack_links(int N, int M, int D, const int32_t* plus, const int32_t* m
 
 cudaError_t launch_rhs_hpipe(const RhsParams& p, const int32_t* links, int lrow, const double* a_plus,
                              const double* a_minus_x, const double* a_minus_o, const double* H_host,
-                             const double* delta_host, int warps, int sms, cudaStream_t s) {
+                             const double* delta_host, int warps, int sms, unsigned long long* tickets,
+                             unsigned long long* ticket_base, cudaStream_t s) {
   switch (p.N) {
 #define HEOM_HPIPE_CASE(n) \
-  case n: return launch_hpipe_t<n>(p, links, lrow, a_plus, a_minus_x, a_minus_o, H_host, delta_host, warps, sms, s);
+  case n: return launch_hpipe_t<n>(p, links, lrow, a_plus, a_minus_x, a_minus_o, H_host, delta_host, warps, sms, tickets, ticket_base, s);
     HEOM_HPIPE_ALL(HEOM_HPIPE_CASE)
 #undef HEOM_HPIPE_CASE
     default: return cudaErrorInvalidValue;
