@@ -49,8 +49,15 @@ struct heom_ctx {
   int32_t* d_linksP = nullptr;
   int lrowP = 0;
   int warps_per_cta = 0;     // option "warps_per_cta": 0 = as many as fit
+  // tensor-core kernel for large N (kernels_large.cu)
+  bool use_large = false;
+  int64_t* d_lptr = nullptr;
+  void* d_lent = nullptr;
+  double *d_Hs = nullptr, *d_delta = nullptr;
+  size_t n_links = 0;
   unsigned long long* d_tickets = nullptr;   // work counter of the persistent kernel
   unsigned long long ticket_base = 0;
+  int rk4_form = -1;         // option "rk4_form": 0 classical stages, 1 Taylor/Horner (large-N kernel only), -1 auto
   int l2_fetch = 0;          // option "l2_fetch": cudaLimitMaxL2FetchGranularity in bytes, 0 = leave the default
   int sms = 148;
   uint8_t* d_tuples = nullptr;
@@ -95,7 +102,7 @@ int links_row(int W) { return (2 * W + (W + 3) / 4 + 3) / 4 * 4; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, off_linksP, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, off_linksP, off_Hs, off_delta, off_lptr, off_lent, total;
 };
 
 Layout layout_of(const heom_ctx* c) {
@@ -122,6 +129,15 @@ Layout layout_of(const heom_ctx* c) {
   L.off_linksH = o; o += align_up(nodes * (size_t)herm_links_row((int)N, c->h.M) * 4);
   L.off_coefH = o; o += align_up(W * D1 * 32);
   L.off_linksP = o; o += align_up(nodes * (size_t)hpipe_links_row((int)N, c->h.M) * 4);
+  L.off_Hs = o; o += align_up(N * N * 8);
+  L.off_delta = o; o += align_up(N * 8);
+  if (large_supported((int)N, (int)W)) {
+    // every valid link appears once as "+" and once as "-": count the "-" links of the host table
+    size_t links = 0;
+    for (size_t q = 0; q < c->h.minus.size(); ++q) links += c->h.minus[q] >= 0;
+    L.off_lptr = o; o += align_up((nodes + 1) * 8);
+    L.off_lent = o; o += align_up(2 * links * 16 + 16);
+  }
   L.total = o;
   return L;
 }
@@ -151,7 +167,11 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
     ctx->ev_used += 2;
     CU(cudaEventRecord(e0, ctx->stream));
   }
-  if (ctx->use_hpipe && ctx->herm_opt && ctx->state_hermitian)
+  if (ctx->use_large)
+    CU(launch_rhs_large(p, ctx->d_lptr, ctx->d_lent, ctx->d_Hs, ctx->d_delta, ctx->c.a_plus.data(),
+                        ctx->c.a_minus_x.data(), ctx->c.a_minus_o.data(), ctx->sms, ctx->d_tickets,
+                        &ctx->ticket_base, ctx->stream));
+  else if (ctx->use_hpipe && ctx->herm_opt && ctx->state_hermitian)
     CU(launch_rhs_hpipe(p, ctx->d_linksP, ctx->lrowP, ctx->c.a_plus.data(), ctx->c.a_minus_x.data(),
                         ctx->c.a_minus_o.data(), ctx->H.data(), ctx->c.delta.data(), ctx->warps_per_cta,
                         ctx->sms, ctx->d_tickets, &ctx->ticket_base, ctx->stream));
@@ -217,6 +237,11 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
   if (s == "l2_fetch") {
     if (value != 0 && value != 32 && value != 64 && value != 128) return fail(ctx, HEOM_EINVAL, "l2_fetch must be 0, 32, 64 or 128");
     ctx->l2_fetch = value;
+    return HEOM_OK;
+  }
+  if (s == "rk4_form") {
+    if (value < -1 || value > 1) return fail(ctx, HEOM_EINVAL, "rk4_form must be -1, 0 or 1");
+    ctx->rk4_form = value;
     return HEOM_OK;
   }
   if (s == "warps_per_cta") {
@@ -309,6 +334,11 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->d_coefH = (double*)(base + L.off_coefH);
   ctx->lrowH = herm_links_row(ctx->h.N, ctx->h.M);
   ctx->use_herm = ctx->kernel >= 1 && herm_supported(ctx->h.N, ctx->h.W, ctx->h.D);
+  ctx->use_large = ctx->kernel == 1 && large_supported(ctx->h.N, ctx->h.W);
+  ctx->d_Hs = (double*)(base + L.off_Hs);
+  ctx->d_delta = (double*)(base + L.off_delta);
+  ctx->d_lptr = (int64_t*)(base + L.off_lptr);
+  ctx->d_lent = (void*)(base + L.off_lent);
   ctx->d_linksP = (int32_t*)(base + L.off_linksP);
   ctx->lrowP = hpipe_links_row(ctx->h.N, ctx->h.M);
   ctx->use_hpipe = ctx->kernel == 1 && hpipe_supported(ctx->h.N, ctx->h.W, ctx->h.D, (long long)ctx->h.nodes);
@@ -356,6 +386,31 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
         std::memcpy(row + 2 * W, &tt[(size_t)s * W], W);
       }
       CU(cudaMemcpy(ctx->d_links, lk.data(), nodes * lrow * 4, cudaMemcpyHostToDevice));
+    }
+    if (ctx->use_large) {
+      // CSR link list in storage-slot order: "+" links first, then "-" links, of every node
+      std::vector<int64_t> lptr(nodes + 1, 0);
+      for (size_t s = 0; s < nodes; ++s) {
+        int64_t cnt = 0;
+        for (size_t l = 0; l < W; ++l) cnt += (tp[s * W + l] >= 0) + (tm[s * W + l] >= 0);
+        lptr[s + 1] = lptr[s] + cnt;
+      }
+      std::vector<int32_t> lent((size_t)lptr[nodes] * 4 + 4, 0);
+#pragma omp parallel for schedule(static)
+      for (int64_t s = 0; s < (int64_t)nodes; ++s) {
+        int32_t* e = &lent[(size_t)lptr[(size_t)s] * 4];
+        for (size_t l = 0; l < W; ++l)
+          if (tp[(size_t)s * W + l] >= 0) { e[0] = tp[(size_t)s * W + l]; e[1] = (int32_t)l; e[2] = 0; e[3] = tt[(size_t)s * W + l]; e += 4; }
+        for (size_t l = 0; l < W; ++l)
+          if (tm[(size_t)s * W + l] >= 0) { e[0] = tm[(size_t)s * W + l]; e[1] = (int32_t)l; e[2] = 1; e[3] = tt[(size_t)s * W + l]; e += 4; }
+      }
+      ctx->n_links = (size_t)lptr[nodes];
+      CU(cudaMemcpy(ctx->d_lptr, lptr.data(), (nodes + 1) * 8, cudaMemcpyHostToDevice));
+      CU(cudaMemcpy(ctx->d_lent, lent.data(), (size_t)lptr[nodes] * 16 + 16, cudaMemcpyHostToDevice));
+      std::vector<double> Hs(ctx->H);
+      for (double& v : Hs) v *= 1.0 / kHbar;
+      CU(cudaMemcpy(ctx->d_Hs, Hs.data(), Hs.size() * 8, cudaMemcpyHostToDevice));
+      CU(cudaMemcpy(ctx->d_delta, ctx->c.delta.data(), (size_t)h.N * 8, cudaMemcpyHostToDevice));
     }
     if (ctx->use_hpipe) {
       const size_t lrow = (size_t)ctx->lrowP;
@@ -483,6 +538,27 @@ heom_status heom_rk4_steps(heom_ctx* ctx, double dt, int nsteps) {
   if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
   RhsParams p = base_params(ctx);
   p.rhs_only = 0;
+  if (ctx->use_large && ctx->rk4_form != 0) {
+    /* Taylor/Horner form (R6): v1 = dt f(y), v_s = (dt/s) f(v_{s-1}), y' = y + v1 + v2 + v3 + v4 -- the
+     * classical RK4 result for a linear autonomous f, regrouped.  acc = y + v1 is stored, v2..v4 are
+     * added to it by global reductions; y and acc then swap roles.  14 instead of 16 state sizes. */
+    for (int step = 0; step < nsteps; ++step) {
+      heom_status s;
+      p.taylor = 1;
+      p.x = ctx->y; p.y = nullptr; p.acc_in = ctx->y; p.out_x = ctx->xa; p.out_acc = ctx->acc;
+      p.ax = dt; p.bx = dt; p.acc_red = 0;
+      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+      p.acc_red = 1; p.acc_in = nullptr;
+      p.x = ctx->xa; p.out_x = ctx->xb; p.ax = p.bx = dt / 2.0;
+      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+      p.x = ctx->xb; p.out_x = ctx->xa; p.ax = p.bx = dt / 3.0;
+      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+      p.x = ctx->xa; p.out_x = nullptr; p.ax = p.bx = dt / 4.0;
+      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+      double2* tmp = ctx->y; ctx->y = ctx->acc; ctx->acc = tmp;
+    }
+    return HEOM_OK;
+  }
   for (int step = 0; step < nsteps; ++step) {
     heom_status s;
     p.x = ctx->y; p.y = ctx->y; p.acc_in = ctx->y; p.out_x = ctx->xa; p.out_acc = ctx->acc;
@@ -540,6 +616,7 @@ heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches)
 
 const char* heom_kernel_name(const heom_ctx* c) {
   if (!c) return "none";
+  if (c->use_large) return "rhs_large_kernel";
   if (c->use_hpipe && c->herm_opt && c->state_hermitian) return "rhs_hpipe_kernel";
   if (c->use_herm && c->herm_opt && c->state_hermitian) return "rhs_herm_kernel";
   return c->use_rows ? "rhs_rows_kernel" : "rhs_generic_kernel";

@@ -31,6 +31,10 @@ struct RhsParams {
   double2* out_acc;       // acc_in + bx*k     (or, in RHS-only mode, k itself)
   double ax, bx;
   int rhs_only;           // 1: out_acc = k, nothing else read or written
+  // Taylor/Horner form of RK4 for a linear autonomous right-hand side (R6); honoured by the
+  // large-N kernel only (the others are always launched with both flags 0):
+  int taylor;             // 1: out_x = ax*k (y is not read)
+  int acc_red;            // 1: out_acc += bx*k by fire-and-forget global reductions (acc_in is not read)
 };
 
 // Generic kernel: any N <= 96, one thread per matrix element.
@@ -67,6 +71,15 @@ void hpipe_pack_links(int N, int M, int D, const int32_t* plus, const int32_t* m
 cudaError_t launch_rhs_hpipe(const RhsParams& p, const int32_t* links, int lrow, const double* a_plus,
                              const double* a_minus_x, const double* a_minus_o, const double* H_host,
                              const double* delta_host, int warps, int sms, unsigned long long* tickets,
+                             unsigned long long* ticket_base, cudaStream_t s);
+
+// Tensor-core (DMMA) kernel for N = 32, 64, 96 (kernels_large.cu), any state.  lptr: DEVICE [nodes+1] CSR
+// offsets; lent: DEVICE int4 link entries {neighbour slot, mode l, 0 "+" | 1 "-", n_l}; Hs_dev: DEVICE
+// [N][N] = H/hbar; delta_dev: DEVICE [N]; a_*: HOST coupling tables [W][D+1]; tickets as for hpipe.
+bool large_supported(int N, int W);
+cudaError_t launch_rhs_large(const RhsParams& p, const int64_t* lptr, const void* lent, const double* Hs_dev,
+                             const double* delta_dev, const double* a_plus, const double* a_minus_x,
+                             const double* a_minus_o, int sms, unsigned long long* tickets,
                              unsigned long long* ticket_base, cudaStream_t s);
 
 // dst[slot_of[u]*dst_stride + e] = src[u*NN + e]  (to_device=1) or the inverse (to_device=0)

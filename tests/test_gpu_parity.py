@@ -39,7 +39,8 @@ def rel_err(a, b):
 
 
 SHAPES = [(2, 1, 4), (7, 1, 3), (14, 0, 3), (3, 2, 4), (1, 0, 5), (5, 0, 0), (96, 0, 1), (33, 1, 1),
-          (7, 1, 5), (16, 0, 2), (4, 0, 6), (6, 1, 3), (9, 0, 3), (11, 1, 2), (13, 0, 2), (15, 0, 2)]
+          (7, 1, 5), (16, 0, 2), (4, 0, 6), (6, 1, 3), (9, 0, 3), (11, 1, 2), (13, 0, 2), (15, 0, 2),
+          (32, 0, 2), (64, 0, 1), (32, 1, 1), (96, 0, 2)]
 
 
 @pytest.mark.parametrize("N,K,D", SHAPES)
