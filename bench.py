@@ -29,6 +29,11 @@ METRIC = "heom_node_updates_per_s"
 UNIT = "node-updates/s"
 
 
+# FP64 peak of one B200: 148 SMs x 64 FP64 FMA/clk x 2 flop x 1.965 GHz (clocks.max.sm).
+# MEASURED_PEAKS.json has no FP64 entry; a register-resident DMMA.8x8x4 probe on this pool measured 37.1 TFLOP/s.
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -50,7 +55,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                 "--format=csv,noheader,nounits", "-lms", "100"],
+                 "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -87,17 +92,30 @@ class ClockSampler:
 
 
 def oracle_throughput(w, target_seconds=15.0):
-    """The oracle as it stands, on the host cores, on a bounded sample of the same workload:
-    a whole number of RK4 steps of the full hierarchy sized to ~target_seconds."""
+    """The oracle as it stands, on the host cores, on a bounded sample of the same workload.
+    States up to 2 GB: a whole number of RK4 steps of the full hierarchy sized to ~target_seconds.
+    Larger states (configs 3 and 5: one oracle step would take minutes and 30-90 GB of host memory):
+    right-hand-side evaluations (oracle_rhs_nodes) of a seeded sample of nodes of the full hierarchy,
+    i.e. node-updates without the RK4 combination."""
     from oracle.oracle import Oracle
     o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D)
     o.set_state(w.sigma0())
-    t0 = time.perf_counter(); o.rk4_steps(w.dt_fs, 1); t1 = time.perf_counter() - t0
-    n = int(max(1, min(w.steps, target_seconds / max(t1, 1e-6))))
-    t0 = time.perf_counter(); o.rk4_steps(w.dt_fs, n); dt = time.perf_counter() - t0
-    return {"value": 4.0 * w.nodes * n / dt, "unit": UNIT, "cores": o.threads, "kind": "oracle",
-            "sample": f"{n} RK4 steps of the full {w.name} hierarchy ({w.nodes} nodes) after 1 warm-up step",
-            "seconds": dt, "steps": n}
+    if w.state_bytes <= 2e9:
+        t0 = time.perf_counter(); o.rk4_steps(w.dt_fs, 1); t1 = time.perf_counter() - t0
+        n = int(max(1, min(w.steps, target_seconds / max(t1, 1e-6))))
+        t0 = time.perf_counter(); o.rk4_steps(w.dt_fs, n); dt = time.perf_counter() - t0
+        return {"value": 4.0 * w.nodes * n / dt, "unit": UNIT, "cores": o.threads, "kind": "oracle",
+                "sample": f"{n} RK4 steps of the full {w.name} hierarchy ({w.nodes} nodes) after 1 warm-up step",
+                "seconds": dt, "steps": n}
+    rng = np.random.default_rng(7)
+    probe = rng.integers(0, w.nodes, 64 * o.threads)
+    t0 = time.perf_counter(); o.rhs_nodes(probe); t1 = time.perf_counter() - t0
+    m = int(min(w.nodes, max(probe.size, probe.size * target_seconds / max(t1, 1e-6))))
+    ids = rng.integers(0, w.nodes, m)
+    t0 = time.perf_counter(); o.rhs_nodes(ids); dt = time.perf_counter() - t0
+    return {"value": m / dt, "unit": UNIT, "cores": o.threads, "kind": "oracle",
+            "sample": f"right-hand side of {m} seeded random nodes of the full {w.name} hierarchy ({w.nodes} nodes), "
+                      f"sigma_0 = |1><1| state, no RK4 combination", "seconds": dt, "steps": 0}
 
 
 def run_reference(args, w):
@@ -140,7 +158,7 @@ def config_dict(w, n_gpus):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", default="cfg2", choices=list(workloads.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -221,21 +239,38 @@ def main():
         peaks, which = measured_peaks()
         value = 4.0 * w.nodes * args.steps * world / (ms * 1e-3)
         alg_bytes_per_launch = 64.0 * w.N * w.N * w.nodes          # 16 S per step / 4 launches
+        alg_flops_per_launch = 8.0 * w.N ** 3 * w.nodes            # real H: 8 N^3 per node-update
         avg_launch_s = (kern_ms / max(kern_n, 1)) * 1e-3
         achieved = alg_bytes_per_launch / avg_launch_s / 1e9
+        # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
+        # (average over the 4 stage launches of one RK4 step), or null where no capture exists
+        ncu_traffic = {"cfg2_fmo7": (963.8e6, "profiles/r1b_cfg2_hpipe.md"),
+                       "cfg5_large96": (94.4e9, "profiles/r1b_cfg5_large.md")}.get(w.name, (None, None))
+        if w.N >= 32:
+            # arithmetic-bound (N/8 = 12 flop/B at N = 96): FP64 pipe (DMMA) roofline
+            tf = alg_flops_per_launch / avg_launch_s / 1e12
+            roof = {"bound": "alu", "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": tf / FP64_PEAK_TFLOPS, "traffic": ncu_traffic[0], "traffic_source": ncu_traffic[1],
+                    "peak_source": "derived: 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz (DMMA probe measured 37.1)",
+                    "kernel": g.kernel_name(), "avg_launch_ms": avg_launch_s * 1e3, "launches_timed": kern_n,
+                    "algorithmic_flops_per_launch": alg_flops_per_launch,
+                    "algorithmic_bytes_per_launch": alg_bytes_per_launch,
+                    "hbm_GBs_at_algorithmic_bytes": achieved}
+        else:
+            roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": achieved / peaks["hbm_gbs"], "traffic": ncu_traffic[0], "traffic_source": ncu_traffic[1],
+                    "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({which})",
+                    "kernel": g.kernel_name(), "avg_launch_ms": avg_launch_s * 1e3,
+                    "launches_timed": kern_n,
+                    "algorithmic_bytes_per_launch": alg_bytes_per_launch,
+                    "frac_of_nominal_8TBs": achieved / 8000.0}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": config_dict(w, world),
             "rk4_steps_per_s": args.steps * world / (ms * 1e-3),
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                         "frac": achieved / peaks["hbm_gbs"], "traffic": None,
-                         "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({which})",
-                         "kernel": g.kernel_name(), "avg_launch_ms": avg_launch_s * 1e3,
-                         "launches_timed": kern_n,
-                         "algorithmic_bytes_per_launch": alg_bytes_per_launch,
-                         "frac_of_nominal_8TBs": achieved / 8000.0},
+            "roofline": roof,
             "e2e": {"value": 4.0 * w.nodes * e_steps * world / e_dt, "unit": UNIT,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "what": "heom_set_state(HOST sigma_0) once, then per step heom_rk4_steps(dt,1) + "

@@ -65,7 +65,16 @@ void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
  *   "order"   device storage order of the nodes: 0 = pinned order, 1 = plain
  *             lexicographic (default 1)
  *   "kernel"  0 = generic element-per-thread kernel, 1 = auto (specialised
- *             kernels where available; default)
+ *             kernels where available; default), 2 = as 1 without the persistent
+ *             pipelined / tensor-core kernels (for comparison)
+ *   "l2_fetch" cudaLimitMaxL2FetchGranularity to request (32, 64, 128), 0 = leave it
+ * and at any time:
+ *   "rk4_form" how heom_rk4_steps groups the classical RK4 step (R6): 0 = the four
+ *             classical stages; 1 or -1 (default) = the Taylor/Horner form v_s = (dt/s) L v_{s-1},
+ *             y' = y + v1 + v2 + v3 + v4 -- identical for this linear autonomous right-hand side up
+ *             to rounding, 14 instead of 16 state sizes of traffic -- where the kernel in use
+ *             supports it (the pipelined small-N kernel and the large-N tensor-core kernel)
+ *   "warps_per_cta" warps per CTA of the pipelined small-N kernel, 0 = as many as fit (default)
  *   "timing"  1 = bracket every RHS launch with CUDA events (heom_kernel_time)
  *   "hermitian" 1 (default) = when heom_set_state / heom_set_full_state find the state
  *             EXACTLY Hermitian (every node equals its conjugate transpose bit for bit), use
@@ -107,9 +116,9 @@ heom_status heom_get_full_state(heom_ctx* ctx, double* sigma);
 /* dsigma = L(current state): one evaluation of Eq. 12-17 on every node; the
  * state is not changed.  dsigma HOST, same layout as heom_get_full_state. */
 heom_status heom_rhs(heom_ctx* ctx, double* dsigma);
-/* Advance the state by nsteps classical RK4 steps of dt_fs (R6).  Enqueues
- * 4*nsteps fused kernels on the bound stream and returns; heom_sync or any
- * HOST getter synchronises. */
+/* Advance the state by nsteps classical RK4 steps of dt_fs (R6; option "rk4_form" selects how
+ * the step is grouped).  Enqueues 4*nsteps fused kernels on the bound stream and returns;
+ * heom_sync or any HOST getter synchronises. */
 heom_status heom_rk4_steps(heom_ctx* ctx, double dt_fs, int nsteps);
 heom_status heom_sync(heom_ctx* ctx);
 /* Eq. 26: pop[i] = Re sigma_0[i][i] (HOST [n_sites]); trace = sum_i sigma_0[i][i].

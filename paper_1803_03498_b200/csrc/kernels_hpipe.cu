@@ -178,7 +178,8 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   const bool rhs_only = p.rhs_only != 0;
   const bool y_is_x = (p.y == p.x), acc_is_x = (p.acc_in == p.x);
   const bool need_A = !rhs_only && !acc_is_x;
-  const bool need_Y = !rhs_only && p.out_x != nullptr && !y_is_x;
+  const bool taylor = p.taylor != 0;                  // next stage input = ax*k (Taylor form): y is not read
+  const bool need_Y = !rhs_only && p.out_x != nullptr && !y_is_x && !taylor;
   const bool write_x = !rhs_only && p.out_x != nullptr;
   const bool producer = lane == 0;
   const unsigned long long pol_stream = policy_evict_first(), pol_keep = policy_evict_last();
@@ -369,7 +370,9 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
         for (int i = 0; i < N; ++i) {
           const double2 yv = xa[i * N];             // y (stage 1: y = x, still in XA)
           const double2 av = acc_is_x ? yv : ac[i * N];
-          if (write_x) xa[i * N] = make_double2(fma(p.ax, k[i].x, yv.x), fma(p.ax, k[i].y, yv.y));
+          if (write_x)
+            xa[i * N] = taylor ? make_double2(p.ax * k[i].x, p.ax * k[i].y)
+                               : make_double2(fma(p.ax, k[i].x, yv.x), fma(p.ax, k[i].y, yv.y));
           ac[i * N] = make_double2(fma(p.bx, k[i].x, av.x), fma(p.bx, k[i].y, av.y));
         }
       }

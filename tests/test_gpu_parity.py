@@ -98,12 +98,15 @@ def test_dimer_1000_steps():
 
 @pytest.mark.parametrize("name,D,steps", [("cfg2", 4, 300), ("cfg3", 5, 100), ("cfg4", 4, 200),
                                           ("cfg5", 1, 50), ("cfg5", 2, 10)])
-@pytest.mark.parametrize("order,kernel,herm", [(0, 1, 1), (1, 1, 1), (1, 1, 0), (1, 0, 0)])
-def test_rk4_parity_reduced_depth(name, D, steps, order, kernel, herm):
+@pytest.mark.parametrize("order,kernel,herm,form", [(0, 1, 1, -1), (1, 1, 1, -1), (1, 1, 1, 0), (1, 1, 0, -1),
+                                                    (1, 2, 1, -1), (1, 0, 0, -1)])
+def test_rk4_parity_reduced_depth(name, D, steps, order, kernel, herm, form):
     """The BASELINE configs at reduced depth (sizes the oracle finishes in seconds; several CTAs
-    and a ragged last CTA), full RK4 runs, every node compared."""
+    and a ragged last CTA), full RK4 runs, every node compared.  form = -1: the kernel's default
+    stage form (Taylor/Horner for the pipelined and the tensor-core kernels, DESIGN.md R6);
+    form = 0: the classical stages.  kernel = 2: the non-persistent Hermitian kernel."""
     w = workloads.get(name).with_(D=D)
-    o, g = _pair(w, order=order, kernel=kernel, hermitian=herm)
+    o, g = _pair(w, order=order, kernel=kernel, hermitian=herm, rk4_form=form)
     o.set_state(w.sigma0()); g.set_state(w.sigma0())
     o.rk4_steps(w.dt_fs, steps); g.rk4_steps(w.dt_fs, steps)
     ref, got = o.get_full_state(), g.get_full_state()
