@@ -34,6 +34,7 @@
 #include "kernels.cuh"
 
 #include <cmath>
+#include <type_traits>
 
 namespace heom {
 namespace {
@@ -274,35 +275,34 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     // ---- couplings: row b of sigma_{u +- e_l}, element j (Eq. 15-17 / 35-36, Eq. 23, 25) -------
     // An invalid "-" link has n_l = 0, an invalid "+" link (top level) carries the record byte 0:
     // both give a zero factor, so a skipped load contributes nothing.
-    bool refilled = false;
-    for (int kk0 = 0; kk0 < M; kk0 += KB) {
-      double2 w[2 * KB * N];
+    // One batch = KBN mode indices kk0..kk0+KBN-1: all 2*KBN*N loads are issued before the first is used.
+    // FIRST marks the batch that starts at kk = 0, the only mode index with a V^o factor (delta_k0).
+    auto gather = [&](auto kbn_tag, auto first_tag, int kk0) {
+      constexpr int KBN = decltype(kbn_tag)::value;
+      constexpr bool FIRST = decltype(first_tag)::value;
+      double2 w[2 * KBN * N];
 #pragma unroll
-      for (int b = 0; b < 2 * KB * N; ++b) w[b] = make_double2(0.0, 0.0);
+      for (int b = 0; b < 2 * KBN * N; ++b) w[b] = make_double2(0.0, 0.0);
 #pragma unroll
-      for (int kb = 0; kb < KB; ++kb) {
-        const int kk = kk0 + kb;
-        if (kk < M) {
-          const int32_t* grp = lk + kk * GROUP;
-          int up[NP4], dn[NP4];
+      for (int kb = 0; kb < KBN; ++kb) {
+        const int32_t* grp = lk + (kk0 + kb) * GROUP;
+        int up[NP4], dn[NP4];
 #pragma unroll
-          for (int t = 0; t < NP4 / 4; ++t) {
-            const int4 a = reinterpret_cast<const int4*>(grp)[t];
-            up[4 * t] = a.x; up[4 * t + 1] = a.y; up[4 * t + 2] = a.z; up[4 * t + 3] = a.w;
-            const int4 c = reinterpret_cast<const int4*>(grp + NP4)[t];
-            dn[4 * t] = c.x; dn[4 * t + 1] = c.y; dn[4 * t + 2] = c.z; dn[4 * t + 3] = c.w;
-          }
+        for (int t = 0; t < NP4 / 4; ++t) {
+          const int4 a = reinterpret_cast<const int4*>(grp)[t];
+          up[4 * t] = a.x; up[4 * t + 1] = a.y; up[4 * t + 2] = a.z; up[4 * t + 3] = a.w;
+          const int4 c = reinterpret_cast<const int4*>(grp + NP4)[t];
+          dn[4 * t] = c.x; dn[4 * t + 1] = c.y; dn[4 * t + 2] = c.z; dn[4 * t + 3] = c.w;
+        }
 #pragma unroll
-          for (int b = 0; b < N; ++b) {
-            ldg_link(w[(2 * kb) * N + b], xj + b * N, up[b], pol_keep);
-            ldg_link(w[(2 * kb + 1) * N + b], xj + b * N, dn[b], pol_keep);
-          }
+        for (int b = 0; b < N; ++b) {
+          ldg_link(w[(2 * kb) * N + b], xj + b * N, up[b], pol_keep);
+          ldg_link(w[(2 * kb + 1) * N + b], xj + b * N, dn[b], pol_keep);
         }
       }
-      if (!refilled) {
+      if (FIRST) {
         // with the gathers in flight: the write-back of the previous pass has left shared memory, so
         // its ring slot can take the next pass
-        refilled = true;
         if (producer) {
           bulk_wait_read0();
           if (qn < npass) issue_x(qn, s ^ 1);
@@ -310,27 +310,48 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
         qn = __shfl_sync(0xffffffffu, qn, 0);
       }
 #pragma unroll
-      for (int kb = 0; kb < KB; ++kb) {
+      for (int kb = 0; kb < KBN; ++kb) {
         const int kk = kk0 + kb;
-        if (kk < M) {
-          const int32_t* grp = lk + kk * GROUP;
-          unsigned rw[NB8 / 2];
+        const int32_t* grp = lk + kk * GROUP;
+        unsigned rw[NB8 / 2];
 #pragma unroll
-          for (int t = 0; t < NB8 / 8; ++t) {
-            const uint4 v = reinterpret_cast<const uint4*>(grp + 2 * NP4)[t];
-            rw[4 * t] = v.x; rw[4 * t + 1] = v.y; rw[4 * t + 2] = v.z; rw[4 * t + 3] = v.w;
-          }
+        for (int t = 0; t < NB8 / 8; ++t) {
+          const uint4 v = reinterpret_cast<const uint4*>(grp + 2 * NP4)[t];
+          rw[4 * t] = v.x; rw[4 * t + 1] = v.y; rw[4 * t + 2] = v.z; rw[4 * t + 3] = v.w;
+        }
 #pragma unroll
-          for (int b = 0; b < N; ++b) {
-            const unsigned rec = (b & 1) ? (rw[b >> 1] >> 16) : (rw[b >> 1] & 0xffffu);
-            const double2 sq = *reinterpret_cast<const double2*>(reinterpret_cast<const unsigned char*>(sSQ) + rec);
-            const int l = b * M + kk;
-            const double a = sq.y * P.cP[l], ax = sq.x * P.cX[l], ao = sq.x * P.cO[l];   // sqrt(n+1)|0, sqrt(n)
-            const double2 wu = w[(2 * kb) * N + b], wd = w[(2 * kb + 1) * N + b];
-            z[b].x = fma(-a, wu.y, z[b].x); z[b].y = fma(a, wu.x, z[b].y);                     // i a+ sigma^+
-            z[b].x = fma(ao, wd.x, fma(-ax, wd.y, z[b].x));                                    // (i a-x + a-o) sigma^-
-            z[b].y = fma(ao, wd.y, fma(ax, wd.x, z[b].y));
+        for (int b = 0; b < N; ++b) {
+          const unsigned rec = (b & 1) ? (rw[b >> 1] >> 16) : (rw[b >> 1] & 0xffffu);
+          const double2 sq = *reinterpret_cast<const double2*>(reinterpret_cast<const unsigned char*>(sSQ) + rec);
+          const int l = b * M + kk;
+          const double a = sq.y * P.cP[l], ax = sq.x * P.cX[l];     // sqrt(n+1)|0, sqrt(n)
+          const double2 wu = w[(2 * kb) * N + b], wd = w[(2 * kb + 1) * N + b];
+          z[b].x = fma(-a, wu.y, z[b].x); z[b].y = fma(a, wu.x, z[b].y);                       // i a+ sigma^+
+          z[b].x = fma(-ax, wd.y, z[b].x); z[b].y = fma(ax, wd.x, z[b].y);                     // i a-x sigma^-
+          if (FIRST && kb == 0) {                                                              // a-o sigma^-, k = 0 only
+            const double ao = sq.x * P.cO[l];
+            z[b].x = fma(ao, wd.x, z[b].x); z[b].y = fma(ao, wd.y, z[b].y);
           }
+        }
+      }
+    };
+    {
+      using std::integral_constant;
+      int kk0 = 0;
+      if (M >= KB) { gather(integral_constant<int, KB>{}, integral_constant<bool, true>{}, 0); kk0 = KB; }
+      for (; kk0 + KB <= M; kk0 += KB) gather(integral_constant<int, KB>{}, integral_constant<bool, false>{}, kk0);
+      if (kk0 < M) {                                  // remainder batch of 1..KB-1 mode indices
+        const int rem = M - kk0;
+        if (kk0 == 0) {
+          if (KB > 1 && rem == 1) gather(integral_constant<int, 1>{}, integral_constant<bool, true>{}, 0);
+          else if (KB > 2 && rem == 2) gather(integral_constant<int, (KB > 2 ? 2 : 1)>{}, integral_constant<bool, true>{}, 0);
+          else if (KB > 3 && rem == 3) gather(integral_constant<int, (KB > 3 ? 3 : 1)>{}, integral_constant<bool, true>{}, 0);
+          else {
+            gather(integral_constant<int, 1>{}, integral_constant<bool, true>{}, 0);
+            for (int kk = 1; kk < M; ++kk) gather(integral_constant<int, 1>{}, integral_constant<bool, false>{}, kk);
+          }
+        } else {
+          for (int kk = kk0; kk < M; ++kk) gather(integral_constant<int, 1>{}, integral_constant<bool, false>{}, kk);
         }
       }
     }
@@ -362,17 +383,36 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     if (active) {
       double2* xa = sXA + g * PS + j;
       double2* ac = sAC + g * PS + j;
+      // one straight-line loop per stage kind (uniform branches), so nothing is selected per element
       if (rhs_only) {
 #pragma unroll
         for (int i = 0; i < N; ++i) ac[i * N] = k[i];
-      } else {
+      } else if (acc_is_x) {                        // stage 1: y = acc_in = x, still in XA
 #pragma unroll
         for (int i = 0; i < N; ++i) {
-          const double2 yv = xa[i * N];             // y (stage 1: y = x, still in XA)
-          const double2 av = acc_is_x ? yv : ac[i * N];
-          if (write_x)
-            xa[i * N] = taylor ? make_double2(p.ax * k[i].x, p.ax * k[i].y)
-                               : make_double2(fma(p.ax, k[i].x, yv.x), fma(p.ax, k[i].y, yv.y));
+          const double2 yv = xa[i * N];
+          xa[i * N] = taylor ? make_double2(p.ax * k[i].x, p.ax * k[i].y)
+                             : make_double2(fma(p.ax, k[i].x, yv.x), fma(p.ax, k[i].y, yv.y));
+          ac[i * N] = make_double2(fma(p.bx, k[i].x, yv.x), fma(p.bx, k[i].y, yv.y));
+        }
+      } else if (!write_x) {                        // stage 4: running sum only
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+          const double2 av = ac[i * N];
+          ac[i * N] = make_double2(fma(p.bx, k[i].x, av.x), fma(p.bx, k[i].y, av.y));
+        }
+      } else if (taylor) {                          // Taylor stages 2, 3: v_s = ax k
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+          const double2 av = ac[i * N];
+          xa[i * N] = make_double2(p.ax * k[i].x, p.ax * k[i].y);
+          ac[i * N] = make_double2(fma(p.bx, k[i].x, av.x), fma(p.bx, k[i].y, av.y));
+        }
+      } else {                                      // classical stages 2, 3: y is in XA
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+          const double2 yv = xa[i * N], av = ac[i * N];
+          xa[i * N] = make_double2(fma(p.ax, k[i].x, yv.x), fma(p.ax, k[i].y, yv.y));
           ac[i * N] = make_double2(fma(p.bx, k[i].x, av.x), fma(p.bx, k[i].y, av.y));
         }
       }
