@@ -57,6 +57,8 @@ struct heom_ctx {
   size_t n_links = 0;
   unsigned long long* d_tickets = nullptr;   // work counter of the persistent kernel
   unsigned long long ticket_base = 0;
+  int acc_red = 1;           // option "acc_red": 1 (default) = Taylor stages 2-4 of the large-N kernel add to the running sum
+                             // with fire-and-forget global reductions, 0 = they load, add and store it
   int rk4_form = -1;         // option "rk4_form": 0 classical stages, 1 Taylor/Horner (large-N kernel only), -1 auto
   int l2_fetch = 0;          // option "l2_fetch": cudaLimitMaxL2FetchGranularity in bytes, 0 = leave the default
   int sms = 148;
@@ -239,6 +241,7 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
     ctx->l2_fetch = value;
     return HEOM_OK;
   }
+  if (s == "acc_red") { ctx->acc_red = value ? 1 : 0; return HEOM_OK; }
   if (s == "rk4_form") {
     if (value < -1 || value > 1) return fail(ctx, HEOM_EINVAL, "rk4_form must be -1, 0 or 1");
     ctx->rk4_form = value;
@@ -548,7 +551,7 @@ heom_status heom_rk4_steps(heom_ctx* ctx, double dt, int nsteps) {
       p.x = ctx->y; p.y = nullptr; p.acc_in = ctx->y; p.out_x = ctx->xa; p.out_acc = ctx->acc;
       p.ax = dt; p.bx = dt; p.acc_red = 0;
       if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-      p.acc_red = 1; p.acc_in = nullptr;
+      p.acc_red = ctx->acc_red; p.acc_in = ctx->acc;
       p.x = ctx->xa; p.out_x = ctx->xb; p.ax = p.bx = dt / 2.0;
       if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
       p.x = ctx->xb; p.out_x = ctx->xa; p.ax = p.bx = dt / 3.0;

@@ -87,7 +87,7 @@ __device__ __forceinline__ void lbulk_prefetch_l2(const void* src_gmem, unsigned
 // D(8x8) += A(8x4) B(4x8), fp64 tensor core.  a: A[lane/4][lane%4]; b: B[lane%4][lane/4];
 // c0, c1: C[lane/4][2*(lane%4) + {0,1}].
 __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 __device__ __forceinline__ double neg(double v) { return -v; }
@@ -180,11 +180,11 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
         for (int ct = 0; ct < CT; ++ct) {
           const double b0 = sBcol[(size_t)(m0 * SS + 4 * ct) * 2];
           const double b1 = sBcol[(size_t)((m0 + 1) * SS + 4 * ct) * 2];
+          // the two k-halves update the same accumulators: keep RG independent DMMAs between them
 #pragma unroll
-          for (int rg = 0; rg < RG; ++rg) {
-            dmma(acc[rg][ct].x, acc[rg][ct].y, hA[rg].x, b0);
-            dmma(acc[rg][ct].x, acc[rg][ct].y, hA[rg].y, b1);
-          }
+          for (int rg = 0; rg < RG; ++rg) dmma(acc[rg][ct].x, acc[rg][ct].y, hA[rg].x, b0);
+#pragma unroll
+          for (int rg = 0; rg < RG; ++rg) dmma(acc[rg][ct].x, acc[rg][ct].y, hA[rg].y, b1);
         }
       }
 #pragma unroll
