@@ -67,6 +67,9 @@ void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
  *   "kernel"  0 = generic element-per-thread kernel, 1 = auto (specialised
  *             kernels where available; default), 2 = as 1 without the persistent
  *             pipelined / tensor-core kernels (for comparison)
+ *   "pade"    0 (default) = Matsubara poles and coefficients (Eq. 19-20); 1 = Pade poles (P:148-176
+ *             Eq. 27-33, R11): the K poles beyond the Drude pole become xi_k/(beta hbar) with weights eta_k.
+ *             Rebuilds the coefficients (heom_get_coefficients reports them)
  *   "l2_fetch" cudaLimitMaxL2FetchGranularity to request (32, 64, 128), 0 = leave it
  * and at any time:
  *   "rk4_form" how heom_rk4_steps groups the classical RK4 step (R6): 0 = the four

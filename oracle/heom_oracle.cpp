@@ -60,6 +60,8 @@ struct oracle_ctx {
   int scaling = 1;
   int terminator = 1;
   int threads = 0;
+  int pade = 0;      /* 0 = Matsubara poles (Eq. 19-20), 1 = Pade poles (Eq. 27-33) */
+  double T_kelvin = 0;
   std::vector<double> H;        /* [N][N] cm^-1                               */
   std::vector<double> lambda;   /* [N] cm^-1                                  */
   std::vector<double> nu;       /* [N] fs^-1                                  */
@@ -162,6 +164,74 @@ void build_links(oracle_ctx* c) {
  * l = b*M + k (Eq. 10 rewritten 0-based), k = 0 the Drude pole.
  * Reading R2: every c of Eq. 16-17 and 35-36 enters as c-hat = c/hbar so that
  * all terms of the RHS are rates.                                            */
+/* ------------------------------------------------------- Pade decomposition
+ * P:148-176 Eq. 27-33 ([K-1/K] Pade spectrum decomposition of the Bose function, the paper's ref. 31):
+ *   1/(1 - exp(-x)) ~ 1/x + 1/2 + sum_{j=1..K} 2 eta_j x / (x^2 + xi_j^2).
+ * xi_j = 2/eigenvalue_j(Lambda) for the K positive eigenvalues of the 2K x 2K matrix Eq. 27, zeta_j the same
+ * for the (2K-1) x (2K-1) matrix Eq. 28 (K-1 positive eigenvalues), and Eq. 29 read as (R11: the
+ * printed indices are garbled)
+ *   eta_j = (K^2 + 3K/2) prod_{k=1..K-1} (zeta_k^2 - xi_j^2) / prod_{k != j} (xi_k^2 - xi_j^2).
+ * Eigenvalues by the cyclic Jacobi rotation method on the dense symmetric matrix: slow, short, hard to get
+ * wrong. */
+std::vector<double> jacobi_eigenvalues(std::vector<double> a, int n) {
+  for (int sweep = 0; sweep < 100; ++sweep) {
+    double off = 0.0;
+    for (int p = 0; p < n; ++p)
+      for (int q = p + 1; q < n; ++q) off += a[(size_t)p * n + q] * a[(size_t)p * n + q];
+    if (off < 1e-300) break;
+    for (int p = 0; p < n; ++p)
+      for (int q = p + 1; q < n; ++q) {
+        const double apq = a[(size_t)p * n + q];
+        if (apq == 0.0) continue;
+        const double theta = (a[(size_t)q * n + q] - a[(size_t)p * n + p]) / (2.0 * apq);
+        const double t = (theta >= 0 ? 1.0 : -1.0) / (std::fabs(theta) + std::sqrt(theta * theta + 1.0));
+        const double cs = 1.0 / std::sqrt(t * t + 1.0), sn = t * cs;
+        for (int k = 0; k < n; ++k) {   /* A <- A J */
+          const double akp = a[(size_t)k * n + p], akq = a[(size_t)k * n + q];
+          a[(size_t)k * n + p] = cs * akp - sn * akq;
+          a[(size_t)k * n + q] = sn * akp + cs * akq;
+        }
+        for (int k = 0; k < n; ++k) {   /* A <- J^T A */
+          const double apk = a[(size_t)p * n + k], aqk = a[(size_t)q * n + k];
+          a[(size_t)p * n + k] = cs * apk - sn * aqk;
+          a[(size_t)q * n + k] = sn * apk + cs * aqk;
+        }
+      }
+  }
+  std::vector<double> ev(n);
+  for (int i = 0; i < n; ++i) ev[i] = a[(size_t)i * n + i];
+  std::sort(ev.begin(), ev.end(), [](double x, double y) { return x > y; });   /* decreasing */
+  return ev;
+}
+
+/* Eq. 27 (shift = 1) and Eq. 28 (shift = 3): (M)_{m,n} = delta_{m,n+-1} / sqrt((2m+shift)(2n+shift)), m,n = 1..size */
+std::vector<double> pade_matrix(int size, int shift) {
+  std::vector<double> a((size_t)size * size, 0.0);
+  for (int m = 1; m <= size; ++m)
+    for (int n = 1; n <= size; ++n)
+      if (m == n - 1 || m == n + 1)
+        a[(size_t)(m - 1) * size + (n - 1)] = 1.0 / std::sqrt((2.0 * m + shift) * (2.0 * n + shift));
+  return a;
+}
+
+void pade_poles(int K, std::vector<double>& xi, std::vector<double>& eta) {
+  xi.assign((size_t)K, 0.0); eta.assign((size_t)K, 0.0);
+  if (K == 0) return;
+  const std::vector<double> ev = jacobi_eigenvalues(pade_matrix(2 * K, 1), 2 * K);
+  for (int i = 0; i < K; ++i) xi[i] = 2.0 / ev[i];                                   /* Eq. 30 */
+  std::vector<double> zeta((size_t)(K > 1 ? K - 1 : 0));
+  if (K > 1) {
+    const std::vector<double> evp = jacobi_eigenvalues(pade_matrix(2 * K - 1, 3), 2 * K - 1);
+    for (int i = 0; i < K - 1; ++i) zeta[i] = 2.0 / evp[i];                          /* Eq. 31 */
+  }
+  for (int j = 0; j < K; ++j) {                                                      /* Eq. 29 */
+    double num = 1.0, den = 1.0;
+    for (int k = 0; k < K - 1; ++k) num *= zeta[k] * zeta[k] - xi[j] * xi[j];
+    for (int k = 0; k < K; ++k) if (k != j) den *= xi[k] * xi[k] - xi[j] * xi[j];
+    eta[j] = ((double)K * K + 1.5 * K) * num / den;
+  }
+}
+
 int build_coefficients(oracle_ctx* c, double T_kelvin) {
   const int N = c->N, M = c->M;
   c->beta_hbar = HBAR_CM_FS / (KB_CM_PER_K * T_kelvin);
@@ -169,6 +239,8 @@ int build_coefficients(oracle_ctx* c, double T_kelvin) {
   c->c_re.assign((size_t)c->W, 0.0);
   c->c_im.assign((size_t)c->W, 0.0);
   c->delta.assign((size_t)N, 0.0);
+  std::vector<double> pxi, peta;
+  if (c->pade) pade_poles(M - 1, pxi, peta);
   for (int b = 0; b < N; ++b) {
     const double lam = c->lambda[b] / HBAR_CM_FS; /* lambda_b / hbar, fs^-1 */
     const double nu = c->nu[b];
@@ -176,17 +248,34 @@ int build_coefficients(oracle_ctx* c, double T_kelvin) {
       const int l = b * M + k;
       if (k == 0) {
         c->gamma[l] = nu;                                           /* Eq. 19 */
-        const double x = c->beta_hbar * nu / 2.0;
-        const double t = std::tan(x);
-        if (lam != 0.0 && (t == 0.0 || !std::isfinite(1.0 / t))) return -1;
-        c->c_re[l] = (lam == 0.0) ? 0.0 : nu * lam / t;             /* Eq. 20 */
+        if (!c->pade) {
+          const double x = c->beta_hbar * nu / 2.0;
+          const double t = std::tan(x);
+          if (lam != 0.0 && (t == 0.0 || !std::isfinite(1.0 / t))) return -1;
+          c->c_re[l] = (lam == 0.0) ? 0.0 : nu * lam / t;           /* Eq. 20 */
+        } else {
+          /* Eq. 33, k = 0:  (2 lambda/(beta hbar)) (1 - sum_j 2 eta_j nu^2 / ((xi_j/(beta hbar))^2 - nu^2)) */
+          double sum = 0.0;
+          for (int jj = 0; jj < M - 1; ++jj) {
+            const double gj = pxi[(size_t)jj] / c->beta_hbar;
+            if (lam != 0.0 && gj * gj - nu * nu == 0.0) return -1;
+            sum += 2.0 * peta[(size_t)jj] * nu * nu / (gj * gj - nu * nu);
+          }
+          c->c_re[l] = (lam == 0.0) ? 0.0 : 2.0 * lam / c->beta_hbar * (1.0 - sum);
+        }
         c->c_im[l] = -lam * nu;           /* the V^o term of Eq. 17 (R4)     */
-      } else {
+      } else if (!c->pade) {
         const double g = 2.0 * PI * k / c->beta_hbar;               /* Eq. 19 */
         c->gamma[l] = g;
         if (lam != 0.0 && g * g - nu * nu == 0.0) return -1;
         c->c_re[l] = (lam == 0.0) ? 0.0
                      : 4.0 * lam * nu / c->beta_hbar * g / (g * g - nu * nu); /* Eq. 20 */
+      } else {
+        const double g = pxi[(size_t)k - 1] / c->beta_hbar;          /* Eq. 32 */
+        c->gamma[l] = g;
+        if (lam != 0.0 && g * g - nu * nu == 0.0) return -1;
+        c->c_re[l] = (lam == 0.0) ? 0.0
+                     : 4.0 * lam * nu / c->beta_hbar * peta[(size_t)k - 1] * g / (g * g - nu * nu); /* Eq. 33, k > 0 */
       }
     }
     /* Eq. 14:  2 lambda_b/(beta hbar^2 nu_b) - sum_k c(b,k)/(hbar gamma(b,k)) */
@@ -307,6 +396,7 @@ int oracle_create(oracle_ctx** out, int n_sites, const double* H_cm, const doubl
     c->H.assign(H_cm, H_cm + (size_t)n_sites * n_sites);
     c->lambda.assign(lambda_cm, lambda_cm + n_sites);
     c->nu.assign(nu_per_fs, nu_per_fs + n_sites);
+    c->T_kelvin = T_kelvin;
     if (build_coefficients(c, T_kelvin) != 0) { delete c; return -1; }
     std::vector<uint8_t> cur((size_t)c->W, 0);
     for (int L = 0; L <= D; ++L) enumerate_level(c->W, 0, L, cur, c->tuples);
@@ -329,7 +419,16 @@ int oracle_set_option(oracle_ctx* c, const char* name, int value) {
   if (s == "scaling") { if (value < 0 || value > 2) return -1; c->scaling = value; return 0; }
   if (s == "terminator") { c->terminator = value ? 1 : 0; return 0; }
   if (s == "threads") { if (value < 0) return -1; c->threads = value; return 0; }
+  if (s == "pade") { c->pade = value ? 1 : 0; return build_coefficients(c, c->T_kelvin); }
   return -1;
+}
+
+int oracle_pade_poles(int K, double* xi, double* eta) {
+  if (K < 0 || K > 64 || (K > 0 && (!xi || !eta))) return -1;
+  std::vector<double> x, e;
+  pade_poles(K, x, e);
+  for (int i = 0; i < K; ++i) { xi[i] = x[(size_t)i]; eta[i] = e[(size_t)i]; }
+  return 0;
 }
 
 int64_t oracle_num_nodes(const oracle_ctx* c) { return c ? c->nodes : -1; }

@@ -45,9 +45,15 @@ void oracle_destroy(oracle_ctx* ctx);
  *               [1] = Eq. 35-36 with |c| = |Re c(b,k)|      (R5)
  *                2 = Eq. 35-36 with |c| = complex modulus of c(b,0)
  *   "terminator" [1] = Eq. 14 on, 0 = off
+ *   "pade"       [0] = Matsubara poles and coefficients (Eq. 19-20), 1 = Pade (Eq. 27-33); rebuilds the
+ *                coefficients, K keeps its meaning (number of poles beyond the Drude pole)
  *   "threads"    OpenMP threads for the loop over nodes [0 = runtime default];
  *                results are bit-identical for any thread count (no reductions). */
 int  oracle_set_option(oracle_ctx* ctx, const char* name, int value);
+
+/* P:148-176 Eq. 27-31: poles xi_j and weights eta_j (j = 1..K, xi increasing) of the [K-1/K] Pade
+ * decomposition of the Bose function, 1/(1-exp(-x)) ~ 1/x + 1/2 + sum_j 2 eta_j x/(x^2 + xi_j^2). */
+int  oracle_pade_poles(int K, double* xi, double* eta);
 
 int64_t oracle_num_nodes(const oracle_ctx* ctx);   /* Eq. 9: C(W+D, W)        */
 int     oracle_num_modes(const oracle_ctx* ctx);   /* W = n_sites*(K+1)       */

@@ -40,8 +40,18 @@ def _load():
     lib.oracle_rhs_nodes.argtypes = [P, P, C.c_int64, P]
     lib.oracle_rk4_steps.argtypes = [P, C.c_double, C.c_int]
     lib.oracle_populations.argtypes = [P, P, P, P]
+    lib.oracle_pade_poles.argtypes = [C.c_int, P, P]
     _lib = lib
     return lib
+
+
+def pade_poles(K):
+    """(xi, eta) of the [K-1/K] Pade decomposition of the Bose function (heom_oracle.h)."""
+    lib = _load()
+    xi = np.empty(K); eta = np.empty(K)
+    if lib.oracle_pade_poles(int(K), xi.ctypes.data, eta.ctypes.data) != 0:
+        raise ValueError("oracle_pade_poles failed")
+    return xi, eta
 
 
 def _dptr(a):
@@ -52,7 +62,7 @@ class Oracle:
     """One truncated hierarchy on the CPU.  Arguments as heom_oracle.h."""
 
     def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, scaling=1, terminator=1,
-                 threads=0):
+                 threads=0, pade=0):
         lib = _load()
         H = np.ascontiguousarray(H_cm, dtype=np.float64)
         self.N = H.shape[0]
@@ -68,7 +78,7 @@ class Oracle:
         self.K, self.D = int(K), int(D)
         self.nodes = int(lib.oracle_num_nodes(h))
         self.W = int(lib.oracle_num_modes(h))
-        for name, v in (("scaling", scaling), ("terminator", terminator), ("threads", threads)):
+        for name, v in (("scaling", scaling), ("terminator", terminator), ("threads", threads), ("pade", pade)):
             self._ck(lib.oracle_set_option(h, name.encode(), int(v)))
 
     def _ck(self, rc):

@@ -18,6 +18,9 @@ using namespace heom;
 struct heom_ctx {
   Hierarchy h;
   Coefficients c;
+  std::vector<double> lambda, nu;   // bath parameters (kept for the "pade" option)
+  double T_kelvin = 0;
+  int pade = 0;
   std::vector<double> H;      // [N][N]
   std::vector<double> Tterm;  // [N][N]
   int device = 0;
@@ -206,10 +209,13 @@ heom_status heom_create(heom_ctx** out, int n_sites, const double* H_cm, const d
   c->device = device;
   c->h.N = n_sites; c->h.K = K; c->h.M = K + 1; c->h.W = n_sites * (K + 1); c->h.D = D;
   std::string err;
-  if (!build_coefficients(n_sites, K, D, lambda_cm, nu_per_fs, T_kelvin, c->c, err)) {
+  if (!build_coefficients(n_sites, K, D, lambda_cm, nu_per_fs, T_kelvin, 0, c->c, err)) {
     delete c;
     return HEOM_EINVAL;
   }
+  c->lambda.assign(lambda_cm, lambda_cm + n_sites);
+  c->nu.assign(nu_per_fs, nu_per_fs + n_sites);
+  c->T_kelvin = T_kelvin;
   c->H.assign(H_cm, H_cm + (size_t)n_sites * n_sites);
   c->Tterm.assign((size_t)n_sites * n_sites, 0.0);
   for (int i = 0; i < n_sites; ++i)
@@ -253,6 +259,19 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
     return HEOM_OK;
   }
   if (ctx->bound) return fail(ctx, HEOM_ESTATE, "option must be set before heom_bind_workspace");
+  if (s == "pade") {
+    Coefficients nc;
+    std::string err;
+    if (!build_coefficients(ctx->h.N, ctx->h.K, ctx->h.D, ctx->lambda.data(), ctx->nu.data(), ctx->T_kelvin,
+                            value ? 1 : 0, nc, err))
+      return fail(ctx, HEOM_EINVAL, err);
+    ctx->c = nc;
+    ctx->pade = value ? 1 : 0;
+    for (int i = 0; i < ctx->h.N; ++i)
+      for (int j = 0; j < ctx->h.N; ++j)
+        ctx->Tterm[(size_t)i * ctx->h.N + j] = (i == j) ? 0.0 : ctx->c.delta[i] + ctx->c.delta[j];
+    return HEOM_OK;
+  }
   if (s == "order") {
     if (value != 0 && value != 1) return fail(ctx, HEOM_EINVAL, "order must be 0 or 1");
     ctx->order = value;

@@ -127,8 +127,67 @@ bool build_hierarchy(int N, int K, int D, int order, Hierarchy& h, std::string& 
   return true;
 }
 
+namespace {
+
+// The K largest eigenvalues (decreasing) of the symmetric tridiagonal matrix with zero diagonal and
+// off-diagonal entries off[0..n-2], by bisection on the Sturm count (eigenvalues below x).
+std::vector<double> largest_eigenvalues(const std::vector<double>& off, int n, int count) {
+  auto below = [&](double x) {            // number of eigenvalues < x
+    int neg = 0;
+    double d = 1.0;
+    for (int i = 0; i < n; ++i) {
+      const double b2 = (i == 0) ? 0.0 : off[(size_t)i - 1] * off[(size_t)i - 1];
+      d = -x - (i == 0 ? 0.0 : b2 / d);
+      if (d == 0.0) d = -1e-300;
+      if (d < 0.0) ++neg;
+    }
+    return neg;
+  };
+  double bound = 0.0;                      // Gershgorin
+  for (int i = 0; i < n; ++i) {
+    const double r = (i > 0 ? std::fabs(off[(size_t)i - 1]) : 0.0) + (i + 1 < n ? std::fabs(off[(size_t)i]) : 0.0);
+    if (r > bound) bound = r;
+  }
+  std::vector<double> ev((size_t)count);
+  for (int k = 0; k < count; ++k) {        // k-th largest: n - k - 1 eigenvalues lie below it
+    double lo = 0.0, hi = bound;
+    for (int iter = 0; iter < 200; ++iter) {
+      const double mid = 0.5 * (lo + hi);
+      if (mid == lo || mid == hi) break;
+      if (below(mid) <= n - k - 1) lo = mid; else hi = mid;
+    }
+    ev[(size_t)k] = 0.5 * (lo + hi);
+  }
+  return ev;
+}
+
+}  // namespace
+
+void pade_poles(int K, std::vector<double>& xi, std::vector<double>& eta) {
+  xi.assign((size_t)K, 0.0); eta.assign((size_t)K, 0.0);
+  if (K <= 0) return;
+  auto offdiag = [](int size, int shift) {  // (m, m+1) entry, m = 1..size-1: 1/sqrt((2m+shift)(2m+2+shift))
+    std::vector<double> o((size_t)(size > 1 ? size - 1 : 0));
+    for (int m = 1; m < size; ++m) o[(size_t)m - 1] = 1.0 / std::sqrt((2.0 * m + shift) * (2.0 * m + 2.0 + shift));
+    return o;
+  };
+  const std::vector<double> ev = largest_eigenvalues(offdiag(2 * K, 1), 2 * K, K);           // Eq. 27, 30
+  for (int j = 0; j < K; ++j) xi[(size_t)j] = 2.0 / ev[(size_t)j];
+  std::vector<double> zeta;
+  if (K > 1) {
+    const std::vector<double> evp = largest_eigenvalues(offdiag(2 * K - 1, 3), 2 * K - 1, K - 1);   // Eq. 28, 31
+    for (int j = 0; j < K - 1; ++j) zeta.push_back(2.0 / evp[(size_t)j]);
+  }
+  for (int j = 0; j < K; ++j) {                                                                  // Eq. 29 (R11)
+    double num = 1.0, den = 1.0;
+    for (double z : zeta) num *= z * z - xi[(size_t)j] * xi[(size_t)j];
+    for (int k = 0; k < K; ++k) if (k != j) den *= xi[(size_t)k] * xi[(size_t)k] - xi[(size_t)j] * xi[(size_t)j];
+    eta[(size_t)j] = ((double)K * K + 1.5 * K) * num / den;
+  }
+}
+
 bool build_coefficients(int N, int K, int D, const double* lambda_cm, const double* nu_per_fs,
-                        double T_kelvin, Coefficients& c, std::string& err) {
+                        double T_kelvin, int pade, Coefficients& c, std::string& err) {
   if (!(T_kelvin > 0.0) || !std::isfinite(T_kelvin)) { err = "T_kelvin must be > 0"; return false; }
   const int M = K + 1, W = N * M;
   const double two_pi = 6.283185307179586476925286766559;
@@ -137,6 +196,8 @@ bool build_coefficients(int N, int K, int D, const double* lambda_cm, const doub
   c.a_plus.assign((size_t)W * (D + 1), 0.0);
   c.a_minus_x.assign((size_t)W * (D + 1), 0.0);
   c.a_minus_o.assign((size_t)W * (D + 1), 0.0);
+  std::vector<double> pxi, peta;
+  if (pade) pade_poles(K, pxi, peta);
   for (int b = 0; b < N; ++b) {
     const double lam = lambda_cm[b], nu = nu_per_fs[b];
     if (!(lam >= 0.0) || !std::isfinite(lam)) { err = "lambda_cm must be >= 0"; return false; }
@@ -148,16 +209,27 @@ bool build_coefficients(int N, int K, int D, const double* lambda_cm, const doub
       double g, cre, cim = 0.0;
       if (k == 0) {
         g = nu;
-        const double x = 0.5 * c.beta_hbar * nu;
-        const double sn = std::sin(x), cs = std::cos(x);
-        if (lh != 0.0 && sn == 0.0) { err = "cot(beta hbar nu/2) is singular"; return false; }
-        cre = (lh == 0.0) ? 0.0 : lh * nu * (cs / sn);
+        if (!pade) {
+          const double x = 0.5 * c.beta_hbar * nu;
+          const double sn = std::sin(x), cs = std::cos(x);
+          if (lh != 0.0 && sn == 0.0) { err = "cot(beta hbar nu/2) is singular"; return false; }
+          cre = (lh == 0.0) ? 0.0 : lh * nu * (cs / sn);
+        } else {                            // Eq. 33, k = 0
+          double sum = 0.0;
+          for (int q = 0; q < K; ++q) {
+            const double gq = pxi[(size_t)q] / c.beta_hbar, dq = gq * gq - nu * nu;
+            if (lh != 0.0 && dq == 0.0) { err = "Pade pole equals the Drude rate"; return false; }
+            sum += 2.0 * peta[(size_t)q] * nu * nu / dq;
+          }
+          cre = (lh == 0.0) ? 0.0 : 2.0 * lh / c.beta_hbar * (1.0 - sum);
+        }
         cim = -lh * nu;
       } else {
-        g = two_pi * (double)k / c.beta_hbar;
+        const double weight = pade ? peta[(size_t)k - 1] : 1.0;          // Eq. 33, k > 0 / Eq. 20
+        g = pade ? pxi[(size_t)k - 1] / c.beta_hbar : two_pi * (double)k / c.beta_hbar;   // Eq. 32 / Eq. 19
         const double den = c.beta_hbar * (g * g - nu * nu);
-        if (lh != 0.0 && den == 0.0) { err = "Matsubara frequency equals the Drude rate"; return false; }
-        cre = (lh == 0.0) ? 0.0 : 4.0 * lh * nu * g / den;
+        if (lh != 0.0 && den == 0.0) { err = "pole frequency equals the Drude rate"; return false; }
+        cre = (lh == 0.0) ? 0.0 : 4.0 * lh * nu * weight * g / den;
       }
       if (!std::isfinite(cre)) { err = "non-finite coefficient"; return false; }
       c.gamma[l] = g; c.c_re[l] = cre; c.c_im[l] = cim;

@@ -43,7 +43,12 @@ struct Coefficients {
 bool build_hierarchy(int N, int K, int D, int order, Hierarchy& h, std::string& err);
 
 // Returns false on a singular coefficient (cot pole, gamma_k == nu_b) or bad input.
+// pade = 0: Matsubara poles (Eq. 19-20); pade = 1: Pade poles (Eq. 27-33, R11).
 bool build_coefficients(int N, int K, int D, const double* lambda_cm, const double* nu_per_fs,
-                        double T_kelvin, Coefficients& c, std::string& err);
+                        double T_kelvin, int pade, Coefficients& c, std::string& err);
+
+// Poles xi_j (increasing) and weights eta_j, j = 1..K, of the [K-1/K] Pade decomposition of the Bose function
+// (Eq. 27-31): eigenvalues of the two symmetric tridiagonal matrices by Sturm-sequence bisection.
+void pade_poles(int K, std::vector<double>& xi, std::vector<double>& eta);
 
 }  // namespace heom

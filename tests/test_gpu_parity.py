@@ -60,7 +60,8 @@ def test_rhs_parity_random_state(N, K, D, order, kernel):
 
 
 @pytest.mark.parametrize("N,K,D", [(2, 1, 4), (7, 1, 4), (14, 0, 3), (3, 2, 4), (5, 0, 0), (16, 0, 2), (4, 0, 6),
-                                   (6, 1, 3), (9, 0, 3), (11, 1, 2), (13, 0, 2), (8, 2, 2)])
+                                   (6, 1, 3), (9, 0, 3), (11, 1, 2), (13, 0, 2), (8, 2, 2), (7, 3, 2), (2, 4, 3),
+                                   (5, 2, 3)])
 @pytest.mark.parametrize("order", [0, 1])
 def test_rhs_parity_hermitian_state(N, K, D, order):
     """Dense HERMITIAN random state: takes the row-gather kernel (kernels_herm.cu); the result must
@@ -118,6 +119,24 @@ def test_rk4_parity_reduced_depth(name, D, steps, order, kernel, herm, form):
     assert asym < 1e-13 * np.abs(got).max()
     if g.kernel_name() in HERM_KERNELS:
         assert asym == 0.0
+
+
+@pytest.mark.parametrize("name,D,K,T", [("cfg2", 3, 3, 77.0), ("cfg4", 3, 2, 77.0), ("cfg5", 1, 1, 150.0)])
+def test_pade_coefficients_parity(name, D, K, T):
+    """S section 8(f) next #1: the same kernels driven by the Pade pole set (option "pade", P:148-176
+    Eq. 27-33): coefficients against the oracle's, then a full RK4 run, every node compared."""
+    w = workloads.get(name).with_(D=D, K=K, T_kelvin=T)
+    from paper_1803_03498_b200 import Heom
+    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, pade=1)
+    g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, pade=1).bind()
+    for q, (a, b) in enumerate(zip(g.coefficients(), o.coefficients())):
+        assert np.allclose(a, b, rtol=1e-12, atol=1e-15)
+    o.set_state(w.sigma0()); g.set_state(w.sigma0())
+    o.rk4_steps(0.25, 200); g.rk4_steps(0.25, 200)
+    ref, got = o.get_full_state(), g.get_full_state()
+    assert rel_err(got, ref) < STATE_TOL
+    pop, tr = g.populations()
+    assert abs(tr - 1.0) < 1e-11
 
 
 def test_nonhermitian_initial_state_propagation():
@@ -182,7 +201,16 @@ def test_full_size_configs(name, steps):
     assert np.max(np.abs(got[ids] - ref)) / np.max(np.abs(ref)) < RHS_TOL
 
 
-@pytest.mark.skipif(os.environ.get("HEOM_FULL", "0") != "1", reason="set HEOM_FULL=1 (needs ~60 GB host RAM)")
+def _host_ram_gb():
+    try:
+        import psutil
+        return psutil.virtual_memory().total / 1e9
+    except Exception:
+        return 0.0
+
+
+@pytest.mark.skipif(os.environ.get("HEOM_FULL", "0") != "1" and _host_ram_gb() < 120.0,
+                    reason="needs ~90 GB host RAM (or set HEOM_FULL=1)")
 @pytest.mark.parametrize("name", ["cfg3", "cfg5"])
 def test_full_size_large_configs_sampled_rhs(name):
     """Configs 3 and 5 at full size: RHS on sampled nodes + invariants after a few steps."""
