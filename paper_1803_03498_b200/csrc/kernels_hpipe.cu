@@ -203,20 +203,23 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     mbar_expect_tx(barA + buf, bx);
     bulk_g2s(acbuf + buf * AB, p.acc_in + (size_t)n0 * NN, bx, barA + buf, pol_stream);
   };
-  // next group of this warp: one ticket per pass, drawn by lane 0 (values >= npass: no more work)
+  // Groups of this warp: one ticket per pass, drawn by lane 0 TWO passes ahead (the atomic's round trip under
+  // contention is microseconds; values >= npass: no more work).  Every warp ends with exactly two such tickets.
   auto draw = [&]() -> int {
     const unsigned long long t = atomicAdd(P.tickets, 1ULL) - P.ticket_base;
     return t < (unsigned long long)npass ? (int)t : npass;
   };
-  int q = 0;
+  int q = 0, qn = 0;                                  // this pass, the pass after it
   if (producer) {
     q = draw();
+    qn = draw();
     if (q < npass) {
       issue_x(q, 0);
       if (need_A) issue_a(q, 0);
     }
   }
   q = __shfl_sync(0xffffffffu, q, 0);
+  qn = __shfl_sync(0xffffffffu, qn, 0);
 
   constexpr int LP = C::LP;
   const int g = lane / LP;
@@ -228,8 +231,8 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   int s = 0, ab = 0;                                  // ring slot and AC buffer of this pass
   unsigned ph = 0, pha = 0;                           // their mbarrier phases
   while (q < npass) {
-    int qn = 0;                                     // the pass after this one
-    if (producer) qn = draw();
+    int qnn = 0;                                    // the pass after the next one (consumed at the end of this pass)
+    if (producer) qnn = draw();                     // always: keeps the number of tickets per launch fixed
     const int n0 = q * G;
     const int ncnt = min(G, p.nodes - n0);
     unsigned char* slot = ring + s * slot_bytes;
@@ -307,7 +310,6 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
           bulk_wait_read0();
           if (qn < npass) issue_x(qn, s ^ 1);
         }
-        qn = __shfl_sync(0xffffffffu, qn, 0);
       }
 #pragma unroll
       for (int kb = 0; kb < KBN; ++kb) {
@@ -428,6 +430,7 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     if ((s ^= 1) == 0) ph ^= 1u;
     if ((ab ^= 1) == 0) pha ^= 1u;
     q = qn;
+    qn = __shfl_sync(0xffffffffu, qnn, 0);
   }
   if (producer) bulk_wait_all();
 }
@@ -480,7 +483,7 @@ cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, c
   if (grid < 1) grid = 1;
   P.tickets = tickets;
   P.ticket_base = *ticket_base;
-  *ticket_base += (unsigned long long)P.npass + (unsigned long long)grid * P.nwarps;   // one failing draw per warp
+  *ticket_base += (unsigned long long)P.npass + 2ULL * grid * P.nwarps;   // two failing draws per warp
   rhs_hpipe_kernel<N><<<grid, P.nwarps * 32, smem, s>>>(P);
   return cudaGetLastError();
 }
