@@ -176,10 +176,11 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
     CU(launch_rhs_large(p, ctx->d_lptr, ctx->d_lent, ctx->d_Hs, ctx->d_delta, ctx->c.a_plus.data(),
                         ctx->c.a_minus_x.data(), ctx->c.a_minus_o.data(), ctx->sms, ctx->d_tickets,
                         &ctx->ticket_base, ctx->stream));
-  else if (ctx->use_hpipe && ctx->herm_opt && ctx->state_hermitian)
+  else if (ctx->use_hpipe)
     CU(launch_rhs_hpipe(p, ctx->d_linksP, ctx->lrowP, ctx->c.a_plus.data(), ctx->c.a_minus_x.data(),
-                        ctx->c.a_minus_o.data(), ctx->H.data(), ctx->c.delta.data(), ctx->warps_per_cta,
-                        ctx->sms, ctx->d_tickets, &ctx->ticket_base, ctx->stream));
+                        ctx->c.a_minus_o.data(), ctx->H.data(), ctx->c.delta.data(),
+                        ctx->herm_opt && ctx->state_hermitian, ctx->warps_per_cta, ctx->sms, ctx->d_tickets,
+                        &ctx->ticket_base, ctx->stream));
   else if (ctx->use_herm && ctx->herm_opt && ctx->state_hermitian)
     CU(launch_rhs_herm(p, ctx->d_linksH, ctx->lrowH, ctx->d_coefH, ctx->H.data(), ctx->c.delta.data(), ctx->stream));
   else if (ctx->use_rows) CU(launch_rhs_rows(p, ctx->d_links, ctx->lrow, ctx->H.data(), ctx->stream));
@@ -581,7 +582,7 @@ heom_status heom_rk4_steps(heom_ctx* ctx, double dt, int nsteps) {
     }
     return HEOM_OK;
   }
-  if (ctx->use_hpipe && ctx->herm_opt && ctx->state_hermitian && ctx->rk4_form != 0) {
+  if (ctx->use_hpipe && ctx->rk4_form != 0) {
     /* The same Taylor/Horner form for the pipelined small-N kernel: the stages never read y, the
      * running sum is updated in shared memory: 14 instead of 16 state sizes per step. */
     p.taylor = 1;
@@ -657,7 +658,7 @@ heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches)
 const char* heom_kernel_name(const heom_ctx* c) {
   if (!c) return "none";
   if (c->use_large) return "rhs_large_kernel";
-  if (c->use_hpipe && c->herm_opt && c->state_hermitian) return "rhs_hpipe_kernel";
+  if (c->use_hpipe) return (c->herm_opt && c->state_hermitian) ? "rhs_hpipe_kernel" : "rhs_hpipe_general_kernel";
   if (c->use_herm && c->herm_opt && c->state_hermitian) return "rhs_herm_kernel";
   return c->use_rows ? "rhs_rows_kernel" : "rhs_generic_kernel";
 }

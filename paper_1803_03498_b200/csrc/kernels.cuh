@@ -58,7 +58,8 @@ void herm_pack_links(int N, int M, const int32_t* plus, const int32_t* minus, co
 cudaError_t launch_rhs_herm(const RhsParams& p, const int32_t* links, int lrow, const double* coef,
                             const double* H_host, const double* delta_host, cudaStream_t s);
 
-// Persistent TMA-pipelined Hermitian-state kernel for 2 <= N <= 16 (kernels_hpipe.cu).  links: DEVICE
+// Persistent TMA-pipelined kernel for 2 <= N <= 16 (kernels_hpipe.cu); hermitian = 1: the state is exactly
+// Hermitian (row-only gathers, exact Hermiticity preserved), 0: general state (row and column gathers).  links: DEVICE
 // [nodes][lrow] int32 written by hpipe_pack_links (neighbour entries are element offsets slot*N*N, uint16
 // occupation records, and the row ends with the node's damping rate).  a_plus, a_minus_x, a_minus_o,
 // H_host, delta_host: HOST (the per-mode constants travel in the kernel parameters).  warps <= 0: as
@@ -70,8 +71,8 @@ void hpipe_pack_links(int N, int M, int D, const int32_t* plus, const int32_t* m
                       double damp, int32_t* row);
 cudaError_t launch_rhs_hpipe(const RhsParams& p, const int32_t* links, int lrow, const double* a_plus,
                              const double* a_minus_x, const double* a_minus_o, const double* H_host,
-                             const double* delta_host, int warps, int sms, unsigned long long* tickets,
-                             unsigned long long* ticket_base, cudaStream_t s);
+                             const double* delta_host, int hermitian, int warps, int sms,
+                             unsigned long long* tickets, unsigned long long* ticket_base, cudaStream_t s);
 
 // Tensor-core (DMMA) kernel for N = 32, 64, 96 (kernels_large.cu), any state.  lptr: DEVICE [nodes+1] CSR
 // offsets; lent: DEVICE int4 link entries {neighbour slot, mode l, 0 "+" | 1 "-", n_l}; Hs_dev: DEVICE

@@ -31,6 +31,14 @@
 //     pass), predicated, from pre-multiplied element offsets (one IMAD.WIDE + one LDG per link);
 //   * the epilogue updates XA (next stage input) and AC (running sum) in place in shared memory and
 //     lane 0 writes them back with cp.async.bulk (shared -> global, bulk async-group).
+//
+// GENERAL (non-Hermitian) states, e.g. the mu rho(0) of linear absorption, use the same
+// pipeline with HERM = false: lane (g,j) forms column j of k_u directly,
+//     k[:,j] = -i (H sigma)[:,j] + i sigma H[:,j] - (d_u + T[:,j]) o sigma[:,j]
+//              + sum_l f_l (row part: element (b,j) of the neighbour's row b -- the same loads as above)
+//              + sum_{l in bath j} f'_l sigma_{u +- e_l}[:,j]     (column part: the lane's own bath, a strided
+//                                                                 column of the neighbour, Eq. 23, 25)
+// with sigma H from the whole sigma tile (broadcast shared-memory reads) and no transposition.
 #include "kernels.cuh"
 
 #include <cmath>
@@ -49,6 +57,7 @@ struct PipeCfg {
   static constexpr int G = 32 / LP;                   // nodes per warp pass
   static constexpr int S = 2;                         // ring slots per warp
   static constexpr int MAXW = (N <= 8) ? 12 : 6;      // warps per CTA (fewer if shared memory is short)
+  static constexpr int MAXW_GENERAL = (N <= 8) ? 8 : 6;   // general states need more registers per thread
   static constexpr int SMEM_BUDGET = 224 * 1024;
   static constexpr int KB = (16 / N) > 0 ? (16 / N) : 1;   // mode indices kk per gather batch (<= 32 loads)
   static constexpr int NP4 = (N + 3) / 4 * 4;         // ints per index group
@@ -140,8 +149,8 @@ __device__ __forceinline__ void ldg_link(double2& r, const double2* base, int of
       "}\n" : "+d"(r.x), "+d"(r.y) : "l"(base), "r"(off), "l"(pol));
 }
 
-template <int N>
-__global__ void __launch_bounds__(PipeCfg<N>::MAXW * 32, 1)
+template <int N, bool HERM>
+__global__ void __launch_bounds__((HERM ? PipeCfg<N>::MAXW : PipeCfg<N>::MAXW_GENERAL) * 32, 1)
 rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   using C = PipeCfg<N>;
   constexpr int NN = C::NN, G = C::G, S = C::S, KB = C::KB, PS = C::PS, RS = C::RS, SZ = C::SZ;
@@ -155,9 +164,13 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   const int warp_bytes = S * slot_bytes + 2 * AB;
   int32_t* sNull = reinterpret_cast<int32_t*>(smem_raw + CW * warp_bytes);    // [lrow]
   double2* sSQ = reinterpret_cast<double2*>(sNull + lrow);                    // [kMaxSqrt][2]
-  unsigned long long* bars = reinterpret_cast<unsigned long long*>(sSQ + 2 * kMaxSqrt);
+  double* sCoef = reinterpret_cast<double*>(sSQ + 2 * kMaxSqrt);              // [3][kMaxModes]: cP, cX, cO (lane-indexed)
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(sCoef + 3 * kMaxModes);
   for (int e = threadIdx.x; e < 2 * kMaxSqrt; e += blockDim.x)
     sSQ[e] = make_double2(sqrt((double)(e >> 1)), (e & 1) ? sqrt((double)((e >> 1) + 1)) : 0.0);
+  for (int e = threadIdx.x; e < kMaxModes; e += blockDim.x) {
+    sCoef[e] = P.cP[e]; sCoef[kMaxModes + e] = P.cX[e]; sCoef[2 * kMaxModes + e] = P.cO[e];
+  }
 
   // a null meta row: every link invalid, every occupation record 0 (all coupling factors vanish)
   for (int e = threadIdx.x; e < lrow; e += blockDim.x) sNull[e] = (e < M * GROUP && (e % GROUP) < 2 * NP4) ? -1 : 0;
@@ -227,6 +240,11 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   const int j = lane_used ? lane % LP : 0;            // idle lanes shadow column 0 of their node
   const double my_delta = P.delta[j];
   const double2* xj = p.x + j;
+  double hcol[HERM ? 1 : N];                          // general states: column j of H / hbar
+  if (!HERM) {
+#pragma unroll
+    for (int m = 0; m < N; ++m) hcol[m] = P.H[m * N + j];
+  }
 
   int s = 0, ab = 0;                                  // ring slot and AC buffer of this pass
   unsigned ph = 0, pha = 0;                           // their mbarrier phases
@@ -248,11 +266,25 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     const int32_t* lk = active ? sL + tl * lrow : sNull;
 
     // ---- Z = -(i/hbar) H sigma - (d_u + T)/2 o sigma, column j (Eq. 12-14) ----------------------
+    // (general states: z = column j of -(i/hbar)[H, sigma] - (d_u + T) o sigma, the whole term)
     double2 z[N];
     {
       double2 col[N];
 #pragma unroll
       for (int m = 0; m < N; ++m) col[m] = sig[m * N + j];
+      double2 sh[HERM ? 1 : N];                     // general states: (sigma H / hbar)[i][j]
+      if (!HERM) {
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+          double ar = 0.0, ai = 0.0;
+#pragma unroll
+          for (int m = 0; m < N; ++m) {
+            const double2 v = sig[i * N + m];       // broadcast within the node
+            ar = fma(v.x, hcol[m], ar); ai = fma(v.y, hcol[m], ai);
+          }
+          sh[i] = make_double2(ar, ai);
+        }
+      }
       if (need_Y) {
         // the sigma columns are in registers: XA is dead, stream the step-start state y into it
         fence_async_smem();
@@ -270,8 +302,13 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
 #pragma unroll
         for (int m = 0; m < N; ++m) { zr = fma(P.H[b * N + m], col[m].x, zr); zi = fma(P.H[b * N + m], col[m].y, zi); }
         const double hd = (b == j) ? mhd : fma(-0.5, P.delta[b] + my_delta, mhd);   // Eq. 14 with Eq. 24
-        z[b].x = fma(hd, col[b].x, zi);             // -i (zr + i zi) = zi - i zr
-        z[b].y = fma(hd, col[b].y, -zr);
+        if (HERM) {
+          z[b].x = fma(hd, col[b].x, zi);           // -i (zr + i zi) = zi - i zr
+          z[b].y = fma(hd, col[b].y, -zr);
+        } else {                                    // -i (H sigma - sigma H) - (d_u + T) sigma
+          z[b].x = fma(2.0 * hd, col[b].x, zi - sh[b].y);
+          z[b].y = fma(2.0 * hd, col[b].y, sh[b].x - zr);
+        }
       }
     }
 
@@ -358,19 +395,49 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
       }
     }
 
-    // ---- k = Z + Z^dagger, column j, through the scratch (conflict-free row stride RS) -----------
-    __syncwarp();
-    if (active) {
-#pragma unroll
-      for (int b = 0; b < N; ++b) scr[g * SZ + b * RS + j] = z[b];
-    }
-    __syncwarp();
     double2 k[N];
+    if (HERM) {
+      // ---- k = Z + Z^dagger, column j, through the scratch (conflict-free row stride RS) ---------
+      __syncwarp();
+      if (active) {
 #pragma unroll
-    for (int i = 0; i < N; ++i) {
-      const double2 zt = scr[tl * SZ + j * RS + i];                // Z[j][i]
-      k[i].x = z[i].x + zt.x;
-      k[i].y = z[i].y - zt.y;
+        for (int b = 0; b < N; ++b) scr[g * SZ + b * RS + j] = z[b];
+      }
+      __syncwarp();
+#pragma unroll
+      for (int i = 0; i < N; ++i) {
+        const double2 zt = scr[tl * SZ + j * RS + i];              // Z[j][i]
+        k[i].x = z[i].x + zt.x;
+        k[i].y = z[i].y - zt.y;
+      }
+    } else {
+      // ---- general states: column part of the couplings (Eq. 15-17 with Eq. 23, 25): the modes of the
+      //      lane's OWN bath b = j act on column j, elements (i, j) of the neighbour, i = 0..N-1 ----------
+      for (int kk = 0; kk < M; ++kk) {
+        const int32_t* grp = lk + kk * GROUP;
+        const int up = grp[j], dn = grp[NP4 + j];
+        double2 wu[N], wd[N];
+#pragma unroll
+        for (int i = 0; i < N; ++i) { wu[i] = make_double2(0.0, 0.0); wd[i] = make_double2(0.0, 0.0); }
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+          ldg_link(wu[i], xj + i * N, up, pol_keep);
+          ldg_link(wd[i], xj + i * N, dn, pol_keep);
+        }
+        const unsigned rec = reinterpret_cast<const unsigned short*>(grp + 2 * NP4)[j];
+        const double2 sq = *reinterpret_cast<const double2*>(reinterpret_cast<const unsigned char*>(sSQ) + rec);
+        const int l = j * M + kk;
+        const double a = sq.y * sCoef[l], ax = sq.x * sCoef[kMaxModes + l], ao = sq.x * sCoef[2 * kMaxModes + l];
+#pragma unroll
+        for (int i = 0; i < N; ++i) {               // V^x = -1, V^o = +1 on column b
+          z[i].x = fma(a, wu[i].y, z[i].x); z[i].y = fma(-a, wu[i].x, z[i].y);                 // -i a+ sigma^+
+          z[i].x = fma(ao, wd[i].x, fma(ax, wd[i].y, z[i].x));                                 // (-i a-x + a-o) sigma^-
+          z[i].y = fma(ao, wd[i].y, fma(-ax, wd[i].x, z[i].y));
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < N; ++i) k[i] = z[i];
+      __syncwarp();
     }
     if (need_A && qn < npass) {
       // the scratch is free again: bring the next pass's running sum (already in L2) into it
@@ -439,18 +506,18 @@ template <int N>
 size_t hpipe_smem(int lrow, int warps) {
   using C = PipeCfg<N>;
   return (size_t)warps * (C::S * ((size_t)C::XB + (size_t)C::G * lrow * 4) + 2 * (size_t)C::AB) +
-         (size_t)lrow * 4 + 2 * kMaxSqrt * 16 + (size_t)warps * (2 * C::S + 2) * 8;
+         (size_t)lrow * 4 + 2 * kMaxSqrt * 16 + 3 * kMaxModes * 8 + (size_t)warps * (2 * C::S + 2) * 8;
 }
 // warps per CTA: as many as fit into the shared-memory budget (0 if not even one fits)
 template <int N>
-int hpipe_warps(int lrow) {
+int hpipe_warps(int lrow, bool herm = true) {
   using C = PipeCfg<N>;
-  int w = C::MAXW;
+  int w = herm ? C::MAXW : C::MAXW_GENERAL;
   while (w >= 1 && hpipe_smem<N>(lrow, w) > (size_t)C::SMEM_BUDGET) --w;
   return w;
 }
 
-template <int N>
+template <int N, bool HERM>
 cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, const double* a_plus,
                            const double* a_minus_x, const double* a_minus_o, const double* H_host,
                            const double* delta_host, int warps, int sms, unsigned long long* tickets,
@@ -459,7 +526,7 @@ cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, c
   PipeParams<N> P;
   P.p = p; P.links = links; P.lrow = lrow;
   P.npass = (p.nodes + C::G - 1) / C::G;
-  const int wmax = hpipe_warps<N>(lrow);
+  const int wmax = hpipe_warps<N>(lrow, HERM);
   if (wmax < 1) return cudaErrorInvalidValue;
   P.nwarps = (warps > 0 && warps < wmax) ? warps : wmax;
   for (int e = 0; e < N * N; ++e) P.H[e] = H_host[e] * p.inv_hbar;
@@ -474,7 +541,7 @@ cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, c
   const size_t smem = hpipe_smem<N>(lrow, P.nwarps);
   static size_t configured = 0;
   if (smem > configured) {
-    cudaError_t e = cudaFuncSetAttribute(rhs_hpipe_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(rhs_hpipe_kernel<N, HERM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = smem;
   }
@@ -484,7 +551,7 @@ cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, c
   P.tickets = tickets;
   P.ticket_base = *ticket_base;
   *ticket_base += (unsigned long long)P.npass + 2ULL * grid * P.nwarps;   // two failing draws per warp
-  rhs_hpipe_kernel<N><<<grid, P.nwarps * 32, smem, s>>>(P);
+  rhs_hpipe_kernel<N, HERM><<<grid, P.nwarps * 32, smem, s>>>(P);
   return cudaGetLastError();
 }
 
@@ -540,11 +607,15 @@ void hpipe_pack_links(int N, int M, int D, const int32_t* plus, const int32_t* m
 
 cudaError_t launch_rhs_hpipe(const RhsParams& p, const int32_t* links, int lrow, const double* a_plus,
                              const double* a_minus_x, const double* a_minus_o, const double* H_host,
-                             const double* delta_host, int warps, int sms, unsigned long long* tickets,
-                             unsigned long long* ticket_base, cudaStream_t s) {
+                             const double* delta_host, int hermitian, int warps, int sms,
+                             unsigned long long* tickets, unsigned long long* ticket_base, cudaStream_t s) {
   switch (p.N) {
-#define HEOM_HPIPE_CASE(n) \
-  case n: return launch_hpipe_t<n>(p, links, lrow, a_plus, a_minus_x, a_minus_o, H_host, delta_host, warps, sms, tickets, ticket_base, s);
+#define HEOM_HPIPE_CASE(n)                                                                                          \
+  case n:                                                                                                           \
+    return hermitian ? launch_hpipe_t<n, true>(p, links, lrow, a_plus, a_minus_x, a_minus_o, H_host, delta_host,  \
+                                               warps, sms, tickets, ticket_base, s)                                \
+                     : launch_hpipe_t<n, false>(p, links, lrow, a_plus, a_minus_x, a_minus_o, H_host, delta_host, \
+                                                warps, sms, tickets, ticket_base, s);
     HEOM_HPIPE_ALL(HEOM_HPIPE_CASE)
 #undef HEOM_HPIPE_CASE
     default: return cudaErrorInvalidValue;
