@@ -244,8 +244,9 @@ def main():
         achieved = alg_bytes_per_launch / avg_launch_s / 1e9
         # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
         # (average over the 4 stage launches of one RK4 step), or null where no capture exists
-        ncu_traffic = {"cfg2_fmo7": (963.8e6, "profiles/r1b_cfg2_hpipe.md"),
-                       "cfg5_large96": (94.4e9, "profiles/r1b_cfg5_large.md")}.get(w.name, (None, None))
+        ncu_traffic = {"cfg2_fmo7": (965.0e6, "profiles/r1c_cfg2_hpipe.md"),
+                       "cfg3_deep7": (36.6e9, "profiles/r1c_cfg3_hpipe.md"),
+                       "cfg5_large96": (94.4e9, "profiles/r1c_cfg5_large.md")}.get(w.name, (None, None))
         if w.N >= 32:
             # arithmetic-bound (N/8 = 12 flop/B at N = 96): FP64 pipe (DMMA) roofline
             tf = alg_flops_per_launch / avg_launch_s / 1e12

@@ -124,13 +124,9 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
   auto load_sigma = [&](int node) {
     if (lane == 0) lmbar_expect_tx(bar, node < nodes ? (unsigned)NN * 16 : 0u);
     __syncwarp();
-#ifdef HEOM_LARGE_ONECOPY   /* timing experiment only: dense layout, wrong results */
-    if (node < nodes && lane == 0) lbulk_g2s(sS, p.x + (size_t)node * NN, NN * 16, bar);
-#else
     if (node < nodes)
       for (int row = lane; row < N; row += 32)
         lbulk_g2s(sS + row * SS, p.x + (size_t)node * NN + (size_t)row * N, N * 16, bar);
-#endif
   };
   auto draw = [&]() -> int {
     const unsigned long long tk = atomicAdd(P.tickets, 1ULL) - P.ticket_base;
