@@ -164,7 +164,10 @@ size_t rhs_generic_smem(int N) {
 cudaError_t launch_rhs_generic(const RhsParams& p, cudaStream_t s) {
   const size_t smem = rhs_generic_smem(p.N);
   if (smem == 0) return cudaErrorInvalidValue;
-  static size_t configured = 0;
+  static size_t configured_on[64] = {};   // per device: the attribute belongs to the device's context
+  int dev_ = 0;
+  cudaGetDevice(&dev_);
+  size_t& configured = configured_on[dev_ & 63];
   if (smem > 48 * 1024 && smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(rhs_generic_kernel,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -277,7 +277,10 @@ cudaError_t launch_herm_t(const RhsParams& p, const int32_t* links, int lrow, co
   for (int e = 0; e < N * N; ++e) P.H[e] = H_host[e];
   for (int e = 0; e < N; ++e) P.delta[e] = delta_host[e];
   const size_t smem = herm_smem<N>(p.W, p.D, lrow);
-  static size_t configured = 0;
+  static size_t configured_on[64] = {};   // per device: the attribute belongs to the device's context
+  int dev_ = 0;
+  cudaGetDevice(&dev_);
+  size_t& configured = configured_on[dev_ & 63];
   if (smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(rhs_herm_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

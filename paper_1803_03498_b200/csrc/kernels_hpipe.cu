@@ -539,7 +539,10 @@ cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, c
     P.cO[l] = on ? a_minus_o[(size_t)l * D1 + 1] : 0.0;     // sqrt(1 / s_l) lambda nu / hbar
   }
   const size_t smem = hpipe_smem<N>(lrow, P.nwarps);
-  static size_t configured = 0;
+  static size_t configured_on[64] = {};   // per device: the attribute belongs to the device's context
+  int dev_ = 0;
+  cudaGetDevice(&dev_);
+  size_t& configured = configured_on[dev_ & 63];
   if (smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(rhs_hpipe_kernel<N, HERM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

@@ -336,7 +336,10 @@ cudaError_t launch_large_t(const RhsParams& p, const int64_t* lptr, const int4* 
     P.cO[l] = on ? a_minus_o[(size_t)l * D1 + 1] : 0.0;
   }
   const size_t smem = large_smem<N>();
-  static bool configured = false;
+  static bool configured_on[64] = {};     // per device: the attribute belongs to the device's context
+  int dev_ = 0;
+  cudaGetDevice(&dev_);
+  bool& configured = configured_on[dev_ & 63];
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(rhs_large_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

@@ -85,6 +85,19 @@ def test_argument_validation_without_gpu():
         g.set_option("no_such_option", 1)
 
 
+def test_option_validation_without_gpu():
+    g = Heom(np.zeros((3, 3)), 35.0, 0.02, 300.0, 2, 2)
+    for name, good, bad in [("order", 0, 2), ("kernel", 2, 3), ("rk4_form", 0, 2), ("l2_fetch", 64, 48),
+                            ("warps_per_cta", 4, 99)]:
+        g.set_option(name, good)
+        with pytest.raises(HeomError) as e:
+            g.set_option(name, bad)
+        assert e.value.status == -1
+    for name in ("timing", "hermitian", "acc_red", "pade"):
+        g.set_option(name, 1)
+        g.set_option(name, 0)
+
+
 def test_no_cpu_fallback():
     """Without a GPU the compute path must fail loudly, never fall back."""
     import torch
