@@ -53,6 +53,7 @@ struct heom_ctx {
   int lrowP = 0;
   int warps_per_cta = 0;     // option "warps_per_cta": 0 = as many as fit
   // tensor-core kernel for large N (kernels_large.cu)
+  bool use_tiny = false;     // whole-propagation kernel for tiny hierarchies (kernels_tiny.cu)
   bool use_large = false;
   int64_t* d_lptr = nullptr;
   void* d_lent = nullptr;
@@ -358,6 +359,7 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->lrowH = herm_links_row(ctx->h.N, ctx->h.M);
   ctx->use_herm = ctx->kernel >= 1 && herm_supported(ctx->h.N, ctx->h.W, ctx->h.D);
   ctx->use_large = ctx->kernel == 1 && large_supported(ctx->h.N, ctx->h.W);
+  ctx->use_tiny = ctx->kernel == 1 && tiny_supported(ctx->h.N, ctx->h.W, ctx->h.D, (long long)ctx->h.nodes);
   ctx->d_Hs = (double*)(base + L.off_Hs);
   ctx->d_delta = (double*)(base + L.off_delta);
   ctx->d_lptr = (int64_t*)(base + L.off_lptr);
@@ -561,6 +563,22 @@ heom_status heom_rk4_steps(heom_ctx* ctx, double dt, int nsteps) {
   if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
   RhsParams p = base_params(ctx);
   p.rhs_only = 0;
+  if (ctx->use_tiny && nsteps > 0) {
+    /* launch-latency-bound hierarchies: all nsteps classical RK4 steps in one launch of one CTA */
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (ctx->timing) {
+      while (ctx->ev_used + 2 > ctx->ev.size()) { cudaEvent_t e; CU(cudaEventCreate(&e)); ctx->ev.push_back(e); }
+      e0 = ctx->ev[ctx->ev_used]; e1 = ctx->ev[ctx->ev_used + 1];
+      ctx->ev_used += 2;
+      CU(cudaEventRecord(e0, ctx->stream));
+    }
+    p.x = ctx->y;
+    CU(launch_rk4_tiny(p, dt, nsteps, ctx->stream));
+    ctx->launches += 1;
+    if (ctx->timing) CU(cudaEventRecord(e1, ctx->stream));
+    return HEOM_OK;
+  }
+  if (nsteps == 0) return HEOM_OK;
   if (ctx->use_large && ctx->rk4_form != 0) {
     /* Taylor/Horner form (R6): v1 = dt f(y), v_s = (dt/s) f(v_{s-1}), y' = y + v1 + v2 + v3 + v4 -- the
      * classical RK4 result for a linear autonomous f, regrouped.  acc = y + v1 is stored, v2..v4 are

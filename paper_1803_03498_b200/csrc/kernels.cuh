@@ -83,6 +83,11 @@ cudaError_t launch_rhs_large(const RhsParams& p, const int64_t* lptr, const void
                              const double* a_minus_o, int sms, unsigned long long* tickets,
                              unsigned long long* ticket_base, cudaStream_t s);
 
+// Whole-propagation kernel for tiny hierarchies (kernels_tiny.cu): nsteps classical RK4 steps of the state p.x
+// (DEVICE, storage-slot order, updated in place) inside ONE launch of one CTA; tables as for the generic kernel.
+bool tiny_supported(int N, int W, int D, long long nodes);
+cudaError_t launch_rk4_tiny(const RhsParams& p, double dt, int nsteps, cudaStream_t s);
+
 // dst[slot_of[u]*dst_stride + e] = src[u*NN + e]  (to_device=1) or the inverse (to_device=0)
 cudaError_t launch_permute(const double2* src, double2* dst, const int32_t* slot_of, int nodes,
                            int NN, int stride, int to_device, cudaStream_t s);

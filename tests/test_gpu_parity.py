@@ -81,10 +81,12 @@ def test_rhs_parity_hermitian_state(N, K, D, order):
     assert rel_err(g.rhs(), o.rhs()) < RHS_TOL
 
 
-def test_dimer_1000_steps():
-    """BASELINE config 1 in full."""
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_dimer_1000_steps(kernel):
+    """BASELINE config 1 in full: kernel = 1 propagates it in one launch of the tiny-hierarchy kernel, kernel = 2
+    stage by stage."""
     w = workloads.dimer()
-    o, g = _pair(w)
+    o, g = _pair(w, kernel=kernel)
     o.set_state(w.sigma0()); g.set_state(w.sigma0())
     o.rk4_steps(w.dt_fs, w.steps); g.rk4_steps(w.dt_fs, w.steps)
     ref, got = o.get_full_state(), g.get_full_state()
@@ -244,4 +246,10 @@ def test_call_order_errors_on_gpu():
     g.set_state(w.sigma0())
     n0 = g.launch_count()
     g.rk4_steps(1.0, 3)
-    assert g.launch_count() - n0 == 12      # 4 fused stage kernels per step, nothing else
+    assert g.launch_count() - n0 == 1       # a tiny hierarchy: the whole propagation is one launch (kernels_tiny.cu)
+    g2 = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, kernel=2).bind()
+    g2.set_state(w.sigma0())
+    n0 = g2.launch_count()
+    g2.rk4_steps(1.0, 3)
+    assert g2.launch_count() - n0 == 12     # otherwise 4 fused stage kernels per step, nothing else
+    assert rel_err(g2.get_full_state(), g.get_full_state()) < 1e-12
