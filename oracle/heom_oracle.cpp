@@ -51,7 +51,12 @@ const double PI = 3.14159265358979323846;
 }  // namespace
 
 struct oracle_ctx {
-  int N = 0;       /* sites = states = baths (per-site baths)          */
+  int N = 0;       /* system states (rows of every sigma_u)                   */
+  int B = 0;       /* baths; bath b couples to the projector |site[b]><site[b]|
+                      (S(b) = 1).  oracle_create: B = N, site[b] = b;
+                      oracle_create_sites: any injective map, e.g. a ground state
+                      without a bath for linear absorption      */
+  std::vector<int> site;        /* [B] bs(b): the state bath b couples to      */
   int K = 0;       /* Matsubara terms beyond the Drude pole                   */
   int M = 0;       /* modes per bath = K+1 = the paper's K             */
   int W = 0;       /* tuple length W = B*K_paper                        */
@@ -63,13 +68,13 @@ struct oracle_ctx {
   int pade = 0;      /* 0 = Matsubara poles (Eq. 19-20), 1 = Pade poles (Eq. 27-33) */
   double T_kelvin = 0;
   std::vector<double> H;        /* [N][N] cm^-1                               */
-  std::vector<double> lambda;   /* [N] cm^-1                                  */
-  std::vector<double> nu;       /* [N] fs^-1                                  */
+  std::vector<double> lambda;   /* [B] cm^-1                                  */
+  std::vector<double> nu;       /* [B] fs^-1                                  */
   double beta_hbar = 0;         /* beta*hbar = hbar/(k_B T), fs               */
   std::vector<double> gamma;    /* [W] Eq. 19, fs^-1                          */
   std::vector<double> c_re;     /* [W] Re c(b,k)/hbar, Eq. 20, fs^-2          */
   std::vector<double> c_im;     /* [W] Im part carried by Eq. 17's V^o term   */
-  std::vector<double> delta;    /* [N] Eq. 14 bracket, fs^-1                  */
+  std::vector<double> delta;    /* [B] Eq. 14 bracket, fs^-1                  */
   std::vector<uint8_t> tuples;  /* [nodes][W]                                 */
   std::vector<int32_t> plus;    /* [nodes][W]                                 */
   std::vector<int32_t> minus;   /* [nodes][W]                                 */
@@ -233,7 +238,7 @@ void pade_poles(int K, std::vector<double>& xi, std::vector<double>& eta) {
 }
 
 int build_coefficients(oracle_ctx* c, double T_kelvin) {
-  const int N = c->N, M = c->M;
+  const int N = c->B, M = c->M;   /* loop over baths */
   c->beta_hbar = HBAR_CM_FS / (KB_CM_PER_K * T_kelvin);
   c->gamma.assign((size_t)c->W, 0.0);
   c->c_re.assign((size_t)c->W, 0.0);
@@ -324,18 +329,18 @@ void rhs_node(const oracle_ctx* c, const cplx* st, int64_t u, cplx* out) {
   for (int l = 0; l < W; ++l) damp += (double)n[l] * c->gamma[l];
   for (size_t e = 0; e < NN; ++e) out[e] -= damp * s[e];
 
-  /* Eq. 14:  - sum_b [ ... ] V_b^x V_b^x sigma_u   (S(b)=1, bs(b)=b) */
+  /* Eq. 14:  - sum_b [ ... ] V_b^x V_b^x sigma_u   (S(b)=1, V_b = |bs(b)><bs(b)|) */
   if (c->terminator)
-    for (int b = 0; b < N; ++b)
+    for (int b = 0; b < c->B; ++b)
       for (int i = 0; i < N; ++i)
         for (int j = 0; j < N; ++j)
-          out[(size_t)i * N + j] -= c->delta[b] * VxVx(b, i, j) * s[(size_t)i * N + j];
+          out[(size_t)i * N + j] -= c->delta[b] * VxVx(c->site[b], i, j) * s[(size_t)i * N + j];
 
   /* Eq. 15 -> Eq. 35:  + sum_{b,k} i sqrt((n+1)|c|) V_b^x sigma^+_{(u,b,k)} */
   for (int l = 0; l < W; ++l) {
     const int32_t up = c->plus[(size_t)u * W + l];
     if (up < 0) continue; /* invalid link contributes nothing */
-    const int b = l / M;  /* Eq. 11 */
+    const int b = c->site[l / M];  /* Eq. 11, then bs(b) */
     const cplx* sp = st + (size_t)up * NN;
     const double f = c->scaling ? std::sqrt(((double)n[l] + 1.0) * abs_c(c, l)) : 1.0;
     for (int i = 0; i < N; ++i)
@@ -350,7 +355,7 @@ void rhs_node(const oracle_ctx* c, const cplx* st, int64_t u, cplx* out) {
   for (int l = 0; l < W; ++l) {
     const int32_t um = c->minus[(size_t)u * W + l];
     if (um < 0) continue;
-    const int b = l / M, k = l % M;
+    const int b = c->site[l / M], k = l % M;
     const cplx* sm = st + (size_t)um * NN;
     double f;
     if (c->scaling) {
@@ -378,24 +383,29 @@ void rhs_all(const oracle_ctx* c, const cplx* st, cplx* out) {
 
 extern "C" {
 
-int oracle_create(oracle_ctx** out, int n_sites, const double* H_cm, const double* lambda_cm,
-                  const double* nu_per_fs, double T_kelvin, int K, int D) {
-  if (!out || !H_cm || !lambda_cm || !nu_per_fs) return -1;
-  if (n_sites < 1 || K < 0 || D < 0 || D > 255 || !(T_kelvin > 0.0)) return -1;
-  for (int i = 0; i < n_sites; ++i) {
-    if (!(lambda_cm[i] >= 0.0) || !(nu_per_fs[i] > 0.0)) return -1;
-    for (int j = 0; j < n_sites; ++j) {
-      if (!std::isfinite(H_cm[i * n_sites + j])) return -1;
-      if (H_cm[i * n_sites + j] != H_cm[j * n_sites + i]) return -1;
-    }
+int oracle_create_sites(oracle_ctx** out, int n_states, const double* H_cm, int n_baths,
+                        const int* bath_state, const double* lambda_cm, const double* nu_per_fs,
+                        double T_kelvin, int K, int D) {
+  if (!out || !H_cm || !lambda_cm || !nu_per_fs || !bath_state) return -1;
+  if (n_states < 1 || n_baths < 1 || n_baths > n_states || K < 0 || D < 0 || D > 255 || !(T_kelvin > 0.0)) return -1;
+  for (int b = 0; b < n_baths; ++b) {
+    if (!(lambda_cm[b] >= 0.0) || !(nu_per_fs[b] > 0.0)) return -1;
+    if (bath_state[b] < 0 || bath_state[b] >= n_states) return -1;
+    for (int b2 = 0; b2 < b; ++b2) if (bath_state[b2] == bath_state[b]) return -1;   /* one bath per state */
   }
+  for (int i = 0; i < n_states; ++i)
+    for (int j = 0; j < n_states; ++j) {
+      if (!std::isfinite(H_cm[i * n_states + j])) return -1;
+      if (H_cm[i * n_states + j] != H_cm[j * n_states + i]) return -1;
+    }
   oracle_ctx* c = new (std::nothrow) oracle_ctx();
   if (!c) return -2;
   try {
-    c->N = n_sites; c->K = K; c->M = K + 1; c->W = n_sites * (K + 1); c->D = D;
-    c->H.assign(H_cm, H_cm + (size_t)n_sites * n_sites);
-    c->lambda.assign(lambda_cm, lambda_cm + n_sites);
-    c->nu.assign(nu_per_fs, nu_per_fs + n_sites);
+    c->N = n_states; c->B = n_baths; c->K = K; c->M = K + 1; c->W = n_baths * (K + 1); c->D = D;
+    c->site.assign(bath_state, bath_state + n_baths);
+    c->H.assign(H_cm, H_cm + (size_t)n_states * n_states);
+    c->lambda.assign(lambda_cm, lambda_cm + n_baths);
+    c->nu.assign(nu_per_fs, nu_per_fs + n_baths);
     c->T_kelvin = T_kelvin;
     if (build_coefficients(c, T_kelvin) != 0) { delete c; return -1; }
     std::vector<uint8_t> cur((size_t)c->W, 0);
@@ -409,6 +419,15 @@ int oracle_create(oracle_ctx** out, int n_sites, const double* H_cm, const doubl
   }
   *out = c;
   return 0;
+}
+
+/* Per-site baths: one bath per state, bath b on state b (BASELINE.json's five configurations). */
+int oracle_create(oracle_ctx** out, int n_sites, const double* H_cm, const double* lambda_cm,
+                  const double* nu_per_fs, double T_kelvin, int K, int D) {
+  if (n_sites < 1) return -1;
+  std::vector<int> ident((size_t)n_sites);
+  for (int b = 0; b < n_sites; ++b) ident[(size_t)b] = b;
+  return oracle_create_sites(out, n_sites, H_cm, n_sites, ident.data(), lambda_cm, nu_per_fs, T_kelvin, K, D);
 }
 
 void oracle_destroy(oracle_ctx* c) { delete c; }
@@ -433,6 +452,7 @@ int oracle_pade_poles(int K, double* xi, double* eta) {
 
 int64_t oracle_num_nodes(const oracle_ctx* c) { return c ? c->nodes : -1; }
 int oracle_num_modes(const oracle_ctx* c) { return c ? c->W : -1; }
+int oracle_num_baths(const oracle_ctx* c) { return c ? c->B : -1; }
 int oracle_num_threads(const oracle_ctx* c) { return c ? nthreads(c) : -1; }
 
 int oracle_get_tables(const oracle_ctx* c, uint8_t* tuples, int32_t* plus, int32_t* minus) {

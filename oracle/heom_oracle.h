@@ -38,6 +38,14 @@ typedef struct oracle_ctx oracle_ctx;
 int  oracle_create(oracle_ctx** out, int n_sites, const double* H_cm,
                    const double* lambda_cm, const double* nu_per_fs,
                    double T_kelvin, int K, int D);
+/* Same, for a system whose states do not all carry a bath (the ground state |0> of
+ * linear absorption, Eq. 53, 56; "each bath couples to one state"): n_states system states,
+ * n_baths <= n_states baths, bath b couples through the projector on state bath_state[b] (0-based, all
+ * different).  lambda_cm, nu_per_fs have n_baths entries; W = n_baths*(K+1); delta has n_baths entries.
+ * oracle_create(n) == oracle_create_sites(n, n, {0..n-1}). */
+int  oracle_create_sites(oracle_ctx** out, int n_states, const double* H_cm, int n_baths,
+                         const int* bath_state, const double* lambda_cm, const double* nu_per_fs,
+                         double T_kelvin, int K, int D);
 void oracle_destroy(oracle_ctx* ctx);
 
 /* Options (set before any rhs/rk4 call; defaults in brackets):
@@ -56,7 +64,8 @@ int  oracle_set_option(oracle_ctx* ctx, const char* name, int value);
 int  oracle_pade_poles(int K, double* xi, double* eta);
 
 int64_t oracle_num_nodes(const oracle_ctx* ctx);   /* Eq. 9: C(W+D, W)        */
-int     oracle_num_modes(const oracle_ctx* ctx);   /* W = n_sites*(K+1)       */
+int     oracle_num_modes(const oracle_ctx* ctx);   /* W = n_baths*(K+1)       */
+int     oracle_num_baths(const oracle_ctx* ctx);
 int     oracle_num_threads(const oracle_ctx* ctx); /* threads the loops use   */
 
 /* tuples uint8 [nodes][W]; plus/minus int32 [nodes][W], -1 = invalid link
@@ -64,7 +73,7 @@ int     oracle_num_threads(const oracle_ctx* ctx); /* threads the loops use   */
 int  oracle_get_tables(const oracle_ctx* ctx, uint8_t* tuples,
                        int32_t* plus, int32_t* minus);
 /* gamma[W], c_re[W], c_im[W] (c-hat = c/hbar in fs^-2; c_im is non-zero for
- * k=0 only and equals -(lambda_b/hbar) nu_b), delta[n_sites] (Eq. 14 bracket,
+ * k=0 only and equals -(lambda_b/hbar) nu_b), delta[n_baths] (Eq. 14 bracket,
  * fs^-1). */
 int  oracle_get_coefficients(const oracle_ctx* ctx, double* gamma, double* c_re,
                              double* c_im, double* delta);

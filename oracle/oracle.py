@@ -24,6 +24,9 @@ def _load():
     dp = C.POINTER(C.c_double)
     lib.oracle_create.argtypes = [C.POINTER(P), C.c_int, dp, dp, dp, C.c_double, C.c_int, C.c_int]
     lib.oracle_create.restype = C.c_int
+    lib.oracle_create_sites.argtypes = [C.POINTER(P), C.c_int, dp, C.c_int, C.POINTER(C.c_int), dp, dp,
+                                        C.c_double, C.c_int, C.c_int]
+    lib.oracle_create_sites.restype = C.c_int
     lib.oracle_destroy.argtypes = [P]
     lib.oracle_destroy.restype = None
     lib.oracle_set_option.argtypes = [P, C.c_char_p, C.c_int]
@@ -62,15 +65,23 @@ class Oracle:
     """One truncated hierarchy on the CPU.  Arguments as heom_oracle.h."""
 
     def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, scaling=1, terminator=1,
-                 threads=0, pade=0):
+                 threads=0, pade=0, bath_state=None):
+        """bath_state=None: one bath per state (oracle_create); else a list of the states the baths couple
+        to (oracle_create_sites), lambda_cm / nu_per_fs then have one entry per bath."""
         lib = _load()
         H = np.ascontiguousarray(H_cm, dtype=np.float64)
         self.N = H.shape[0]
-        lam = np.ascontiguousarray(np.broadcast_to(lambda_cm, (self.N,)), dtype=np.float64)
-        nu = np.ascontiguousarray(np.broadcast_to(nu_per_fs, (self.N,)), dtype=np.float64)
+        self.B = self.N if bath_state is None else len(bath_state)
+        lam = np.ascontiguousarray(np.broadcast_to(lambda_cm, (self.B,)), dtype=np.float64)
+        nu = np.ascontiguousarray(np.broadcast_to(nu_per_fs, (self.B,)), dtype=np.float64)
         h = C.c_void_p()
-        rc = lib.oracle_create(C.byref(h), self.N, _dptr(H), _dptr(lam), _dptr(nu),
-                               float(T_kelvin), int(K), int(D))
+        if bath_state is None:
+            rc = lib.oracle_create(C.byref(h), self.N, _dptr(H), _dptr(lam), _dptr(nu),
+                                   float(T_kelvin), int(K), int(D))
+        else:
+            bs = (C.c_int * self.B)(*[int(x) for x in bath_state])
+            rc = lib.oracle_create_sites(C.byref(h), self.N, _dptr(H), self.B, bs, _dptr(lam), _dptr(nu),
+                                         float(T_kelvin), int(K), int(D))
         if rc != 0:
             raise ValueError(f"oracle_create failed with status {rc}")
         self._h = h
@@ -105,7 +116,7 @@ class Oracle:
         return t, p, m
 
     def coefficients(self):
-        g = np.empty(self.W); cr = np.empty(self.W); ci = np.empty(self.W); d = np.empty(self.N)
+        g = np.empty(self.W); cr = np.empty(self.W); ci = np.empty(self.W); d = np.empty(self.B)
         self._ck(self._lib.oracle_get_coefficients(self._h, g.ctypes.data, cr.ctypes.data,
                                                    ci.ctypes.data, d.ctypes.data))
         return g, cr, ci, d

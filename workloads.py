@@ -146,3 +146,26 @@ def random_density(N, seed):
     A = rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
     rho = A @ A.conj().T
     return rho / np.trace(rho).real
+
+
+def with_ground_state(w, seed=1803034990):
+    """Linear-absorption stand-in (Eq. 53, 56): the workload's H with the electronic ground state
+    prepended as state 0 (energy 0, uncoupled: Eq. 48's block form), bath b on state b+1, and one seeded
+    transition dipole d_m per site (unit vectors, like the BChl Q_y dipoles the paper takes from the
+    crystal structure).  Returns (H_ext [N+1][N+1], bath_state [N], dipoles [N][3])."""
+    N = w.N
+    H = np.zeros((N + 1, N + 1))
+    H[1:, 1:] = w.H_cm
+    rng = np.random.default_rng(seed)
+    d = rng.standard_normal((N, 3))
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    return H, list(range(1, N + 1)), d
+
+
+def dipole_operator(dipoles, p):
+    """mu_p = mu_p^+ + mu_p^- with mu_p^+ = sum_m (e_p . d_m) |m><0| (Eq. 53), e_p the p-th Cartesian unit vector (Eq. 55)."""
+    N = dipoles.shape[0]
+    mu = np.zeros((N + 1, N + 1))
+    mu[1:, 0] = dipoles[:, p]
+    mu[0, 1:] = dipoles[:, p]
+    return mu
