@@ -59,6 +59,18 @@ typedef enum {
 heom_status heom_create(heom_ctx** out, int n_sites, const double* H_cm,
                         const double* lambda_cm, const double* nu_per_fs,
                         double T_kelvin, int K, int D, int device);
+/* The same for a system in which not every state carries a bath: the electronic
+ * ground state |0> of linear absorption (Eq. 48, 53, 56), which no bath couples to (P:128:
+ * each bath b couples through the projector on ONE state, S(b) = 1).
+ *   n_states    system states = rows of every sigma_u; H_cm is n_states*n_states
+ *   n_baths     1 <= n_baths <= n_states
+ *   bath_state  HOST [n_baths] 0-based state bath b couples to, all different (else HEOM_EINVAL)
+ *   lambda_cm, nu_per_fs  HOST [n_baths]
+ * Tuple length W = n_baths*(K+1); mode l = b*(K+1) + k belongs to bath b (Eq. 10-11).
+ * heom_create(n, ...) == heom_create_sites(n, ..., n, {0..n-1}, ...). */
+heom_status heom_create_sites(heom_ctx** out, int n_states, const double* H_cm, int n_baths,
+                              const int* bath_state, const double* lambda_cm, const double* nu_per_fs,
+                              double T_kelvin, int K, int D, int device);
 void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
 
 /* Options, to be set before heom_bind_workspace:
@@ -86,7 +98,8 @@ void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
 heom_status heom_set_option(heom_ctx* ctx, const char* name, int value);
 
 int64_t heom_num_nodes(const heom_ctx* ctx); /* Eq. 9: C(W+D, D) */
-int heom_num_modes(const heom_ctx* ctx);     /* W = n_sites*(K+1) */
+int heom_num_modes(const heom_ctx* ctx);     /* W = n_baths*(K+1) */
+int heom_num_baths(const heom_ctx* ctx);
 
 /* Copies the host tables in the PINNED order.  Any pointer may be NULL.
  *   tuples HOST uint8 [nodes][W]; plus, minus HOST int32 [nodes][W]:
@@ -94,7 +107,7 @@ int heom_num_modes(const heom_ctx* ctx);     /* W = n_sites*(K+1) */
 heom_status heom_get_tables(const heom_ctx* ctx, uint8_t* tuples, int32_t* plus,
                             int32_t* minus);
 /* gamma[W] (Eq. 19, fs^-1); c_re[W], c_im[W] = c(b,k)/hbar (Eq. 20 and the V^o
- * part of Eq. 17, fs^-2); delta[n_sites] = Eq. 14 bracket (fs^-1).  All HOST. */
+ * part of Eq. 17, fs^-2); delta[n_baths] = Eq. 14 bracket (fs^-1).  All HOST. */
 heom_status heom_get_coefficients(const heom_ctx* ctx, double* gamma, double* c_re,
                                   double* c_im, double* delta);
 
@@ -128,6 +141,11 @@ heom_status heom_sync(heom_ctx* ctx);
  * Computed by a device reduction kernel; output pointers may be NULL. */
 heom_status heom_populations(heom_ctx* ctx, double* pop, double* trace_re,
                              double* trace_im);
+
+/* Tr(A sigma_0) = sum_ij A[i][j] sigma_0[j][i]: the integrand of the dipole correlation function of
+ * Eq. 56 with A = mu_p.  A HOST [N][N] complex128 row-major; re, im HOST (may be NULL).
+ * Computed by a device reduction kernel; synchronises. */
+heom_status heom_expectation(heom_ctx* ctx, const double* A, double* re, double* im);
 
 /* Introspection for the harness. */
 int64_t heom_launch_count(const heom_ctx* ctx); /* kernels launched so far */

@@ -18,7 +18,7 @@ _STATUS = {0: "HEOM_OK", -1: "HEOM_EINVAL", -2: "HEOM_ENOMEM", -3: "HEOM_ECUDA",
 
 # every symbol include/heom.h declares (tests check the library exports all of them)
 SYMBOLS = [
-    "heom_create", "heom_destroy", "heom_set_option", "heom_num_nodes", "heom_num_modes",
+    "heom_create", "heom_create_sites", "heom_num_baths", "heom_expectation", "heom_destroy", "heom_set_option", "heom_num_nodes", "heom_num_modes",
     "heom_get_tables", "heom_get_coefficients", "heom_workspace_bytes", "heom_bind_workspace",
     "heom_set_state", "heom_set_full_state", "heom_get_full_state", "heom_rhs", "heom_rk4_steps",
     "heom_sync", "heom_populations", "heom_launch_count", "heom_kernel_time", "heom_kernel_name",
@@ -45,6 +45,10 @@ def load_library():
     lib = C.CDLL(LIB_PATH)
     P, dp = C.c_void_p, C.POINTER(C.c_double)
     lib.heom_create.argtypes = [C.POINTER(P), C.c_int, dp, dp, dp, C.c_double, C.c_int, C.c_int, C.c_int]
+    lib.heom_create_sites.argtypes = [C.POINTER(P), C.c_int, dp, C.c_int, C.POINTER(C.c_int), dp, dp, C.c_double,
+                                      C.c_int, C.c_int, C.c_int]
+    lib.heom_num_baths.argtypes = [P]
+    lib.heom_expectation.argtypes = [P, P, P, P]
     lib.heom_destroy.argtypes = [P]
     lib.heom_destroy.restype = None
     lib.heom_set_option.argtypes = [P, C.c_char_p, C.c_int]
@@ -81,18 +85,26 @@ def _dptr(a):
 class Heom:
     """One truncated hierarchy bound to one GPU stream.  Mirrors include/heom.h one to one."""
 
-    def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, device=0, **options):
+    def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, device=0, bath_state=None, **options):
+        """bath_state=None: heom_create (one bath per state); else heom_create_sites with the listed states
+        (lambda_cm, nu_per_fs then have one entry per bath)."""
         self._lib = load_library()
         self._h = None
         H = np.ascontiguousarray(H_cm, dtype=np.float64)
         if H.ndim != 2 or H.shape[0] != H.shape[1]:
             raise ValueError("H_cm must be square")
         self.N = H.shape[0]
-        lam = np.ascontiguousarray(np.broadcast_to(lambda_cm, (self.N,)), dtype=np.float64)
-        nu = np.ascontiguousarray(np.broadcast_to(nu_per_fs, (self.N,)), dtype=np.float64)
+        self.B = self.N if bath_state is None else len(bath_state)
+        lam = np.ascontiguousarray(np.broadcast_to(lambda_cm, (self.B,)), dtype=np.float64)
+        nu = np.ascontiguousarray(np.broadcast_to(nu_per_fs, (self.B,)), dtype=np.float64)
         h = C.c_void_p()
-        rc = self._lib.heom_create(C.byref(h), self.N, _dptr(H), _dptr(lam), _dptr(nu),
-                                   float(T_kelvin), int(K), int(D), int(device))
+        if bath_state is None:
+            rc = self._lib.heom_create(C.byref(h), self.N, _dptr(H), _dptr(lam), _dptr(nu),
+                                       float(T_kelvin), int(K), int(D), int(device))
+        else:
+            bs = (C.c_int * self.B)(*[int(x) for x in bath_state])
+            rc = self._lib.heom_create_sites(C.byref(h), self.N, _dptr(H), self.B, bs, _dptr(lam), _dptr(nu),
+                                             float(T_kelvin), int(K), int(D), int(device))
         if rc != 0:
             raise HeomError(rc, "heom_create rejected its arguments")
         self._h = h
@@ -133,7 +145,7 @@ class Heom:
         return t, p, m
 
     def coefficients(self):
-        g = np.empty(self.W); cr = np.empty(self.W); ci = np.empty(self.W); d = np.empty(self.N)
+        g = np.empty(self.W); cr = np.empty(self.W); ci = np.empty(self.W); d = np.empty(self.B)
         self._ck(self._lib.heom_get_coefficients(self._h, g.ctypes.data, cr.ctypes.data,
                                                  ci.ctypes.data, d.ctypes.data))
         return g, cr, ci, d
@@ -195,6 +207,15 @@ class Heom:
         self._ck(self._lib.heom_populations(self._h, pop.ctypes.data, C.addressof(tr[0]),
                                             C.addressof(tr[1])))
         return pop, complex(tr[0].value, tr[1].value)
+
+    def expectation(self, A):
+        """Tr(A sigma_0) (heom_expectation)."""
+        a = np.ascontiguousarray(A, dtype=np.complex128)
+        if a.shape != (self.N, self.N):
+            raise ValueError("A must be N x N")
+        v = C.c_double(), C.c_double()
+        self._ck(self._lib.heom_expectation(self._h, a.ctypes.data, C.addressof(v[0]), C.addressof(v[1])))
+        return complex(v[0].value, v[1].value)
 
     # -- introspection --------------------------------------------------------------------
     def launch_count(self):

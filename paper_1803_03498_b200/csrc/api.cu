@@ -16,8 +16,15 @@
 using namespace heom;
 
 struct heom_ctx {
-  Hierarchy h;
-  Coefficients c;
+  Hierarchy h;                      // h.N = system states; h.W = B*M modes (tuple length, host tables)
+  Coefficients c;                   // per bath: [B*M] / [B]; what heom_get_coefficients returns
+  // Bath -> state map (heom_create_sites; identity for heom_create).  The kernels index modes per STATE
+  // (l_dev = state*M + k, Wd = N*M): a state without a bath gets M mode columns whose links are all invalid
+  // and whose coupling constants are zero, so no kernel knows about the map.
+  int B = 0;                        // baths
+  std::vector<int> site;            // [B] state of bath b
+  std::vector<int> bath_of;         // [N] bath of state s, -1 = none
+  Coefficients cd;                  // the same coefficients in the kernels' per-state mode indexing [Wd] / [N]
   std::vector<double> lambda, nu;   // bath parameters (kept for the "pade" option)
   double T_kelvin = 0;
   int pade = 0;
@@ -58,6 +65,7 @@ struct heom_ctx {
   int64_t* d_lptr = nullptr;
   void* d_lent = nullptr;
   double *d_Hs = nullptr, *d_delta = nullptr;
+  double2* d_A = nullptr;    // operator of heom_expectation
   size_t n_links = 0;
   unsigned long long* d_tickets = nullptr;   // work counter of the persistent kernel
   unsigned long long ticket_base = 0;
@@ -93,10 +101,43 @@ heom_status cuda_fail(heom_ctx* c, cudaError_t e, const char* where) {
     if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);       \
   } while (0)
 
+int dev_modes(const heom_ctx* c) { return c->h.N * c->h.M; }   // Wd: mode columns of the device tables
+
+// c->cd, c->Tterm from c->c and the bath -> state map
+void expand_coefficients(heom_ctx* c) {
+  const int N = c->h.N, M = c->h.M, D1 = c->h.D + 1, Wd = N * M;
+  Coefficients& d = c->cd;
+  d.beta_hbar = c->c.beta_hbar;
+  d.gamma.assign((size_t)Wd, 0.0); d.c_re.assign((size_t)Wd, 0.0); d.c_im.assign((size_t)Wd, 0.0);
+  d.delta.assign((size_t)N, 0.0);
+  d.a_plus.assign((size_t)Wd * D1, 0.0); d.a_minus_x.assign((size_t)Wd * D1, 0.0); d.a_minus_o.assign((size_t)Wd * D1, 0.0);
+  for (int s = 0; s < N; ++s) {
+    const int b = c->bath_of[(size_t)s];
+    if (b < 0) continue;
+    d.delta[(size_t)s] = c->c.delta[(size_t)b];
+    for (int k = 0; k < M; ++k) {
+      const size_t ld = (size_t)s * M + k, lh = (size_t)b * M + k;
+      d.gamma[ld] = c->c.gamma[lh]; d.c_re[ld] = c->c.c_re[lh]; d.c_im[ld] = c->c.c_im[lh];
+      for (int n = 0; n < D1; ++n) {
+        d.a_plus[ld * D1 + n] = c->c.a_plus[lh * D1 + n];
+        d.a_minus_x[ld * D1 + n] = c->c.a_minus_x[lh * D1 + n];
+        d.a_minus_o[ld * D1 + n] = c->c.a_minus_o[lh * D1 + n];
+      }
+    }
+  }
+  c->Tterm.assign((size_t)N * N, 0.0);
+  for (int i = 0; i < N; ++i)
+    for (int j = 0; j < N; ++j)
+      if (i != j) c->Tterm[(size_t)i * N + j] = d.delta[(size_t)i] + d.delta[(size_t)j];  // Eq. 14 + 24
+}
+
 bool ensure_hierarchy(heom_ctx* c) {
   if (c->hierarchy_built && c->built_order == c->order) return true;
   std::string err;
-  if (!build_hierarchy(c->h.N, c->h.K, c->h.D, c->order, c->h, err)) { c->err = err; return false; }
+  const int n_states = c->h.N;
+  const bool ok = build_hierarchy(c->B, c->h.K, c->h.D, c->order, c->h, err);   // tuples over the B*M modes
+  c->h.N = n_states;
+  if (!ok) { c->err = err; return false; }
   c->hierarchy_built = true;
   c->built_order = c->order;
   return true;
@@ -108,12 +149,12 @@ int links_row(int W) { return (2 * W + (W + 3) / 4 + 3) / 4 * 4; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, off_linksP, off_Hs, off_delta, off_lptr, off_lent, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, off_linksP, off_Hs, off_delta, off_A, off_lptr, off_lent, total;
 };
 
 Layout layout_of(const heom_ctx* c) {
   Layout L{};
-  const size_t nodes = (size_t)c->h.nodes, W = (size_t)c->h.W, N = (size_t)c->h.N, D1 = (size_t)c->h.D + 1;
+  const size_t nodes = (size_t)c->h.nodes, W = (size_t)dev_modes(c), N = (size_t)c->h.N, D1 = (size_t)c->h.D + 1;
   L.state = align_up(nodes * (size_t)node_stride((int)N) * sizeof(double2));
   size_t o = 0;
   L.off_y = o; o += L.state;
@@ -137,6 +178,7 @@ Layout layout_of(const heom_ctx* c) {
   L.off_linksP = o; o += align_up(nodes * (size_t)hpipe_links_row((int)N, c->h.M) * 4);
   L.off_Hs = o; o += align_up(N * N * 8);
   L.off_delta = o; o += align_up(N * 8);
+  L.off_A = o; o += align_up(N * N * 16);
   if (large_supported((int)N, (int)W)) {
     // every valid link appears once as "+" and once as "-": count the "-" links of the host table
     size_t links = 0;
@@ -150,7 +192,7 @@ Layout layout_of(const heom_ctx* c) {
 
 RhsParams base_params(const heom_ctx* c) {
   RhsParams p{};
-  p.N = c->h.N; p.M = c->h.M; p.W = c->h.W; p.D = c->h.D; p.nodes = (int)c->h.nodes;
+  p.N = c->h.N; p.M = c->h.M; p.W = dev_modes(c); p.D = c->h.D; p.nodes = (int)c->h.nodes;
   p.stride = c->stride;
   p.inv_hbar = 1.0 / kHbar;
   p.H = c->d_H; p.Tterm = c->d_T; p.damp = c->d_damp;
@@ -174,16 +216,16 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
     CU(cudaEventRecord(e0, ctx->stream));
   }
   if (ctx->use_large)
-    CU(launch_rhs_large(p, ctx->d_lptr, ctx->d_lent, ctx->d_Hs, ctx->d_delta, ctx->c.a_plus.data(),
-                        ctx->c.a_minus_x.data(), ctx->c.a_minus_o.data(), ctx->sms, ctx->d_tickets,
+    CU(launch_rhs_large(p, ctx->d_lptr, ctx->d_lent, ctx->d_Hs, ctx->d_delta, ctx->cd.a_plus.data(),
+                        ctx->cd.a_minus_x.data(), ctx->cd.a_minus_o.data(), ctx->sms, ctx->d_tickets,
                         &ctx->ticket_base, ctx->stream));
   else if (ctx->use_hpipe)
-    CU(launch_rhs_hpipe(p, ctx->d_linksP, ctx->lrowP, ctx->c.a_plus.data(), ctx->c.a_minus_x.data(),
-                        ctx->c.a_minus_o.data(), ctx->H.data(), ctx->c.delta.data(),
+    CU(launch_rhs_hpipe(p, ctx->d_linksP, ctx->lrowP, ctx->cd.a_plus.data(), ctx->cd.a_minus_x.data(),
+                        ctx->cd.a_minus_o.data(), ctx->H.data(), ctx->cd.delta.data(),
                         ctx->herm_opt && ctx->state_hermitian, ctx->warps_per_cta, ctx->sms, ctx->d_tickets,
                         &ctx->ticket_base, ctx->stream));
   else if (ctx->use_herm && ctx->herm_opt && ctx->state_hermitian)
-    CU(launch_rhs_herm(p, ctx->d_linksH, ctx->lrowH, ctx->d_coefH, ctx->H.data(), ctx->c.delta.data(), ctx->stream));
+    CU(launch_rhs_herm(p, ctx->d_linksH, ctx->lrowH, ctx->d_coefH, ctx->H.data(), ctx->cd.delta.data(), ctx->stream));
   else if (ctx->use_rows) CU(launch_rhs_rows(p, ctx->d_links, ctx->lrow, ctx->H.data(), ctx->stream));
   else CU(launch_rhs_generic(p, ctx->stream));
   ctx->launches += 1;
@@ -195,34 +237,42 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
 
 extern "C" {
 
-heom_status heom_create(heom_ctx** out, int n_sites, const double* H_cm, const double* lambda_cm,
-                        const double* nu_per_fs, double T_kelvin, int K, int D, int device) {
+heom_status heom_create_sites(heom_ctx** out, int n_states, const double* H_cm, int n_baths, const int* bath_state,
+                              const double* lambda_cm, const double* nu_per_fs, double T_kelvin, int K, int D,
+                              int device) {
   if (!out) return HEOM_EINVAL;
   *out = nullptr;
-  if (!H_cm || !lambda_cm || !nu_per_fs || n_sites < 1 || K < 0 || D < 0 || D > 255 || device < 0)
+  if (!H_cm || !lambda_cm || !nu_per_fs || !bath_state || n_states < 1 || n_baths < 1 || n_baths > n_states ||
+      K < 0 || D < 0 || D > 255 || device < 0)
     return HEOM_EINVAL;
-  for (int i = 0; i < n_sites; ++i)
-    for (int j = 0; j < n_sites; ++j) {
-      const double a = H_cm[(size_t)i * n_sites + j], b = H_cm[(size_t)j * n_sites + i];
+  for (int i = 0; i < n_states; ++i)
+    for (int j = 0; j < n_states; ++j) {
+      const double a = H_cm[(size_t)i * n_states + j], b = H_cm[(size_t)j * n_states + i];
       if (!std::isfinite(a) || a != b) return HEOM_EINVAL;
     }
+  std::vector<int> bath_of((size_t)n_states, -1);
+  for (int b = 0; b < n_baths; ++b) {
+    const int s = bath_state[b];
+    if (s < 0 || s >= n_states || bath_of[(size_t)s] >= 0) return HEOM_EINVAL;   // one bath per state at most
+    bath_of[(size_t)s] = b;
+  }
   heom_ctx* c = new (std::nothrow) heom_ctx();
   if (!c) return HEOM_ENOMEM;
   c->device = device;
-  c->h.N = n_sites; c->h.K = K; c->h.M = K + 1; c->h.W = n_sites * (K + 1); c->h.D = D;
+  c->B = n_baths;
+  c->site.assign(bath_state, bath_state + n_baths);
+  c->bath_of = bath_of;
+  c->h.N = n_states; c->h.K = K; c->h.M = K + 1; c->h.W = n_baths * (K + 1); c->h.D = D;
   std::string err;
-  if (!build_coefficients(n_sites, K, D, lambda_cm, nu_per_fs, T_kelvin, 0, c->c, err)) {
+  if (!build_coefficients(n_baths, K, D, lambda_cm, nu_per_fs, T_kelvin, 0, c->c, err)) {
     delete c;
     return HEOM_EINVAL;
   }
-  c->lambda.assign(lambda_cm, lambda_cm + n_sites);
-  c->nu.assign(nu_per_fs, nu_per_fs + n_sites);
+  c->lambda.assign(lambda_cm, lambda_cm + n_baths);
+  c->nu.assign(nu_per_fs, nu_per_fs + n_baths);
   c->T_kelvin = T_kelvin;
-  c->H.assign(H_cm, H_cm + (size_t)n_sites * n_sites);
-  c->Tterm.assign((size_t)n_sites * n_sites, 0.0);
-  for (int i = 0; i < n_sites; ++i)
-    for (int j = 0; j < n_sites; ++j)
-      if (i != j) c->Tterm[(size_t)i * n_sites + j] = c->c.delta[i] + c->c.delta[j];  // Eq. 14 + 24
+  c->H.assign(H_cm, H_cm + (size_t)n_states * n_states);
+  expand_coefficients(c);
   if (!ensure_hierarchy(c)) {
     const bool oom = c->err.find("memory") != std::string::npos;
     delete c;
@@ -230,6 +280,16 @@ heom_status heom_create(heom_ctx** out, int n_sites, const double* H_cm, const d
   }
   *out = c;
   return HEOM_OK;
+}
+
+heom_status heom_create(heom_ctx** out, int n_sites, const double* H_cm, const double* lambda_cm,
+                        const double* nu_per_fs, double T_kelvin, int K, int D, int device) {
+  if (!out) return HEOM_EINVAL;
+  *out = nullptr;
+  if (n_sites < 1) return HEOM_EINVAL;
+  std::vector<int> ident((size_t)n_sites);
+  for (int b = 0; b < n_sites; ++b) ident[(size_t)b] = b;
+  return heom_create_sites(out, n_sites, H_cm, n_sites, ident.data(), lambda_cm, nu_per_fs, T_kelvin, K, D, device);
 }
 
 void heom_destroy(heom_ctx* c) {
@@ -264,14 +324,12 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
   if (s == "pade") {
     Coefficients nc;
     std::string err;
-    if (!build_coefficients(ctx->h.N, ctx->h.K, ctx->h.D, ctx->lambda.data(), ctx->nu.data(), ctx->T_kelvin,
+    if (!build_coefficients(ctx->B, ctx->h.K, ctx->h.D, ctx->lambda.data(), ctx->nu.data(), ctx->T_kelvin,
                             value ? 1 : 0, nc, err))
       return fail(ctx, HEOM_EINVAL, err);
     ctx->c = nc;
     ctx->pade = value ? 1 : 0;
-    for (int i = 0; i < ctx->h.N; ++i)
-      for (int j = 0; j < ctx->h.N; ++j)
-        ctx->Tterm[(size_t)i * ctx->h.N + j] = (i == j) ? 0.0 : ctx->c.delta[i] + ctx->c.delta[j];
+    expand_coefficients(ctx);
     return HEOM_OK;
   }
   if (s == "order") {
@@ -289,6 +347,7 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
 
 int64_t heom_num_nodes(const heom_ctx* c) { return c ? c->h.nodes : -1; }
 int heom_num_modes(const heom_ctx* c) { return c ? c->h.W : -1; }
+int heom_num_baths(const heom_ctx* c) { return c ? c->B : -1; }
 
 heom_status heom_get_tables(const heom_ctx* c, uint8_t* tuples, int32_t* plus, int32_t* minus) {
   if (!c) return HEOM_EINVAL;
@@ -305,7 +364,7 @@ heom_status heom_get_coefficients(const heom_ctx* c, double* gamma, double* c_re
   if (gamma) std::memcpy(gamma, c->c.gamma.data(), W * 8);
   if (c_re) std::memcpy(c_re, c->c.c_re.data(), W * 8);
   if (c_im) std::memcpy(c_im, c->c.c_im.data(), W * 8);
-  if (delta) std::memcpy(delta, c->c.delta.data(), (size_t)c->h.N * 8);
+  if (delta) std::memcpy(delta, c->c.delta.data(), (size_t)c->B * 8);
   return HEOM_OK;
 }
 
@@ -352,21 +411,23 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->ticket_base = 0;
   CU(cudaMemset(ctx->d_tickets, 0, 8));
   ctx->d_links = (int32_t*)(base + L.off_links);
-  ctx->lrow = links_row(ctx->h.W);
-  ctx->use_rows = ctx->kernel >= 1 && rows_supported(ctx->h.N, ctx->h.W, ctx->h.D, ctx->lrow);
+  const int Wd = dev_modes(ctx);
+  ctx->lrow = links_row(Wd);
+  ctx->use_rows = ctx->kernel >= 1 && rows_supported(ctx->h.N, Wd, ctx->h.D, ctx->lrow);
   ctx->d_linksH = (int32_t*)(base + L.off_linksH);
   ctx->d_coefH = (double*)(base + L.off_coefH);
   ctx->lrowH = herm_links_row(ctx->h.N, ctx->h.M);
-  ctx->use_herm = ctx->kernel >= 1 && herm_supported(ctx->h.N, ctx->h.W, ctx->h.D);
-  ctx->use_large = ctx->kernel == 1 && large_supported(ctx->h.N, ctx->h.W);
-  ctx->use_tiny = ctx->kernel == 1 && tiny_supported(ctx->h.N, ctx->h.W, ctx->h.D, (long long)ctx->h.nodes);
+  ctx->use_herm = ctx->kernel >= 1 && herm_supported(ctx->h.N, Wd, ctx->h.D);
+  ctx->use_large = ctx->kernel == 1 && large_supported(ctx->h.N, Wd);
+  ctx->use_tiny = ctx->kernel == 1 && tiny_supported(ctx->h.N, Wd, ctx->h.D, (long long)ctx->h.nodes);
   ctx->d_Hs = (double*)(base + L.off_Hs);
   ctx->d_delta = (double*)(base + L.off_delta);
+  ctx->d_A = (double2*)(base + L.off_A);
   ctx->d_lptr = (int64_t*)(base + L.off_lptr);
   ctx->d_lent = (void*)(base + L.off_lent);
   ctx->d_linksP = (int32_t*)(base + L.off_linksP);
   ctx->lrowP = hpipe_links_row(ctx->h.N, ctx->h.M);
-  ctx->use_hpipe = ctx->kernel == 1 && hpipe_supported(ctx->h.N, ctx->h.W, ctx->h.D, (long long)ctx->h.nodes);
+  ctx->use_hpipe = ctx->kernel == 1 && hpipe_supported(ctx->h.N, Wd, ctx->h.D, (long long)ctx->h.nodes);
   {
     cudaDeviceProp prop;
     CU(cudaGetDeviceProperties(&prop, ctx->device));
@@ -376,7 +437,7 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
 
   // Device tables in STORAGE-slot order: row slot_of[u] holds the slots of u's neighbours.
   const Hierarchy& h = ctx->h;
-  const size_t nodes = (size_t)h.nodes, W = (size_t)h.W;
+  const size_t nodes = (size_t)h.nodes, W = (size_t)Wd, Wh = (size_t)h.W, Mm = (size_t)h.M;
   try {
     std::vector<int32_t> tp(nodes * W), tm(nodes * W);
     std::vector<uint8_t> tt(nodes * W);
@@ -385,13 +446,16 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
     for (int64_t u = 0; u < (int64_t)nodes; ++u) {
       const size_t s = (size_t)h.slot_of[(size_t)u];
       double d = 0.0;
-      for (size_t l = 0; l < W; ++l) {
-        const int32_t a = h.plus[(size_t)u * W + l], b = h.minus[(size_t)u * W + l];
+      for (size_t l = 0; l < W; ++l) {      // device mode column l = state*M + k
+        const int bath = ctx->bath_of[l / Mm];
+        if (bath < 0) { tp[s * W + l] = -1; tm[s * W + l] = -1; tt[s * W + l] = 0; continue; }
+        const size_t lh = (size_t)bath * Mm + l % Mm;   // host mode index (Eq. 10)
+        const int32_t a = h.plus[(size_t)u * Wh + lh], b = h.minus[(size_t)u * Wh + lh];
         tp[s * W + l] = a < 0 ? -1 : h.slot_of[(size_t)a];
         tm[s * W + l] = b < 0 ? -1 : h.slot_of[(size_t)b];
-        const uint8_t n = h.tuples[(size_t)u * W + l];
+        const uint8_t n = h.tuples[(size_t)u * Wh + lh];
         tt[s * W + l] = n;
-        d += (double)n * ctx->c.gamma[l];  // Eq. 13
+        d += (double)n * ctx->cd.gamma[l];  // Eq. 13
       }
       damp[s] = d;
     }
@@ -435,7 +499,7 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
       std::vector<double> Hs(ctx->H);
       for (double& v : Hs) v *= 1.0 / kHbar;
       CU(cudaMemcpy(ctx->d_Hs, Hs.data(), Hs.size() * 8, cudaMemcpyHostToDevice));
-      CU(cudaMemcpy(ctx->d_delta, ctx->c.delta.data(), (size_t)h.N * 8, cudaMemcpyHostToDevice));
+      CU(cudaMemcpy(ctx->d_delta, ctx->cd.delta.data(), (size_t)h.N * 8, cudaMemcpyHostToDevice));
     }
     if (ctx->use_hpipe) {
       const size_t lrow = (size_t)ctx->lrowP;
@@ -449,7 +513,7 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
       const size_t D1 = (size_t)h.D + 1;
       std::vector<double> cf(W * D1 * 4, 0.0);
       for (size_t q = 0; q < W * D1; ++q) {
-        cf[4 * q] = ctx->c.a_plus[q]; cf[4 * q + 1] = ctx->c.a_minus_x[q]; cf[4 * q + 2] = ctx->c.a_minus_o[q];
+        cf[4 * q] = ctx->cd.a_plus[q]; cf[4 * q + 1] = ctx->cd.a_minus_x[q]; cf[4 * q + 2] = ctx->cd.a_minus_o[q];
       }
       CU(cudaMemcpy(ctx->d_coefH, cf.data(), W * D1 * 32, cudaMemcpyHostToDevice));
     }
@@ -468,9 +532,9 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   CU(cudaMemcpy(ctx->d_slot, h.slot_of.data(), nodes * 4, cudaMemcpyHostToDevice));
   CU(cudaMemcpy(ctx->d_H, ctx->H.data(), NN * 8, cudaMemcpyHostToDevice));
   CU(cudaMemcpy(ctx->d_T, ctx->Tterm.data(), NN * 8, cudaMemcpyHostToDevice));
-  CU(cudaMemcpy(ctx->d_ap, ctx->c.a_plus.data(), WD * 8, cudaMemcpyHostToDevice));
-  CU(cudaMemcpy(ctx->d_amx, ctx->c.a_minus_x.data(), WD * 8, cudaMemcpyHostToDevice));
-  CU(cudaMemcpy(ctx->d_amo, ctx->c.a_minus_o.data(), WD * 8, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(ctx->d_ap, ctx->cd.a_plus.data(), WD * 8, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(ctx->d_amx, ctx->cd.a_minus_x.data(), WD * 8, cudaMemcpyHostToDevice));
+  CU(cudaMemcpy(ctx->d_amo, ctx->cd.a_minus_o.data(), WD * 8, cudaMemcpyHostToDevice));
   ctx->bound = true;
   ctx->have_state = false;
   return HEOM_OK;
@@ -652,6 +716,25 @@ heom_status heom_populations(heom_ctx* ctx, double* pop, double* trace_re, doubl
   if (pop) std::memcpy(pop, ctx->h_pinned, (size_t)N * 8);
   if (trace_re) *trace_re = ctx->h_pinned[N];
   if (trace_im) *trace_im = ctx->h_pinned[N + 1];
+  return HEOM_OK;
+}
+
+heom_status heom_expectation(heom_ctx* ctx, const double* A, double* re, double* im) {
+  if (!ctx || !A) return HEOM_EINVAL;
+  if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
+  const int N = ctx->h.N;
+  const size_t NN = (size_t)N * N;
+  for (size_t e = 0; e < 2 * NN; ++e)
+    if (!std::isfinite(A[e])) return fail(ctx, HEOM_EINVAL, "operator has a non-finite entry");
+  CU(cudaStreamSynchronize(ctx->stream));  // the pinned staging buffer may still be in flight
+  std::memcpy(ctx->h_pinned, A, NN * 16);
+  CU(cudaMemcpyAsync(ctx->d_A, ctx->h_pinned, NN * 16, cudaMemcpyHostToDevice, ctx->stream));
+  CU(launch_expectation(ctx->y + (size_t)ctx->h.slot_of[0] * ctx->stride, ctx->d_A, N, ctx->d_scratch, ctx->stream));
+  ctx->launches += 1;
+  CU(cudaMemcpyAsync(ctx->h_pinned, ctx->d_scratch, 16, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  if (re) *re = ctx->h_pinned[0];
+  if (im) *im = ctx->h_pinned[1];
   return HEOM_OK;
 }
 

@@ -94,4 +94,7 @@ cudaError_t launch_permute(const double2* src, double2* dst, const int32_t* slot
 // out[0..N-1] = Re sigma_0[i][i]; out[N], out[N+1] = trace (re, im)
 cudaError_t launch_populations(const double2* node0, int N, double* out, cudaStream_t s);
 
+// out[0], out[1] = Tr(A sigma_0) (re, im); A: DEVICE [N][N] complex128
+cudaError_t launch_expectation(const double2* node0, const double2* A, int N, double* out, cudaStream_t s);
+
 }  // namespace heom

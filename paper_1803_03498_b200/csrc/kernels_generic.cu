@@ -153,6 +153,23 @@ __global__ void populations_kernel(const double2* __restrict__ node0, int N, dou
   if (threadIdx.x == 0) { out[N] = tr; out[N + 1] = ti; }
 }
 
+// Tr(A sigma_0) = sum_ij A[i][j] sigma_0[j][i] (the dipole correlation function of Eq. 56); one warp, fixed order
+__global__ void expectation_kernel(const double2* __restrict__ node0, const double2* __restrict__ A, int N,
+                                   double* __restrict__ out) {
+  double tr = 0.0, ti = 0.0;
+  for (int e = threadIdx.x; e < N * N; e += 32) {
+    const int i = e / N, j = e - i * N;
+    const double2 a = A[e], s = node0[(size_t)j * N + i];
+    tr += a.x * s.x - a.y * s.y;
+    ti += a.x * s.y + a.y * s.x;
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    tr += __shfl_xor_sync(0xffffffffu, tr, o);
+    ti += __shfl_xor_sync(0xffffffffu, ti, o);
+  }
+  if (threadIdx.x == 0) { out[0] = tr; out[1] = ti; }
+}
+
 }  // namespace
 
 size_t rhs_generic_smem(int N) {
@@ -192,6 +209,11 @@ cudaError_t launch_permute(const double2* src, double2* dst, const int32_t* slot
 
 cudaError_t launch_populations(const double2* node0, int N, double* out, cudaStream_t s) {
   populations_kernel<<<1, 32, 0, s>>>(node0, N, out);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_expectation(const double2* node0, const double2* A, int N, double* out, cudaStream_t s) {
+  expectation_kernel<<<1, 32, 0, s>>>(node0, A, N, out);
   return cudaGetLastError();
 }
 

@@ -111,3 +111,29 @@ def test_no_cpu_fallback():
     with pytest.raises(HeomError) as e:
         g.bind_raw(256, g.workspace_bytes())
     assert e.value.status == -3
+
+
+# ------------------------------------------------ bath -> state map (heom_create_sites)
+@pytest.mark.parametrize("N,bath_state,K,D", [(2, [1], 2, 5), (8, [1, 2, 3, 4, 5, 6, 7], 1, 3), (4, [3, 0], 1, 4),
+                                               (33, list(range(1, 33)), 0, 2), (3, [2, 1, 0], 0, 3)])
+def test_site_map_tables_and_coefficients_vs_oracle(N, bath_state, K, D):
+    H = np.zeros((N, N))
+    B = len(bath_state)
+    lam = np.linspace(20.0, 40.0, B); nu = np.linspace(0.02, 0.03, B)
+    o = Oracle(H, lam, nu, 150.0, K, D, bath_state=bath_state)
+    g = Heom(H, lam, nu, 150.0, K, D, bath_state=bath_state)
+    assert g.nodes == o.nodes and g.W == o.W == B * (K + 1) and g.B == B
+    for a, b in zip(g.tables(), o.tables()):
+        assert a.dtype == b.dtype and np.array_equal(a, b)
+    for q, (a, b) in enumerate(zip(g.coefficients(), o.coefficients())):
+        assert a.shape == b.shape
+        assert np.allclose(a, b, rtol=1e-11 if q == 3 else 1e-15, atol=1e-300)
+    # workspace: 4 state buffers of n_states x n_states matrices
+    assert g.workspace_bytes() >= 4 * 16 * N * N * g.nodes
+
+
+def test_site_map_validation():
+    H = np.zeros((3, 3))
+    for bad in ([1, 1], [3], [-1], [0, 1, 2, 0], []):
+        with pytest.raises(HeomError):
+            Heom(H, 35.0, 0.02, 300.0, 0, 2, bath_state=bad)
