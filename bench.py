@@ -98,7 +98,7 @@ def oracle_throughput(w, target_seconds=15.0):
     right-hand-side evaluations (oracle_rhs_nodes) of a seeded sample of nodes of the full hierarchy,
     i.e. node-updates without the RK4 combination."""
     from oracle.oracle import Oracle
-    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D)
+    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, bath_state=w.bath_state)
     o.set_state(w.sigma0())
     if w.state_bytes <= 2e9:
         t0 = time.perf_counter(); o.rk4_steps(w.dt_fs, 1); t1 = time.perf_counter() - t0
@@ -124,7 +124,7 @@ def run_reference(args, w):
         return
     # each "step" of the reference arm is a bounded sample: one oracle RK4 step of the full hierarchy
     from oracle.oracle import Oracle
-    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D)
+    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, bath_state=w.bath_state)
     o.set_state(w.sigma0())
     t0 = time.perf_counter(); o.rk4_steps(w.dt_fs, 1); t1 = time.perf_counter() - t0
     budget = 150.0
@@ -146,7 +146,9 @@ def run_reference(args, w):
 
 
 def config_dict(w, n_gpus):
-    return {"workload": f"{w.name}: BASELINE.json configs[{list(workloads.CONFIGS).index(w.name[:4])}] "
+    origin = (f"BASELINE.json configs[{list(workloads.CONFIGS).index(w.name[:4])}]" if w.name[:4] in workloads.CONFIGS
+              else "linear-absorption variant of configs[1] (ground state + 7 sites, sigma_0(0) = mu_z|0><0|; not a BASELINE config)")
+    return {"workload": f"{w.name}: {origin} "
                         f"N={w.N} K={w.K} D={w.D} T={w.T_kelvin:g}K nodes={w.nodes} dt={w.dt_fs}fs",
             "state_mb": round(w.state_bytes / 1e6, 1),
             "l2_policy": "state buffers (4 x %.0f MB) exceed the 126 MB L2; no flush needed" % (w.state_bytes / 1e6)
@@ -160,7 +162,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="cfg2", choices=list(workloads.CONFIGS))
+    ap.add_argument("--config", default="cfg2", choices=list(workloads.CONFIGS) + list(workloads.EXTRA))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="name=value library option")
@@ -186,10 +188,10 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     opts = dict(kv.split("=") for kv in args.option)
     stream = torch.cuda.Stream(device=local_rank)
-    g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, device=local_rank,
+    g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, device=local_rank, bath_state=w.bath_state,
              **{k: int(v) for k, v in opts.items()})
     g.bind(stream=stream)
-    sigma0 = replicas.replica_sigma0(w, rank)
+    sigma0 = replicas.replica_sigma0(w, rank) if w.sigma0_matrix is None else w.sigma0()
     flush = None
     if w.state_bytes <= 130e6:
         flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=f"cuda:{local_rank}")

@@ -22,6 +22,9 @@
  *                   trace and Hermiticity invariants; relaxation towards
  *                   Boltzmann populations; independence of sigma_0 from the
  *                   rescaling of Eq. 35-36; dense-Liouvillian expm comparison.
+ *   bath -> state
+ *   map           : two-level absorber cumulant closed form; lambda = 0 per-site
+ *                   equivalence; Eq. 48 block structure (tests/test_oracle_sites.py).
  *   Parity unpinned: nothing in this file is without a pin, but configs 2-5 of
  *   BASELINE.json have no printed values anywhere (the paper prints none);
  *   they rest on the pins above evaluated at those shapes.

@@ -33,14 +33,20 @@ class Workload:
     D: int                    # truncation depth
     dt_fs: float
     steps: int
+    bath_state: tuple = None      # None: one bath per state; else the states the baths couple to (heom_create_sites)
+    sigma0_matrix: np.ndarray = None   # None: |1><1|
 
     @property
     def N(self):
         return self.H_cm.shape[0]
 
     @property
+    def B(self):
+        return self.N if self.bath_state is None else len(self.bath_state)
+
+    @property
     def W(self):
-        return self.N * (self.K + 1)
+        return self.B * (self.K + 1)
 
     @property
     def nodes(self):
@@ -59,6 +65,8 @@ class Workload:
 
     def sigma0(self):
         """sigma_0(0) = |1><1| (BASELINE.json: all configs)."""
+        if self.sigma0_matrix is not None:
+            return self.sigma0_matrix.astype(np.complex128)
         s = np.zeros((self.N, self.N), dtype=np.complex128)
         s[0, 0] = 1.0
         return s
@@ -116,13 +124,26 @@ def large():
                     0.5, 50)
 
 
+def absorption_fmo():
+    """Not a BASELINE config: the paper's linear-absorption use (Fig. 5: FMO at 77 K) on the FMO-like
+    stand-in.  cfg2's H with the ground state as state 0, its 7 baths on states 1..7, sigma_0(0) = mu_z |0><0|
+    (a non-Hermitian state: the general-state kernels), N = 8, W = 14, D = 8, the same 319 770 nodes."""
+    w = fmo_like()
+    H, bath_state, dip = with_ground_state(w)
+    mu = dipole_operator(dip, 2)
+    s0 = np.zeros((8, 8), dtype=np.complex128)
+    s0[:, 0] = mu[:, 0]
+    return Workload("absorb_fmo8", H, 35.0, 50.0, 77.0, 1, 8, 1.0, 1000, tuple(bath_state), s0)
+
+
 CONFIGS = {
     "cfg1": dimer, "cfg2": fmo_like, "cfg3": deep, "cfg4": lhcii_like, "cfg5": large,
 }
+EXTRA = {"absorb": absorption_fmo}
 
 
 def get(name):
-    return CONFIGS[name]()
+    return (CONFIGS.get(name) or EXTRA[name])()
 
 
 def random_state(nodes, N, seed, hermitian=False):
