@@ -94,7 +94,13 @@ void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
  *   "hermitian" 1 (default) = when heom_set_state / heom_set_full_state find the state
  *             EXACTLY Hermitian (every node equals its conjugate transpose bit for bit), use
  *             the row-gather kernel that keeps it exactly Hermitian; 0 = always the general
- *             kernel.  "timing" and "hermitian" may be changed at any time. */
+ *             kernel.  "timing" and "hermitian" may be changed at any time.
+ *   "ket"     1 (default) = when heom_set_state finds sigma_0 with exactly ONE non-zero column c, state c
+ *             without a bath (heom_create_sites) and uncoupled in H (H[c][j] = 0 for j != c) -- the
+ *             mu_p|0><0| state of linear absorption, P:301 -- every sigma_u keeps that shape, and the state is
+ *             held and propagated as one N-vector per node (kernels_ket.cu; Taylor/Horner form of RK4).
+ *             All getters still return full matrices.  0 = always full matrices.  Takes effect at the next
+ *             heom_set_state; heom_set_full_state always selects full matrices. */
 heom_status heom_set_option(heom_ctx* ctx, const char* name, int value);
 
 int64_t heom_num_nodes(const heom_ctx* ctx); /* Eq. 9: C(W+D, D) */

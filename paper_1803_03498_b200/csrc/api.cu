@@ -66,6 +66,10 @@ struct heom_ctx {
   void* d_lent = nullptr;
   double *d_Hs = nullptr, *d_delta = nullptr;
   double2* d_A = nullptr;    // operator of heom_expectation
+  // column-sparse states (kernels_ket.cu): sigma_u = v_u e_col^T, selected by heom_set_state after an exact check
+  int ket_opt = 1;           // option "ket": 1 = use the column kernel when the conditions hold, 0 = never
+  int ket_col = -1;          // >= 0: the state is held as kets [nodes][N] (ky, kacc in the y region; kxa, kxb in acc's)
+  double2* d_S0 = nullptr;   // sigma_0 expanded to a full matrix for the observables
   size_t n_links = 0;
   unsigned long long* d_tickets = nullptr;   // work counter of the persistent kernel
   unsigned long long ticket_base = 0;
@@ -149,7 +153,7 @@ int links_row(int W) { return (2 * W + (W + 3) / 4 + 3) / 4 * 4; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, off_linksP, off_Hs, off_delta, off_A, off_lptr, off_lent, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, off_linksP, off_Hs, off_delta, off_A, off_S0, off_lptr, off_lent, total;
 };
 
 Layout layout_of(const heom_ctx* c) {
@@ -179,6 +183,7 @@ Layout layout_of(const heom_ctx* c) {
   L.off_Hs = o; o += align_up(N * N * 8);
   L.off_delta = o; o += align_up(N * 8);
   L.off_A = o; o += align_up(N * N * 16);
+  L.off_S0 = o; o += align_up(N * N * 16);
   if (large_supported((int)N, (int)W)) {
     // every valid link appears once as "+" and once as "-": count the "-" links of the host table
     size_t links = 0;
@@ -215,7 +220,10 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
     ctx->ev_used += 2;
     CU(cudaEventRecord(e0, ctx->stream));
   }
-  if (ctx->use_large)
+  if (ctx->ket_col >= 0)
+    CU(launch_rhs_ket(p, ctx->d_linksP, ctx->lrowP, ctx->ket_col, ctx->cd.a_plus.data(), ctx->cd.a_minus_x.data(),
+                      ctx->cd.a_minus_o.data(), ctx->H.data(), ctx->cd.delta.data(), ctx->sms, ctx->stream));
+  else if (ctx->use_large)
     CU(launch_rhs_large(p, ctx->d_lptr, ctx->d_lent, ctx->d_Hs, ctx->d_delta, ctx->cd.a_plus.data(),
                         ctx->cd.a_minus_x.data(), ctx->cd.a_minus_o.data(), ctx->sms, ctx->d_tickets,
                         &ctx->ticket_base, ctx->stream));
@@ -230,6 +238,24 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
   else CU(launch_rhs_generic(p, ctx->stream));
   ctx->launches += 1;
   if (ctx->timing) CU(cudaEventRecord(e1, ctx->stream));
+  return HEOM_OK;
+}
+
+// ket buffers: two in the y region, two in the acc region (each region holds nodes*N*N >= 2*nodes*N elements)
+double2* ket_buf(const heom_ctx* c, int which) {
+  const size_t n = (size_t)c->h.nodes * c->h.N;
+  double2* base = (which < 2) ? c->y : c->acc;
+  return base + (size_t)(which & 1) * n;
+}
+enum { KET_Y = 0, KET_ACC = 1, KET_XA = 2, KET_XB = 3 };
+
+// DEVICE pointer to sigma_0 as a full N x N matrix (ket mode: expanded into d_S0 first)
+heom_status sigma0_matrix(heom_ctx* ctx, const double2** out) {
+  if (ctx->ket_col < 0) { *out = ctx->y + (size_t)ctx->h.slot_of[0] * ctx->stride; return HEOM_OK; }
+  CU(launch_ket_expand(ket_buf(ctx, KET_Y) + (size_t)ctx->h.slot_of[0] * ctx->h.N, ctx->d_S0, 1, ctx->h.N,
+                       ctx->ket_col, ctx->stream));
+  ctx->launches += 1;
+  *out = ctx->d_S0;
   return HEOM_OK;
 }
 
@@ -310,6 +336,7 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
     return HEOM_OK;
   }
   if (s == "acc_red") { ctx->acc_red = value ? 1 : 0; return HEOM_OK; }
+  if (s == "ket") { ctx->ket_opt = value ? 1 : 0; return HEOM_OK; }   // takes effect at the next heom_set_state
   if (s == "rk4_form") {
     if (value < -1 || value > 1) return fail(ctx, HEOM_EINVAL, "rk4_form must be -1, 0 or 1");
     ctx->rk4_form = value;
@@ -423,6 +450,8 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->d_Hs = (double*)(base + L.off_Hs);
   ctx->d_delta = (double*)(base + L.off_delta);
   ctx->d_A = (double2*)(base + L.off_A);
+  ctx->d_S0 = (double2*)(base + L.off_S0);
+  ctx->ket_col = -1;
   ctx->d_lptr = (int64_t*)(base + L.off_lptr);
   ctx->d_lent = (void*)(base + L.off_lent);
   ctx->d_linksP = (int32_t*)(base + L.off_linksP);
@@ -557,7 +586,36 @@ heom_status heom_set_state(heom_ctx* ctx, const double* sigma0) {
       }
     ctx->state_hermitian = herm;
   }
+  ctx->ket_col = -1;
+  if (ctx->ket_opt && ctx->use_hpipe && !ctx->use_tiny && ket_supported(ctx->h.N, dev_modes(ctx), ctx->h.D)) {
+    // column-sparse state?  exactly one non-zero column c, state c without a bath and uncoupled in H
+    const int N = ctx->h.N;
+    int col = -1, ncols = 0;
+    for (int j = 0; j < N; ++j) {
+      bool nz = false;
+      for (int i = 0; i < N; ++i) nz = nz || sigma0[2 * (i * N + j)] != 0.0 || sigma0[2 * (i * N + j) + 1] != 0.0;
+      if (nz) { col = j; ++ncols; }
+    }
+    bool ok = ncols == 1 && ctx->bath_of[(size_t)col] < 0;
+    for (int j = 0; ok && j < N; ++j)
+      if (j != col && ctx->H[(size_t)col * N + j] != 0.0) ok = false;
+    if (ok) ctx->ket_col = col;
+  }
   CU(cudaStreamSynchronize(ctx->stream));  // the pinned staging buffer may still be in flight
+  if (ctx->ket_col >= 0) {
+    const int N = ctx->h.N;
+    for (int i = 0; i < N; ++i) {
+      ctx->h_pinned[2 * i] = sigma0[2 * (i * N + ctx->ket_col)];
+      ctx->h_pinned[2 * i + 1] = sigma0[2 * (i * N + ctx->ket_col) + 1];
+    }
+    double2* ky = ket_buf(ctx, KET_Y);
+    CU(cudaMemsetAsync(ky, 0, (size_t)ctx->h.nodes * N * 16, ctx->stream));
+    CU(cudaMemcpyAsync(ky + (size_t)ctx->h.slot_of[0] * N, ctx->h_pinned, (size_t)N * 16, cudaMemcpyHostToDevice,
+                       ctx->stream));
+    ctx->state_hermitian = false;
+    ctx->have_state = true;
+    return HEOM_OK;
+  }
   std::memcpy(ctx->h_pinned, sigma0, NN * 16);
   CU(cudaMemsetAsync(ctx->y, 0, ctx->state_bytes, ctx->stream));
   CU(cudaMemcpyAsync(ctx->y + (size_t)ctx->h.slot_of[0] * ctx->stride, ctx->h_pinned, NN * 16,
@@ -570,6 +628,7 @@ heom_status heom_set_full_state(heom_ctx* ctx, const double* sigma) {
   if (!ctx || !sigma) return HEOM_EINVAL;
   if (!ctx->bound) return fail(ctx, HEOM_ESTATE, "no workspace bound");
   const size_t NN = (size_t)ctx->h.N * ctx->h.N, nodes = (size_t)ctx->h.nodes;
+  ctx->ket_col = -1;
   {
     // exact Hermiticity of every node selects the row-gather kernel (checked, never assumed)
     const int N = ctx->h.N;
@@ -604,6 +663,11 @@ static heom_status read_back(heom_ctx* ctx, const double2* dev_state, double2* s
 heom_status heom_get_full_state(heom_ctx* ctx, double* sigma) {
   if (!ctx || !sigma) return HEOM_EINVAL;
   if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
+  if (ctx->ket_col >= 0) {
+    CU(launch_ket_expand(ket_buf(ctx, KET_Y), ctx->xa, ctx->h.nodes, ctx->h.N, ctx->ket_col, ctx->stream));
+    ctx->launches += 1;
+    return read_back(ctx, ctx->xa, ctx->xb, sigma);
+  }
   return read_back(ctx, ctx->y, ctx->xa, sigma);
 }
 
@@ -611,6 +675,14 @@ heom_status heom_rhs(heom_ctx* ctx, double* dsigma) {
   if (!ctx || !dsigma) return HEOM_EINVAL;
   if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
   RhsParams p = base_params(ctx);
+  if (ctx->ket_col >= 0) {
+    p.x = ket_buf(ctx, KET_Y); p.rhs_only = 1; p.out_acc = ket_buf(ctx, KET_XA);
+    heom_status s = launch_rhs(ctx, p);
+    if (s != HEOM_OK) return s;
+    CU(launch_ket_expand(ket_buf(ctx, KET_XA), ctx->xa, ctx->h.nodes, ctx->h.N, ctx->ket_col, ctx->stream));
+    ctx->launches += 1;
+    return read_back(ctx, ctx->xa, ctx->xb, dsigma);
+  }
   p.x = ctx->y; p.rhs_only = 1; p.out_acc = ctx->xa;
   heom_status s = launch_rhs(ctx, p);
   if (s != HEOM_OK) return s;
@@ -627,6 +699,23 @@ heom_status heom_rk4_steps(heom_ctx* ctx, double dt, int nsteps) {
   if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
   RhsParams p = base_params(ctx);
   p.rhs_only = 0;
+  if (ctx->ket_col >= 0) {
+    /* column-sparse state: Taylor/Horner form (R6) on the kets, 4 launches per step */
+    double2 *ky = ket_buf(ctx, KET_Y), *ka = ket_buf(ctx, KET_ACC), *kxa = ket_buf(ctx, KET_XA), *kxb = ket_buf(ctx, KET_XB);
+    p.taylor = 1;
+    for (int step = 0; step < nsteps; ++step) {
+      heom_status s;
+      p.x = ky; p.acc_in = ky; p.out_x = kxa; p.out_acc = ka; p.ax = p.bx = dt;          /* v1; acc = y + v1 */
+      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+      p.x = kxa; p.acc_in = ka; p.out_x = kxb; p.ax = p.bx = dt / 2.0;                    /* v2; acc += v2 */
+      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+      p.x = kxb; p.out_x = kxa; p.ax = p.bx = dt / 3.0;                                   /* v3; acc += v3 */
+      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+      p.x = kxa; p.out_x = nullptr; p.out_acc = ky; p.ax = p.bx = dt / 4.0;               /* y = acc + v4 */
+      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
+    }
+    return HEOM_OK;
+  }
   if (ctx->use_tiny && nsteps > 0) {
     /* launch-latency-bound hierarchies: all nsteps classical RK4 steps in one launch of one CTA */
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -709,7 +798,9 @@ heom_status heom_populations(heom_ctx* ctx, double* pop, double* trace_re, doubl
   if (!ctx) return HEOM_EINVAL;
   if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
   const int N = ctx->h.N;
-  CU(launch_populations(ctx->y + (size_t)ctx->h.slot_of[0] * ctx->stride, N, ctx->d_scratch, ctx->stream));
+  const double2* s0 = nullptr;
+  { heom_status st = sigma0_matrix(ctx, &s0); if (st != HEOM_OK) return st; }
+  CU(launch_populations(s0, N, ctx->d_scratch, ctx->stream));
   ctx->launches += 1;
   CU(cudaMemcpyAsync(ctx->h_pinned, ctx->d_scratch, (size_t)(N + 2) * 8, cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
@@ -729,7 +820,9 @@ heom_status heom_expectation(heom_ctx* ctx, const double* A, double* re, double*
   CU(cudaStreamSynchronize(ctx->stream));  // the pinned staging buffer may still be in flight
   std::memcpy(ctx->h_pinned, A, NN * 16);
   CU(cudaMemcpyAsync(ctx->d_A, ctx->h_pinned, NN * 16, cudaMemcpyHostToDevice, ctx->stream));
-  CU(launch_expectation(ctx->y + (size_t)ctx->h.slot_of[0] * ctx->stride, ctx->d_A, N, ctx->d_scratch, ctx->stream));
+  const double2* s0 = nullptr;
+  { heom_status st = sigma0_matrix(ctx, &s0); if (st != HEOM_OK) return st; }
+  CU(launch_expectation(s0, ctx->d_A, N, ctx->d_scratch, ctx->stream));
   ctx->launches += 1;
   CU(cudaMemcpyAsync(ctx->h_pinned, ctx->d_scratch, 16, cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
@@ -758,6 +851,7 @@ heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches)
 
 const char* heom_kernel_name(const heom_ctx* c) {
   if (!c) return "none";
+  if (c->ket_col >= 0) return "rhs_ket_kernel";
   if (c->use_large) return "rhs_large_kernel";
   if (c->use_hpipe) return (c->herm_opt && c->state_hermitian) ? "rhs_hpipe_kernel" : "rhs_hpipe_general_kernel";
   if (c->use_herm && c->herm_opt && c->state_hermitian) return "rhs_herm_kernel";

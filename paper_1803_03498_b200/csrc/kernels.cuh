@@ -94,6 +94,17 @@ cudaError_t launch_permute(const double2* src, double2* dst, const int32_t* slot
 // out[0..N-1] = Re sigma_0[i][i]; out[N], out[N+1] = trace (re, im)
 cudaError_t launch_populations(const double2* node0, int N, double* out, cudaStream_t s);
 
+// Column-sparse states (kernels_ket.cu): sigma_u = v_u e_col^T for every node, state `col` without a bath and
+// uncoupled in H (linear absorption).  p.x, p.acc_in, p.out_x, p.out_acc are KET buffers [nodes][N];
+// p.rhs_only / p.ax / p.bx as for the matrix kernels (Taylor form: out_x = ax k, out_acc = acc_in + bx k).
+// links / lrow: the rows written by hpipe_pack_links; a_*, H_host, delta_host: HOST.
+bool ket_supported(int N, int W, int D);
+cudaError_t launch_rhs_ket(const RhsParams& p, const int32_t* links, int lrow, int col, const double* a_plus,
+                           const double* a_minus_x, const double* a_minus_o, const double* H_host,
+                           const double* delta_host, int sms, cudaStream_t s);
+// dst[slot][i][j] = (j == col) ? ket[slot][i] : 0   (full matrices for the host-visible getters)
+cudaError_t launch_ket_expand(const double2* ket, double2* dst, long long nodes, int N, int col, cudaStream_t s);
+
 // out[0], out[1] = Tr(A sigma_0) (re, im); A: DEVICE [N][N] complex128
 cudaError_t launch_expectation(const double2* node0, const double2* A, int N, double* out, cudaStream_t s);
 

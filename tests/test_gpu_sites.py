@@ -62,7 +62,7 @@ def test_absorption_propagation_parity(sites, K, D, steps, form):
     w = workloads.fmo_like()
     w = w.with_(H_cm=w.H_cm[:sites, :sites])
     H, bath_state, dip = workloads.with_ground_state(w)
-    o, g = _pair(H, w.lambda_cm, w.nu_per_fs, 77.0, K, D, bath_state, rk4_form=form)
+    o, g = _pair(H, w.lambda_cm, w.nu_per_fs, 77.0, K, D, bath_state, rk4_form=form, ket=0 if form == 0 else 1)
     mu = workloads.dipole_operator(dip, 2).astype(complex)
     rho0 = np.zeros_like(mu); rho0[0, 0] = 1.0
     s0 = mu @ rho0
@@ -101,3 +101,81 @@ def test_linear_absorption_spectrum_matches_oracle():
     peak = omega[np.argmax(spec)]
     ev = np.linalg.eigvalsh(w.H_cm)
     assert np.min(np.abs(peak - ev)) < 60.0
+
+
+# ------------------------------------------------------------- column-sparse states (kernels_ket.cu)
+def _ket_system(N, col, seed):
+    """Random H with state `col` uncoupled (Eq. 48 block form), baths on every other state."""
+    rng = np.random.default_rng(5000 + seed)
+    H = rng.normal(0.0, 80.0, (N, N)); H = (H + H.T) / 2
+    H[col, :] = 0.0; H[:, col] = 0.0; H[col, col] = rng.normal(0.0, 50.0)
+    bath_state = [s for s in range(N) if s != col]
+    B = N - 1
+    return H, bath_state, rng.uniform(20.0, 45.0, B), rng.uniform(0.015, 0.03, B)
+
+
+@pytest.mark.parametrize("N,col,K,D,steps", [(8, 0, 1, 4, 200), (8, 7, 0, 5, 200), (5, 2, 2, 4, 150), (3, 1, 3, 5, 100),
+                                             (16, 0, 0, 3, 100), (13, 12, 1, 2, 100), (2, 0, 1, 9, 100), (9, 4, 0, 4, 100)])
+def test_ket_kernel_parity(N, col, K, D, steps):
+    """sigma_0(0) with one non-zero column on an unbathed, uncoupled state: held as kets; the RHS, the RK4 run on
+    every node, the populations and Tr(A sigma_0) all against the oracle's full matrices."""
+    H, bath_state, lam, nu = _ket_system(N, col, N + K + D)
+    o, g = _pair(H, lam, nu, 120.0, K, D, bath_state)
+    rng = np.random.default_rng(N)
+    s0 = np.zeros((N, N), dtype=complex)
+    s0[:, col] = rng.standard_normal(N) + 1j * rng.standard_normal(N)
+    o.set_state(s0); g.set_state(s0)
+    if g.nodes * N * N > 2048:
+        assert g.kernel_name() == "rhs_ket_kernel"
+    assert np.array_equal(g.get_full_state(), o.get_full_state())
+    assert rel_err(g.rhs(), o.rhs()) < RHS_TOL
+    o.rk4_steps(0.5, steps); g.rk4_steps(0.5, steps)
+    ref, got = o.get_full_state(), g.get_full_state()
+    assert rel_err(got, ref) < STATE_TOL
+    mask = np.ones(N, bool); mask[col] = False
+    assert np.abs(got[:, :, mask]).max() == 0.0
+    A = rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
+    c_ref = np.trace(A @ ref[0])
+    assert abs(g.expectation(A) - c_ref) < 1e-11 * max(1.0, abs(c_ref))
+    pop, tr = g.populations()
+    assert np.allclose(pop, np.diag(ref[0]).real, atol=1e-11) and abs(tr - np.trace(ref[0])) < 1e-11
+    # the same run with full matrices (option ket = 0) agrees too, and a later full-state upload leaves ket mode
+    g.set_option("ket", 0)
+    g.set_state(s0)
+    assert g.kernel_name() != "rhs_ket_kernel"
+    g.rk4_steps(0.5, steps)
+    assert rel_err(g.get_full_state(), ref) < STATE_TOL
+    g.set_option("ket", 1)
+    g.set_state(s0)
+    st = workloads.random_state(o.nodes, N, seed=3)
+    o.set_full_state(st); g.set_full_state(st)
+    assert g.kernel_name() != "rhs_ket_kernel"
+    assert rel_err(g.rhs(), o.rhs()) < RHS_TOL
+
+
+def test_ket_kernel_not_taken_when_conditions_fail():
+    """One non-zero column is not enough: the state of that column must be unbathed AND uncoupled in H."""
+    N, K, D = 6, 1, 4
+    H, bath_state, lam, nu = _ket_system(N, 0, 1)
+    s0 = np.zeros((N, N), dtype=complex); s0[:, 0] = np.arange(1, N + 1)
+    # (a) column of a bathed state
+    o, g = _pair(H, lam, nu, 120.0, K, D, bath_state)
+    s1 = np.zeros((N, N), dtype=complex); s1[:, 2] = np.arange(1, N + 1)
+    o.set_state(s1); g.set_state(s1)
+    assert g.kernel_name() != "rhs_ket_kernel"
+    o.rk4_steps(0.5, 50); g.rk4_steps(0.5, 50)
+    assert rel_err(g.get_full_state(), o.get_full_state()) < STATE_TOL
+    # (b) unbathed state coupled in H: the other columns fill in
+    H2 = H.copy(); H2[0, 3] = H2[3, 0] = 25.0
+    o, g = _pair(H2, lam, nu, 120.0, K, D, bath_state)
+    o.set_state(s0); g.set_state(s0)
+    assert g.kernel_name() != "rhs_ket_kernel"
+    o.rk4_steps(0.5, 50); g.rk4_steps(0.5, 50)
+    ref = o.get_full_state()
+    assert np.abs(ref[:, :, 1:]).max() > 0.0
+    assert rel_err(g.get_full_state(), ref) < STATE_TOL
+    # (c) two non-zero columns
+    o, g = _pair(H, lam, nu, 120.0, K, D, bath_state)
+    s2 = s0.copy(); s2[1, 1] = 1.0
+    o.set_state(s2); g.set_state(s2)
+    assert g.kernel_name() != "rhs_ket_kernel"
