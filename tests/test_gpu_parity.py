@@ -253,3 +253,26 @@ def test_call_order_errors_on_gpu():
     g2.rk4_steps(1.0, 3)
     assert g2.launch_count() - n0 == 12     # otherwise 4 fused stage kernels per step, nothing else
     assert rel_err(g2.get_full_state(), g.get_full_state()) < 1e-12
+
+
+@pytest.mark.skipif(os.environ.get("HEOM_LONG", "0") != "1",
+                    reason="full-length runs: minutes of oracle time per config (set HEOM_LONG=1)")
+@pytest.mark.parametrize("name", ["cfg2", "cfg4"])
+def test_full_length_runs(name):
+    """The north-star statement taken literally: BASELINE configs 2 and 4 at FULL size for their FULL step count
+    (1000 / 500 RK4 steps) from sigma_0 = |1><1|, every node of the final state compared with the oracle
+    (1e-10 max-abs relative to max|sigma|).  Opt-in: the oracle needs ~5 / ~14 minutes on 16 cores; the result of
+    the last run on a B200 is recorded in profiles/r1d_full_length.md."""
+    w = workloads.get(name)
+    o, g = _pair(w)
+    o.set_state(w.sigma0()); g.set_state(w.sigma0())
+    g.rk4_steps(w.dt_fs, w.steps)
+    o.rk4_steps(w.dt_fs, w.steps)
+    ref, got = o.get_full_state(), g.get_full_state()
+    err = rel_err(got, ref)
+    pop, tr = g.populations()
+    print(f"FULL_LENGTH {w.name} nodes={w.nodes} steps={w.steps} kernel={g.kernel_name()} rel_err={err:.3e} "
+          f"trace={tr.real:.15f} rho11={pop[0]:.12f}")
+    assert err < STATE_TOL
+    assert abs(tr - 1.0) < 1e-11
+    assert np.array_equal(got, np.conj(np.swapaxes(got, 1, 2)))

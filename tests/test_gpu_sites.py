@@ -116,11 +116,12 @@ def _ket_system(N, col, seed):
 
 @pytest.mark.parametrize("N,col,K,D,steps", [(8, 0, 1, 4, 200), (8, 7, 0, 5, 200), (5, 2, 2, 4, 150), (3, 1, 3, 5, 100),
                                              (16, 0, 0, 3, 100), (13, 12, 1, 2, 100), (2, 0, 1, 9, 100), (9, 4, 0, 4, 100)])
-def test_ket_kernel_parity(N, col, K, D, steps):
+@pytest.mark.parametrize("order", [1, 0])
+def test_ket_kernel_parity(N, col, K, D, steps, order):
     """sigma_0(0) with one non-zero column on an unbathed, uncoupled state: held as kets; the RHS, the RK4 run on
     every node, the populations and Tr(A sigma_0) all against the oracle's full matrices."""
     H, bath_state, lam, nu = _ket_system(N, col, N + K + D)
-    o, g = _pair(H, lam, nu, 120.0, K, D, bath_state)
+    o, g = _pair(H, lam, nu, 120.0, K, D, bath_state, order=order)
     rng = np.random.default_rng(N)
     s0 = np.zeros((N, N), dtype=complex)
     s0[:, col] = rng.standard_normal(N) + 1j * rng.standard_normal(N)
