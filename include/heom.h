@@ -153,6 +153,35 @@ heom_status heom_populations(heom_ctx* ctx, double* pop, double* trace_re,
  * Computed by a device reduction kernel; synchronises. */
 heom_status heom_expectation(heom_ctx* ctx, const double* A, double* re, double* im);
 
+/* ---- One hierarchy sharded over several GPUs (the paper's partitions + halo regions) ----
+ * One process per GPU; rank r of `world` owns a contiguous range of the lexicographic node order and keeps ghost
+ * copies of the neighbours of its nodes that live on other ranks.  A partition context behaves like a context
+ * whose hierarchy is the n_owned + n_ghost LOCAL nodes (heom_num_nodes, heom_get_tables with local indices,
+ * heom_set_full_state / heom_get_full_state / heom_rhs over the local nodes; ghost rows of a result are not
+ * meaningful).  Local order: owned nodes, then ghosts grouped by owning rank in the order the owner sends them,
+ * so the ghost rows of a state buffer ARE the receive buffer of the exchange.  The caller moves the halos
+ * (torch.distributed / NCCL all_to_all_single in paper_1803_03498_b200/sharded.py): per RK4 step
+ *   for stage in 0..3: heom_rk4_stage; heom_stage_output -> buf; heom_pack_halo(buf -> send);
+ *                      all-to-all: send rows -> the peers' ghost rows of buf
+ * heom_set_state sets the rank's copy of sigma_0 (owned or ghost) if it holds one. */
+heom_status heom_create_partition(heom_ctx** out, int n_states, const double* H_cm, int n_baths,
+                                  const int* bath_state, const double* lambda_cm, const double* nu_per_fs,
+                                  double T_kelvin, int K, int D, int device, int rank, int world);
+int64_t heom_partition_owned(const heom_ctx* ctx); /* n_owned (the first n_owned local nodes) */
+/* global_ids HOST int64 [local nodes]: pinned-order id (R1) of every local node; send_counts, recv_counts HOST
+ * int64 [world]: nodes sent to / ghosts received from every peer; send_idx HOST int32 [sum send_counts]: local
+ * indices of the nodes to send, grouped by peer.  Any pointer may be NULL. */
+heom_status heom_partition_plan(const heom_ctx* ctx, int64_t* global_ids, int64_t* send_counts,
+                                int64_t* recv_counts, int32_t* send_idx);
+/* One fused RHS + RK4-stage launch, stage = 0..3 of the current step (matrix kernels only). */
+heom_status heom_rk4_stage(heom_ctx* ctx, double dt_fs, int stage);
+/* DEVICE pointer (complex128 [local nodes][N][N], local order) of the buffer the NEXT stage reads, i.e. the one
+ * whose ghost rows must be refreshed after `stage` (after stage 3: the new state y). */
+heom_status heom_stage_output(heom_ctx* ctx, int stage, void** dev_ptr);
+/* dst_dev[q] = node send_idx[q] of src_dev (device kernel on the bound stream); dst_dev DEVICE, sum(send_counts)
+ * nodes of N*N complex128. */
+heom_status heom_pack_halo(heom_ctx* ctx, const void* src_dev, void* dst_dev);
+
 /* Introspection for the harness. */
 int64_t heom_launch_count(const heom_ctx* ctx); /* kernels launched so far */
 /* With option "timing"=1: sum of CUDA-event durations of the RHS/stage kernels

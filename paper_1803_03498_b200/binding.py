@@ -18,7 +18,8 @@ _STATUS = {0: "HEOM_OK", -1: "HEOM_EINVAL", -2: "HEOM_ENOMEM", -3: "HEOM_ECUDA",
 
 # every symbol include/heom.h declares (tests check the library exports all of them)
 SYMBOLS = [
-    "heom_create", "heom_create_sites", "heom_num_baths", "heom_expectation", "heom_destroy", "heom_set_option", "heom_num_nodes", "heom_num_modes",
+    "heom_create", "heom_create_sites", "heom_create_partition", "heom_partition_owned", "heom_partition_plan",
+    "heom_rk4_stage", "heom_stage_output", "heom_pack_halo", "heom_num_baths", "heom_expectation", "heom_destroy", "heom_set_option", "heom_num_nodes", "heom_num_modes",
     "heom_get_tables", "heom_get_coefficients", "heom_workspace_bytes", "heom_bind_workspace",
     "heom_set_state", "heom_set_full_state", "heom_get_full_state", "heom_rhs", "heom_rk4_steps",
     "heom_sync", "heom_populations", "heom_launch_count", "heom_kernel_time", "heom_kernel_name",
@@ -47,6 +48,14 @@ def load_library():
     lib.heom_create.argtypes = [C.POINTER(P), C.c_int, dp, dp, dp, C.c_double, C.c_int, C.c_int, C.c_int]
     lib.heom_create_sites.argtypes = [C.POINTER(P), C.c_int, dp, C.c_int, C.POINTER(C.c_int), dp, dp, C.c_double,
                                       C.c_int, C.c_int, C.c_int]
+    lib.heom_create_partition.argtypes = [C.POINTER(P), C.c_int, dp, C.c_int, C.POINTER(C.c_int), dp, dp, C.c_double,
+                                          C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
+    lib.heom_partition_owned.argtypes = [P]
+    lib.heom_partition_owned.restype = C.c_int64
+    lib.heom_partition_plan.argtypes = [P, P, P, P, P]
+    lib.heom_rk4_stage.argtypes = [P, C.c_double, C.c_int]
+    lib.heom_stage_output.argtypes = [P, C.c_int, C.POINTER(P)]
+    lib.heom_pack_halo.argtypes = [P, P, P]
     lib.heom_num_baths.argtypes = [P]
     lib.heom_expectation.argtypes = [P, P, P, P]
     lib.heom_destroy.argtypes = [P]
@@ -85,9 +94,11 @@ def _dptr(a):
 class Heom:
     """One truncated hierarchy bound to one GPU stream.  Mirrors include/heom.h one to one."""
 
-    def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, device=0, bath_state=None, **options):
+    def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, device=0, bath_state=None, partition=None,
+                 **options):
         """bath_state=None: heom_create (one bath per state); else heom_create_sites with the listed states
-        (lambda_cm, nu_per_fs then have one entry per bath)."""
+        (lambda_cm, nu_per_fs then have one entry per bath).  partition=(rank, world): heom_create_partition --
+        this context holds rank's part of the hierarchy (owned + ghost nodes)."""
         self._lib = load_library()
         self._h = None
         H = np.ascontiguousarray(H_cm, dtype=np.float64)
@@ -98,7 +109,14 @@ class Heom:
         lam = np.ascontiguousarray(np.broadcast_to(lambda_cm, (self.B,)), dtype=np.float64)
         nu = np.ascontiguousarray(np.broadcast_to(nu_per_fs, (self.B,)), dtype=np.float64)
         h = C.c_void_p()
-        if bath_state is None:
+        self.partition = partition
+        if partition is not None:
+            states = list(range(self.N)) if bath_state is None else bath_state
+            bs = (C.c_int * self.B)(*[int(x) for x in states])
+            rc = self._lib.heom_create_partition(C.byref(h), self.N, _dptr(H), self.B, bs, _dptr(lam), _dptr(nu),
+                                                 float(T_kelvin), int(K), int(D), int(device),
+                                                 int(partition[0]), int(partition[1]))
+        elif bath_state is None:
             rc = self._lib.heom_create(C.byref(h), self.N, _dptr(H), _dptr(lam), _dptr(nu),
                                        float(T_kelvin), int(K), int(D), int(device))
         else:
@@ -207,6 +225,39 @@ class Heom:
         self._ck(self._lib.heom_populations(self._h, pop.ctypes.data, C.addressof(tr[0]),
                                             C.addressof(tr[1])))
         return pop, complex(tr[0].value, tr[1].value)
+
+    # -- partitions (one hierarchy over several GPUs) -----------------------------------------
+    def owned(self):
+        return int(self._lib.heom_partition_owned(self._h))
+
+    def partition_plan(self):
+        """(global_ids [local nodes], send_counts [world], recv_counts [world], send_idx [sum send_counts])."""
+        world = self.partition[1]
+        gid = np.empty(self.nodes, dtype=np.int64)
+        sc = np.empty(world, dtype=np.int64); rc_ = np.empty(world, dtype=np.int64)
+        self._ck(self._lib.heom_partition_plan(self._h, gid.ctypes.data, sc.ctypes.data, rc_.ctypes.data, None))
+        idx = np.empty(int(sc.sum()), dtype=np.int32)
+        self._ck(self._lib.heom_partition_plan(self._h, None, None, None, idx.ctypes.data if idx.size else None))
+        return gid, sc, rc_, idx
+
+    def rk4_stage(self, dt_fs, stage):
+        self._ck(self._lib.heom_rk4_stage(self._h, float(dt_fs), int(stage)))
+
+    def stage_output(self, stage):
+        """Device pointer of the buffer whose ghost rows must be refreshed after `stage`."""
+        ptr = C.c_void_p()
+        self._ck(self._lib.heom_stage_output(self._h, int(stage), C.byref(ptr)))
+        return int(ptr.value)
+
+    def pack_halo(self, src_ptr, dst_ptr):
+        self._ck(self._lib.heom_pack_halo(self._h, int(src_ptr), int(dst_ptr)))
+
+    def buffer_view(self, dev_ptr):
+        """torch view [local nodes][2 N N] float64 of a state buffer inside the bound workspace tensor."""
+        import torch
+        off = int(dev_ptr) - self._workspace.data_ptr()
+        nbytes = self.nodes * self.N * self.N * 16
+        return self._workspace[off:off + nbytes].view(torch.float64).view(self.nodes, 2 * self.N * self.N)
 
     def expectation(self, A):
         """Tr(A sigma_0) (heom_expectation)."""

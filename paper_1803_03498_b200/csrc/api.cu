@@ -70,6 +70,11 @@ struct heom_ctx {
   int ket_opt = 1;           // option "ket": 1 = use the column kernel when the conditions hold, 0 = never
   int ket_col = -1;          // >= 0: the state is held as kets [nodes][N] (ky, kacc in the y region; kxa, kxb in acc's)
   double2* d_S0 = nullptr;   // sigma_0 expanded to a full matrix for the observables
+  // one rank's part of a hierarchy sharded over several GPUs (heom_create_partition)
+  bool partitioned = false;
+  int part_rank = 0, part_world = 1;
+  Partition part;
+  int32_t* d_send = nullptr; // DEVICE copy of part.send_idx
   size_t n_links = 0;
   unsigned long long* d_tickets = nullptr;   // work counter of the persistent kernel
   unsigned long long ticket_base = 0;
@@ -105,7 +110,9 @@ heom_status cuda_fail(heom_ctx* c, cudaError_t e, const char* where) {
     if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);       \
   } while (0)
 
-int dev_modes(const heom_ctx* c) { return c->h.N * c->h.M; }   // Wd: mode columns of the device tables
+int dev_modes(const heom_ctx* c) { return c->h.N * c->h.M; }
+// storage slot of the hierarchy's root node sigma_0 (-1: a partition that does not hold it)
+int64_t root_slot(const heom_ctx* c) { return c->partitioned ? c->part.root : (int64_t)c->h.slot_of[0]; }   // Wd: mode columns of the device tables
 
 // c->cd, c->Tterm from c->c and the bath -> state map
 void expand_coefficients(heom_ctx* c) {
@@ -139,7 +146,8 @@ bool ensure_hierarchy(heom_ctx* c) {
   if (c->hierarchy_built && c->built_order == c->order) return true;
   std::string err;
   const int n_states = c->h.N;
-  const bool ok = build_hierarchy(c->B, c->h.K, c->h.D, c->order, c->h, err);   // tuples over the B*M modes
+  bool ok = build_hierarchy(c->B, c->h.K, c->h.D, c->partitioned ? 1 : c->order, c->h, err);   // tuples over the B*M modes
+  if (ok && c->partitioned) ok = restrict_hierarchy(c->h, c->part_rank, c->part_world, c->part, err);
   c->h.N = n_states;
   if (!ok) { c->err = err; return false; }
   c->hierarchy_built = true;
@@ -153,7 +161,7 @@ int links_row(int W) { return (2 * W + (W + 3) / 4 + 3) / 4 * 4; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, off_linksP, off_Hs, off_delta, off_A, off_S0, off_lptr, off_lent, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, off_linksP, off_Hs, off_delta, off_A, off_S0, off_send, off_lptr, off_lent, total;
 };
 
 Layout layout_of(const heom_ctx* c) {
@@ -184,6 +192,7 @@ Layout layout_of(const heom_ctx* c) {
   L.off_delta = o; o += align_up(N * 8);
   L.off_A = o; o += align_up(N * N * 16);
   L.off_S0 = o; o += align_up(N * N * 16);
+  L.off_send = o; o += align_up(c->part.send_idx.size() * 4 + 16);
   if (large_supported((int)N, (int)W)) {
     // every valid link appears once as "+" and once as "-": count the "-" links of the host table
     size_t links = 0;
@@ -251,7 +260,8 @@ enum { KET_Y = 0, KET_ACC = 1, KET_XA = 2, KET_XB = 3 };
 
 // DEVICE pointer to sigma_0 as a full N x N matrix (ket mode: expanded into d_S0 first)
 heom_status sigma0_matrix(heom_ctx* ctx, const double2** out) {
-  if (ctx->ket_col < 0) { *out = ctx->y + (size_t)ctx->h.slot_of[0] * ctx->stride; return HEOM_OK; }
+  if (root_slot(ctx) < 0) return fail(ctx, HEOM_ESTATE, "sigma_0 is not held by this partition");
+  if (ctx->ket_col < 0) { *out = ctx->y + (size_t)root_slot(ctx) * ctx->stride; return HEOM_OK; }
   CU(launch_ket_expand(ket_buf(ctx, KET_Y) + (size_t)ctx->h.slot_of[0] * ctx->h.N, ctx->d_S0, 1, ctx->h.N,
                        ctx->ket_col, ctx->stream));
   ctx->launches += 1;
@@ -259,15 +269,52 @@ heom_status sigma0_matrix(heom_ctx* ctx, const double2** out) {
   return HEOM_OK;
 }
 
+// One fused RHS + RK4-stage launch (stage = 0..3) of the matrix kernels, in the form the kernel in use takes (R6):
+//  - Taylor/Horner (pipelined small-N and tensor-core kernels unless rk4_form = 0):
+//      v1 = dt f(y), v_s = (dt/s) f(v_{s-1}), y' = y + v1 + v2 + v3 + v4; the stages never read y: 14 state sizes
+//  - classical: k1 = f(y); xa = y + dt/2 k1; acc = y + dt/6 k1 | k2 = f(xa); xb = y + dt/2 k2; acc += dt/3 k2 |
+//               k3 = f(xb); xa = y + dt k3; acc += dt/3 k3     | k4 = f(xa); y = acc + dt/6 k4
+// After the stage the next stage's input is xa (stages 0, 2), xb (stage 1) or y (stage 3): heom_stage_output.
+heom_status launch_stage(heom_ctx* ctx, double dt, int stage) {
+  RhsParams p = base_params(ctx);
+  p.rhs_only = 0;
+  const bool taylor_large = ctx->use_large && ctx->rk4_form != 0;
+  const bool taylor_pipe = !taylor_large && ctx->use_hpipe && ctx->rk4_form != 0;
+  p.x = stage == 0 ? ctx->y : (stage == 2 ? ctx->xb : ctx->xa);
+  p.out_x = stage == 3 ? nullptr : (stage == 1 ? ctx->xb : ctx->xa);
+  p.acc_in = stage == 0 ? ctx->y : ctx->acc;
+  if (taylor_large) {
+    /* acc = y + v1 is stored, v2..v4 are added to it by global reductions; y and acc then swap roles */
+    p.taylor = 1; p.y = nullptr; p.out_acc = ctx->acc;
+    p.acc_red = stage == 0 ? 0 : ctx->acc_red;
+    p.ax = p.bx = dt / (double)(stage + 1);
+    heom_status s = launch_rhs(ctx, p);
+    if (s != HEOM_OK) return s;
+    if (stage == 3) { double2* tmp = ctx->y; ctx->y = ctx->acc; ctx->acc = tmp; }
+    return HEOM_OK;
+  }
+  p.y = ctx->y;
+  p.out_acc = stage == 3 ? ctx->y : ctx->acc;
+  if (taylor_pipe) {
+    p.taylor = 1;
+    p.ax = p.bx = dt / (double)(stage + 1);
+  } else {
+    p.ax = stage == 2 ? dt : dt / 2.0;
+    p.bx = (stage == 0 || stage == 3) ? dt / 6.0 : dt / 3.0;
+  }
+  return launch_rhs(ctx, p);
+}
+
 }  // namespace
 
 extern "C" {
 
-heom_status heom_create_sites(heom_ctx** out, int n_states, const double* H_cm, int n_baths, const int* bath_state,
-                              const double* lambda_cm, const double* nu_per_fs, double T_kelvin, int K, int D,
-                              int device) {
+static heom_status create_impl(heom_ctx** out, int n_states, const double* H_cm, int n_baths, const int* bath_state,
+                               const double* lambda_cm, const double* nu_per_fs, double T_kelvin, int K, int D,
+                               int device, int rank, int world) {
   if (!out) return HEOM_EINVAL;
   *out = nullptr;
+  if (world < 0 || (world > 0 && (rank < 0 || rank >= world))) return HEOM_EINVAL;
   if (!H_cm || !lambda_cm || !nu_per_fs || !bath_state || n_states < 1 || n_baths < 1 || n_baths > n_states ||
       K < 0 || D < 0 || D > 255 || device < 0)
     return HEOM_EINVAL;
@@ -285,6 +332,8 @@ heom_status heom_create_sites(heom_ctx** out, int n_states, const double* H_cm, 
   heom_ctx* c = new (std::nothrow) heom_ctx();
   if (!c) return HEOM_ENOMEM;
   c->device = device;
+  c->partitioned = world > 0;
+  c->part_rank = rank; c->part_world = world > 0 ? world : 1;
   c->B = n_baths;
   c->site.assign(bath_state, bath_state + n_baths);
   c->bath_of = bath_of;
@@ -305,6 +354,32 @@ heom_status heom_create_sites(heom_ctx** out, int n_states, const double* H_cm, 
     return oom ? HEOM_ENOMEM : HEOM_EINVAL;
   }
   *out = c;
+  return HEOM_OK;
+}
+
+heom_status heom_create_sites(heom_ctx** out, int n_states, const double* H_cm, int n_baths, const int* bath_state,
+                              const double* lambda_cm, const double* nu_per_fs, double T_kelvin, int K, int D,
+                              int device) {
+  return create_impl(out, n_states, H_cm, n_baths, bath_state, lambda_cm, nu_per_fs, T_kelvin, K, D, device, 0, 0);
+}
+
+heom_status heom_create_partition(heom_ctx** out, int n_states, const double* H_cm, int n_baths, const int* bath_state,
+                                  const double* lambda_cm, const double* nu_per_fs, double T_kelvin, int K, int D,
+                                  int device, int rank, int world) {
+  if (world < 1) return HEOM_EINVAL;
+  return create_impl(out, n_states, H_cm, n_baths, bath_state, lambda_cm, nu_per_fs, T_kelvin, K, D, device, rank, world);
+}
+
+int64_t heom_partition_owned(const heom_ctx* c) { return !c ? -1 : (c->partitioned ? c->part.n_owned : c->h.nodes); }
+
+heom_status heom_partition_plan(const heom_ctx* c, int64_t* global_ids, int64_t* send_counts, int64_t* recv_counts,
+                                int32_t* send_idx) {
+  if (!c || !c->partitioned) return HEOM_EINVAL;
+  const Partition& q = c->part;
+  if (global_ids) std::memcpy(global_ids, q.global_id.data(), q.global_id.size() * 8);
+  if (send_counts) std::memcpy(send_counts, q.send_counts.data(), q.send_counts.size() * 8);
+  if (recv_counts) std::memcpy(recv_counts, q.recv_counts.data(), q.recv_counts.size() * 8);
+  if (send_idx && !q.send_idx.empty()) std::memcpy(send_idx, q.send_idx.data(), q.send_idx.size() * 4);
   return HEOM_OK;
 }
 
@@ -361,6 +436,7 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
   }
   if (s == "order") {
     if (value != 0 && value != 1) return fail(ctx, HEOM_EINVAL, "order must be 0 or 1");
+    if (ctx->partitioned) return fail(ctx, HEOM_EINVAL, "a partition keeps its own node order");
     ctx->order = value;
     return HEOM_OK;
   }
@@ -446,11 +522,14 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->lrowH = herm_links_row(ctx->h.N, ctx->h.M);
   ctx->use_herm = ctx->kernel >= 1 && herm_supported(ctx->h.N, Wd, ctx->h.D);
   ctx->use_large = ctx->kernel == 1 && large_supported(ctx->h.N, Wd);
-  ctx->use_tiny = ctx->kernel == 1 && tiny_supported(ctx->h.N, Wd, ctx->h.D, (long long)ctx->h.nodes);
+  ctx->use_tiny = ctx->kernel == 1 && !ctx->partitioned && tiny_supported(ctx->h.N, Wd, ctx->h.D, (long long)ctx->h.nodes);
   ctx->d_Hs = (double*)(base + L.off_Hs);
   ctx->d_delta = (double*)(base + L.off_delta);
   ctx->d_A = (double2*)(base + L.off_A);
   ctx->d_S0 = (double2*)(base + L.off_S0);
+  ctx->d_send = (int32_t*)(base + L.off_send);
+  if (!ctx->part.send_idx.empty())
+    CU(cudaMemcpy(ctx->d_send, ctx->part.send_idx.data(), ctx->part.send_idx.size() * 4, cudaMemcpyHostToDevice));
   ctx->ket_col = -1;
   ctx->d_lptr = (int64_t*)(base + L.off_lptr);
   ctx->d_lent = (void*)(base + L.off_lent);
@@ -587,7 +666,7 @@ heom_status heom_set_state(heom_ctx* ctx, const double* sigma0) {
     ctx->state_hermitian = herm;
   }
   ctx->ket_col = -1;
-  if (ctx->ket_opt && ctx->use_hpipe && !ctx->use_tiny && ket_supported(ctx->h.N, dev_modes(ctx), ctx->h.D)) {
+  if (ctx->ket_opt && ctx->use_hpipe && !ctx->use_tiny && !ctx->partitioned && ket_supported(ctx->h.N, dev_modes(ctx), ctx->h.D)) {
     // column-sparse state?  exactly one non-zero column c, state c without a bath and uncoupled in H
     const int N = ctx->h.N;
     int col = -1, ncols = 0;
@@ -618,8 +697,9 @@ heom_status heom_set_state(heom_ctx* ctx, const double* sigma0) {
   }
   std::memcpy(ctx->h_pinned, sigma0, NN * 16);
   CU(cudaMemsetAsync(ctx->y, 0, ctx->state_bytes, ctx->stream));
-  CU(cudaMemcpyAsync(ctx->y + (size_t)ctx->h.slot_of[0] * ctx->stride, ctx->h_pinned, NN * 16,
-                     cudaMemcpyHostToDevice, ctx->stream));
+  if (root_slot(ctx) >= 0)   // a partition sets its copy of sigma_0 (owned or ghost) if it holds one
+    CU(cudaMemcpyAsync(ctx->y + (size_t)root_slot(ctx) * ctx->stride, ctx->h_pinned, NN * 16,
+                       cudaMemcpyHostToDevice, ctx->stream));
   ctx->have_state = true;
   return HEOM_OK;
 }
@@ -732,58 +812,39 @@ heom_status heom_rk4_steps(heom_ctx* ctx, double dt, int nsteps) {
     return HEOM_OK;
   }
   if (nsteps == 0) return HEOM_OK;
-  if (ctx->use_large && ctx->rk4_form != 0) {
-    /* Taylor/Horner form (R6): v1 = dt f(y), v_s = (dt/s) f(v_{s-1}), y' = y + v1 + v2 + v3 + v4 -- the
-     * classical RK4 result for a linear autonomous f, regrouped.  acc = y + v1 is stored, v2..v4 are
-     * added to it by global reductions; y and acc then swap roles.  14 instead of 16 state sizes. */
-    for (int step = 0; step < nsteps; ++step) {
-      heom_status s;
-      p.taylor = 1;
-      p.x = ctx->y; p.y = nullptr; p.acc_in = ctx->y; p.out_x = ctx->xa; p.out_acc = ctx->acc;
-      p.ax = dt; p.bx = dt; p.acc_red = 0;
-      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-      p.acc_red = ctx->acc_red; p.acc_in = ctx->acc;
-      p.x = ctx->xa; p.out_x = ctx->xb; p.ax = p.bx = dt / 2.0;
-      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-      p.x = ctx->xb; p.out_x = ctx->xa; p.ax = p.bx = dt / 3.0;
-      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-      p.x = ctx->xa; p.out_x = nullptr; p.ax = p.bx = dt / 4.0;
-      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-      double2* tmp = ctx->y; ctx->y = ctx->acc; ctx->acc = tmp;
+  if (ctx->partitioned && ctx->part_world > 1)
+    return fail(ctx, HEOM_ESTATE, "a partition advances stage by stage (heom_rk4_stage + halo exchange)");
+  for (int step = 0; step < nsteps; ++step)
+    for (int stage = 0; stage < 4; ++stage) {
+      heom_status s = launch_stage(ctx, dt, stage);
+      if (s != HEOM_OK) return s;
     }
-    return HEOM_OK;
-  }
-  if (ctx->use_hpipe && ctx->rk4_form != 0) {
-    /* The same Taylor/Horner form for the pipelined small-N kernel: the stages never read y, the
-     * running sum is updated in shared memory: 14 instead of 16 state sizes per step. */
-    p.taylor = 1;
-    for (int step = 0; step < nsteps; ++step) {
-      heom_status s;
-      p.x = ctx->y; p.y = ctx->y; p.acc_in = ctx->y; p.out_x = ctx->xa; p.out_acc = ctx->acc;
-      p.ax = dt; p.bx = dt;                                   /* xa = v1 = dt k;  acc = y + v1 */
-      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-      p.x = ctx->xa; p.acc_in = ctx->acc; p.out_x = ctx->xb; p.ax = p.bx = dt / 2.0;
-      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;      /* xb = v2;  acc += v2 */
-      p.x = ctx->xb; p.out_x = ctx->xa; p.ax = p.bx = dt / 3.0;
-      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;      /* xa = v3;  acc += v3 */
-      p.x = ctx->xa; p.out_x = nullptr; p.out_acc = ctx->y; p.bx = dt / 4.0;
-      if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;      /* y = acc + v4 */
-    }
-    return HEOM_OK;
-  }
-  for (int step = 0; step < nsteps; ++step) {
-    heom_status s;
-    p.x = ctx->y; p.y = ctx->y; p.acc_in = ctx->y; p.out_x = ctx->xa; p.out_acc = ctx->acc;
-    p.ax = dt / 2.0; p.bx = dt / 6.0;
-    if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-    p.x = ctx->xa; p.acc_in = ctx->acc; p.out_x = ctx->xb; p.out_acc = ctx->acc;
-    p.ax = dt / 2.0; p.bx = dt / 3.0;
-    if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-    p.x = ctx->xb; p.out_x = ctx->xa; p.ax = dt; p.bx = dt / 3.0;
-    if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-    p.x = ctx->xa; p.out_x = nullptr; p.out_acc = ctx->y; p.bx = dt / 6.0;
-    if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-  }
+  return HEOM_OK;
+}
+
+heom_status heom_rk4_stage(heom_ctx* ctx, double dt, int stage) {
+  if (!ctx || stage < 0 || stage > 3 || !std::isfinite(dt)) return HEOM_EINVAL;
+  if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
+  if (ctx->ket_col >= 0 || ctx->use_tiny)
+    return fail(ctx, HEOM_ESTATE, "stage-wise stepping is for the matrix kernels (set options ket=0, kernel=2)");
+  return launch_stage(ctx, dt, stage);
+}
+
+heom_status heom_stage_output(heom_ctx* ctx, int stage, void** dev_ptr) {
+  if (!ctx || !dev_ptr || stage < 0 || stage > 3) return HEOM_EINVAL;
+  if (!ctx->bound) return fail(ctx, HEOM_ESTATE, "no workspace bound");
+  *dev_ptr = (stage == 3) ? ctx->y : (stage == 1 ? ctx->xb : ctx->xa);
+  return HEOM_OK;
+}
+
+heom_status heom_pack_halo(heom_ctx* ctx, const void* src_dev, void* dst_dev) {
+  if (!ctx || !src_dev || !dst_dev) return HEOM_EINVAL;
+  if (!ctx->bound || !ctx->partitioned) return fail(ctx, HEOM_ESTATE, "not a bound partition");
+  const long long rows = (long long)ctx->part.send_idx.size();
+  if (rows == 0) return HEOM_OK;
+  CU(launch_pack_rows((const double2*)src_dev, (double2*)dst_dev, ctx->d_send, rows, ctx->h.N * ctx->h.N, ctx->stride,
+                      ctx->stream));
+  ctx->launches += 1;
   return HEOM_OK;
 }
 

@@ -3,6 +3,7 @@
 
 #include <cmath>
 #include <limits>
+#include <utility>
 
 namespace heom {
 namespace {
@@ -124,6 +125,86 @@ bool build_hierarchy(int N, int K, int D, int order, Hierarchy& h, std::string& 
     }
   }
   for (int64_t u = 0; u < nodes; ++u) h.node_at[(size_t)h.slot_of[(size_t)u]] = (int32_t)u;
+  return true;
+}
+
+bool restrict_hierarchy(Hierarchy& h, int rank, int world, Partition& part, std::string& err) {
+  if (world < 1 || rank < 0 || rank >= world) { err = "invalid rank/world"; return false; }
+  const int64_t nodes = h.nodes;
+  const int W = h.W;
+  if (world > nodes) { err = "more ranks than nodes"; return false; }
+  std::vector<int64_t> lo((size_t)world + 1);
+  for (int r = 0; r <= world; ++r) lo[(size_t)r] = nodes * r / world;
+  auto owner_of = [&](int64_t slot) {
+    int a = 0, b = world;                       // largest r with lo[r] <= slot
+    while (b - a > 1) { const int m = (a + b) / 2; if (lo[(size_t)m] <= slot) a = m; else b = m; }
+    return a;
+  };
+  const int64_t s0 = lo[(size_t)rank], s1 = lo[(size_t)rank + 1], n_owned = s1 - s0;
+  // ghosts (by global slot) and, by the symmetry of the link graph (u -> a by +e_l iff a -> u by -e_l), the owned
+  // nodes every peer needs: those with a neighbour in the peer's range
+  std::vector<uint8_t> is_ghost((size_t)nodes, 0);
+  std::vector<std::vector<int32_t>> send((size_t)world);
+  for (int64_t s = s0; s < s1; ++s) {
+    const int64_t u = h.node_at[(size_t)s];
+    int last_peer = -1;
+    std::vector<int> peers;
+    for (int l = 0; l < W; ++l)
+      for (int dir = 0; dir < 2; ++dir) {
+        const int32_t v = dir ? h.minus[(size_t)u * W + l] : h.plus[(size_t)u * W + l];
+        if (v < 0) continue;
+        const int64_t t = h.slot_of[(size_t)v];
+        if (t >= s0 && t < s1) continue;
+        is_ghost[(size_t)t] = 1;
+        const int p = owner_of(t);
+        if (p != last_peer) {
+          bool seen = false;
+          for (int q : peers) seen = seen || q == p;
+          if (!seen) peers.push_back(p);
+          last_peer = p;
+        }
+      }
+    for (int p : peers) send[(size_t)p].push_back((int32_t)(s - s0));
+  }
+  std::vector<int64_t> ghost_slots;
+  for (int64_t t = 0; t < nodes; ++t) if (is_ghost[(size_t)t]) ghost_slots.push_back(t);
+  const int64_t n_ghost = (int64_t)ghost_slots.size(), n_local = n_owned + n_ghost;
+  if (n_local > 2147483647LL) { err = "partition too large"; return false; }
+  std::vector<int32_t> local_of((size_t)nodes, -1);     // global slot -> local index
+  for (int64_t s = s0; s < s1; ++s) local_of[(size_t)s] = (int32_t)(s - s0);
+  for (int64_t q = 0; q < n_ghost; ++q) local_of[(size_t)ghost_slots[(size_t)q]] = (int32_t)(n_owned + q);
+
+  part.rank = rank; part.world = world; part.n_owned = n_owned; part.n_ghost = n_ghost;
+  part.global_id.assign((size_t)n_local, 0);
+  part.send_counts.assign((size_t)world, 0); part.recv_counts.assign((size_t)world, 0);
+  part.send_idx.clear();
+  for (int p = 0; p < world; ++p) {
+    part.send_counts[(size_t)p] = (int64_t)send[(size_t)p].size();
+    part.send_idx.insert(part.send_idx.end(), send[(size_t)p].begin(), send[(size_t)p].end());
+  }
+  for (int64_t q = 0; q < n_ghost; ++q) part.recv_counts[(size_t)owner_of(ghost_slots[(size_t)q])] += 1;
+
+  Hierarchy loc;
+  loc.N = h.N; loc.K = h.K; loc.M = h.M; loc.W = W; loc.D = h.D; loc.nodes = n_local;
+  loc.tuples.assign((size_t)n_local * W, 0);
+  loc.plus.assign((size_t)n_local * W, -1);
+  loc.minus.assign((size_t)n_local * W, -1);
+  loc.slot_of.resize((size_t)n_local); loc.node_at.resize((size_t)n_local);
+  for (int64_t i = 0; i < n_local; ++i) {
+    const int64_t slot = i < n_owned ? s0 + i : ghost_slots[(size_t)(i - n_owned)];
+    const int64_t u = h.node_at[(size_t)slot];
+    part.global_id[(size_t)i] = u;
+    loc.slot_of[(size_t)i] = (int32_t)i; loc.node_at[(size_t)i] = (int32_t)i;
+    for (int l = 0; l < W; ++l) {
+      loc.tuples[(size_t)i * W + l] = h.tuples[(size_t)u * W + l];
+      if (i >= n_owned) continue;                   // ghost rows: copies only, no links
+      const int32_t a = h.plus[(size_t)u * W + l], b = h.minus[(size_t)u * W + l];
+      loc.plus[(size_t)i * W + l] = a < 0 ? -1 : local_of[(size_t)h.slot_of[(size_t)a]];
+      loc.minus[(size_t)i * W + l] = b < 0 ? -1 : local_of[(size_t)h.slot_of[(size_t)b]];
+    }
+  }
+  part.root = local_of[(size_t)h.slot_of[0]];
+  h = std::move(loc);
   return true;
 }
 

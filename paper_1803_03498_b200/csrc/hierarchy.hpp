@@ -27,6 +27,25 @@ struct Hierarchy {
   std::vector<int32_t> node_at;  // [nodes]
 };
 
+// One rank's part of a hierarchy split over `world` ranks (the paper's partitions + halo regions,
+// P:501): the rank owns a contiguous range of the lexicographic storage order; its ghosts are the neighbours of
+// owned nodes that live elsewhere.  Local node order: owned nodes by global lexicographic slot, then ghosts by
+// global slot (hence grouped by owning rank, in the order the owner sends them).
+struct Partition {
+  int rank = 0, world = 1;
+  int64_t n_owned = 0, n_ghost = 0;
+  std::vector<int64_t> global_id;    // [n_owned + n_ghost] pinned-order id of each local node
+  std::vector<int64_t> send_counts;  // [world] owned nodes peer p needs
+  std::vector<int64_t> recv_counts;  // [world] ghosts owned by peer p (contiguous in the ghost region)
+  std::vector<int32_t> send_idx;     // [sum send_counts] local indices, grouped by peer, ascending
+  int64_t root = -1;                 // local index of the hierarchy's root node (n = 0), -1 if not local
+};
+
+// Replaces `h` (a full hierarchy built with order = 1) by the rank's local hierarchy: tuples and link tables of the
+// n_owned + n_ghost local nodes with local indices (ghost rows: every link invalid; they are never the result of
+// a computation, only copies), slot_of = node_at = identity.
+bool restrict_hierarchy(Hierarchy& h, int rank, int world, Partition& part, std::string& err);
+
 struct Coefficients {
   double beta_hbar = 0;            // fs
   std::vector<double> gamma;       // [W]   Eq. 19

@@ -105,6 +105,10 @@ cudaError_t launch_rhs_ket(const RhsParams& p, const int32_t* links, int lrow, i
 // dst[slot][i][j] = (j == col) ? ket[slot][i] : 0   (full matrices for the host-visible getters)
 cudaError_t launch_ket_expand(const double2* ket, double2* dst, long long nodes, int N, int col, cudaStream_t s);
 
+// dst[q][0..NN) = src[idx[q]*stride + 0..NN): the send buffer of a halo exchange
+cudaError_t launch_pack_rows(const double2* src, double2* dst, const int32_t* idx, long long rows, int NN, int stride,
+                             cudaStream_t s);
+
 // out[0], out[1] = Tr(A sigma_0) (re, im); A: DEVICE [N][N] complex128
 cudaError_t launch_expectation(const double2* node0, const double2* A, int N, double* out, cudaStream_t s);
 

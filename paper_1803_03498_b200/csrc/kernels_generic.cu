@@ -153,6 +153,17 @@ __global__ void populations_kernel(const double2* __restrict__ node0, int N, dou
   if (threadIdx.x == 0) { out[N] = tr; out[N + 1] = ti; }
 }
 
+// halo send buffer: dst[q][e] = src[idx[q]][e], one node (NN complex elements) per row
+__global__ void pack_rows_kernel(const double2* __restrict__ src, double2* __restrict__ dst,
+                                 const int32_t* __restrict__ idx, long long rows, int NN, int stride) {
+  const long long total = rows * NN;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+    const long long q = t / NN;
+    const int e = (int)(t - q * NN);
+    dst[t] = src[(size_t)idx[q] * stride + e];
+  }
+}
+
 // Tr(A sigma_0) = sum_ij A[i][j] sigma_0[j][i] (the dipole correlation function of Eq. 56); one warp, fixed order
 __global__ void expectation_kernel(const double2* __restrict__ node0, const double2* __restrict__ A, int N,
                                    double* __restrict__ out) {
@@ -209,6 +220,15 @@ cudaError_t launch_permute(const double2* src, double2* dst, const int32_t* slot
 
 cudaError_t launch_populations(const double2* node0, int N, double* out, cudaStream_t s) {
   populations_kernel<<<1, 32, 0, s>>>(node0, N, out);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_pack_rows(const double2* src, double2* dst, const int32_t* idx, long long rows, int NN, int stride,
+                             cudaStream_t s) {
+  long long blocks = (rows * NN + 255) / 256;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  if (blocks < 1) blocks = 1;
+  pack_rows_kernel<<<(int)blocks, 256, 0, s>>>(src, dst, idx, rows, NN, stride);
   return cudaGetLastError();
 }
 

@@ -1,0 +1,101 @@
+"""One hierarchy sharded over several GPUs: one process per GPU, halo exchange over NCCL.
+
+The paper partitions the ADO graph into self-contained parts plus halo regions and exchanges the halos every
+right-hand-side evaluation.  Here rank r owns a contiguous range of the lexicographic node order
+(heom_create_partition); after every fused RHS + RK4-stage launch the rows other ranks hold as ghosts are packed by
+a device kernel (heom_pack_halo) and sent with ONE all_to_all_single, received straight into the ghost rows of the
+buffer the next stage reads (the local node order makes the ghost region the receive buffer: no unpack).
+4 exchanges per RK4 step.  torch.distributed is plumbing only; every arithmetic step runs in the library's kernels.
+"""
+import numpy as np
+
+from .binding import Heom
+
+
+def halo_all_to_all(buf, send, n_owned, send_counts, recv_counts, group=None):
+    """rows of `send` (grouped by destination rank) -> the ghost rows buf[n_owned:] of the peers (grouped by
+    source rank): one all_to_all_single, received in place."""
+    import torch.distributed as dist
+    n_send = int(np.sum(send_counts))
+    dist.all_to_all_single(buf[n_owned:], send[:n_send],
+                           output_split_sizes=[int(c) for c in recv_counts],
+                           input_split_sizes=[int(c) for c in send_counts], group=group)
+
+
+class ShardedHeom:
+    """Rank `rank` of `world`: a partition context + the exchange.  group=None: the default process group."""
+
+    def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, rank, world, device=0, bath_state=None,
+                 group=None, **options):
+        self.rank, self.world, self.group = int(rank), int(world), group
+        self.g = Heom(H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, device=device, bath_state=bath_state,
+                      partition=(rank, world), **options)
+        self.n_owned = self.g.owned()
+        self.global_ids, self.send_counts, self.recv_counts, self.send_idx = self.g.partition_plan()
+        self._send = None
+
+    def bind(self, stream=None):
+        import torch
+        self.g.bind(stream=stream)
+        rows = max(1, int(self.send_counts.sum()))
+        self._send = torch.empty((rows, 2 * self.g.N * self.g.N), dtype=torch.float64,
+                                 device=self.g._workspace.device)
+        return self
+
+    # -- state ----------------------------------------------------------------------------------
+    def set_state(self, sigma0):
+        self.g.set_state(sigma0)
+
+    def owned_state(self):
+        """(global pinned-order ids, states) of the nodes this rank owns."""
+        full = self.g.get_full_state()
+        return self.global_ids[:self.n_owned], full[:self.n_owned]
+
+    def gather_state(self, total_nodes):
+        """The whole state in the pinned order on every rank (small cases / tests): all_gather of the owned parts."""
+        import torch.distributed as dist
+        ids, st = self.owned_state()
+        parts = [None] * self.world
+        dist.all_gather_object(parts, (ids, st), group=self.group)
+        out = np.empty((total_nodes, self.g.N, self.g.N), dtype=np.complex128)
+        for i, s in parts:
+            out[i] = s
+        return out
+
+    # -- propagation ----------------------------------------------------------------------------
+    def exchange(self, stage):
+        """Refresh the ghost rows of the buffer the next stage reads."""
+        ptr = self.g.stage_output(stage)
+        buf = self.g.buffer_view(ptr)
+        if int(self.send_counts.sum()):
+            self.g.pack_halo(ptr, self._send.data_ptr())
+        halo_all_to_all(buf, self._send, self.n_owned, self.send_counts, self.recv_counts, self.group)
+
+    def rk4_steps(self, dt_fs, nsteps):
+        for _ in range(int(nsteps)):
+            for stage in range(4):
+                self.g.rk4_stage(dt_fs, stage)
+                if self.world > 1:
+                    self.exchange(stage)
+
+    def populations(self):
+        """Eq. 26 on the rank that owns sigma_0 (rank 0: the root is the first node of the order)."""
+        return self.g.populations()
+
+
+def exchange_plan_check(plans):
+    """Host-side consistency of the plans of all ranks (tests): what rank p sends to r is, node for node, what r
+    expects from p.  plans[r] = (global_ids, n_owned, send_counts, recv_counts, send_idx)."""
+    world = len(plans)
+    for r in range(world):
+        gid_r, own_r, sc_r, rc_r, idx_r = plans[r]
+        goff = own_r
+        for p in range(world):
+            gid_p, own_p, sc_p, rc_p, idx_p = plans[p]
+            soff = int(sc_p[:r].sum())
+            sent = gid_p[idx_p[soff:soff + int(sc_p[r])]]
+            want = gid_r[goff:goff + int(rc_r[p])]
+            if sent.shape != want.shape or not np.array_equal(sent, want):
+                return False
+            goff += int(rc_r[p])
+    return True
