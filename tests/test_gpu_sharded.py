@@ -1,0 +1,118 @@
+"""-m gpu: the sharded path (heom_create_partition + stage-wise stepping + halo exchange) on ONE GPU.
+
+The `world` partition contexts live in one process and are advanced one after the other, stage by stage; the
+exchange between them is the same pack kernel (heom_pack_halo) followed by device copies of exactly the rows
+halo_all_to_all would move (no rank waits on another inside a kernel).  The union of the owned rows is compared
+with the oracle's global state."""
+import numpy as np
+import pytest
+import torch
+
+import workloads
+from oracle.oracle import Oracle
+
+pytestmark = pytest.mark.gpu
+STATE_TOL = 1e-10
+RHS_TOL = 1e-13
+
+
+def rel_err(a, b):
+    return np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300)
+
+
+class LocalWorld:
+    def __init__(self, w, world, bath_state=None, **opts):
+        from paper_1803_03498_b200 import Heom
+        self.world = world
+        self.parts = [Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, partition=(r, world),
+                           bath_state=bath_state, **opts).bind() for r in range(world)]
+        self.plans = [g.partition_plan() for g in self.parts]
+        self.send = [torch.empty((max(1, int(p[1].sum())), 2 * g.N * g.N), dtype=torch.float64, device="cuda")
+                     for g, p in zip(self.parts, self.plans)]
+
+    def exchange(self, ptrs):
+        for g, s, p in zip(self.parts, self.send, ptrs):
+            if g.partition_plan()[1].sum():
+                g.pack_halo(p, s.data_ptr())
+        torch.cuda.synchronize()
+        for r, g in enumerate(self.parts):
+            buf = g.buffer_view(ptrs[r])
+            goff = g.owned()
+            for p in range(self.world):
+                n = int(self.plans[r][2][p])                      # recv_counts[p]
+                soff = int(self.plans[p][1][:r].sum())            # where p's rows for r start in p's send buffer
+                assert n == int(self.plans[p][1][r])
+                buf[goff:goff + n] = self.send[p][soff:soff + n]
+                goff += n
+        torch.cuda.synchronize()
+
+    def set_state(self, s0):
+        for g in self.parts:
+            g.set_state(s0)
+
+    def set_full_state(self, st):
+        for g, p in zip(self.parts, self.plans):
+            g.set_full_state(st[p[0]])
+
+    def rk4_steps(self, dt, n):
+        for _ in range(n):
+            for stage in range(4):
+                for g in self.parts:
+                    g.rk4_stage(dt, stage)
+                self.exchange([g.stage_output(stage) for g in self.parts])
+
+    def gather(self, getter, total):
+        out = None
+        for g, p in zip(self.parts, self.plans):
+            loc = getter(g)
+            if out is None:
+                out = np.empty((total,) + loc.shape[1:], dtype=loc.dtype)
+            out[p[0][:g.owned()]] = loc[:g.owned()]
+        return out
+
+
+@pytest.mark.parametrize("name,D,steps,world", [("cfg2", 4, 100, 2), ("cfg2", 4, 60, 5), ("cfg3", 5, 60, 3),
+                                                ("cfg4", 3, 60, 4), ("cfg5", 1, 20, 2), ("cfg5", 2, 6, 3),
+                                                ("cfg1", 4, 200, 3)])
+@pytest.mark.parametrize("herm,form", [(1, -1), (0, -1), (1, 0)])
+def test_sharded_rk4_parity(name, D, steps, world, herm, form):
+    w = workloads.get(name).with_(D=D)
+    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D)
+    lw = LocalWorld(w, world, hermitian=herm, rk4_form=form)
+    assert sum(g.owned() for g in lw.parts) == o.nodes
+    # a single right-hand side on a dense random state first (ghost rows of the result are not meaningful)
+    st = workloads.random_state(o.nodes, w.N, seed=5)
+    o.set_full_state(st); lw.set_full_state(st)
+    assert rel_err(lw.gather(lambda g: g.rhs(), o.nodes), o.rhs()) < RHS_TOL
+    o.set_state(w.sigma0()); lw.set_state(w.sigma0())
+    o.rk4_steps(w.dt_fs, steps); lw.rk4_steps(w.dt_fs, steps)
+    ref = o.get_full_state()
+    got = lw.gather(lambda g: g.get_full_state(), o.nodes)
+    assert rel_err(got, ref) < STATE_TOL
+    pop, tr = lw.parts[0].populations()                             # rank 0 owns sigma_0
+    assert abs(tr - 1.0) < 1e-11 and np.allclose(pop, np.diag(ref[0]).real, atol=1e-11)
+    # ghost copies agree with their owners' rows after the last exchange
+    for g, p in zip(lw.parts, lw.plans):
+        loc = g.get_full_state()
+        assert rel_err(loc, ref[p[0]]) < STATE_TOL
+
+
+def test_sharded_world_1_equals_plain():
+    from paper_1803_03498_b200 import Heom
+    w = workloads.fmo_like().with_(D=3)
+    a = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D).bind()
+    b = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, partition=(0, 1)).bind()
+    a.set_state(w.sigma0()); b.set_state(w.sigma0())
+    a.rk4_steps(1.0, 50); b.rk4_steps(1.0, 50)                     # world 1: rk4_steps is allowed
+    gid = b.partition_plan()[0]
+    assert np.array_equal(b.get_full_state(), a.get_full_state()[gid])
+
+
+def test_partition_refuses_unsplit_stepping():
+    from paper_1803_03498_b200 import Heom, HeomError
+    w = workloads.dimer()
+    g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, partition=(1, 2)).bind()
+    g.set_state(w.sigma0())
+    with pytest.raises(HeomError) as e:
+        g.rk4_steps(1.0, 1)
+    assert e.value.status == -4
