@@ -145,7 +145,7 @@ def run_reference(args, w):
     print(json.dumps(line))
 
 
-def config_dict(w, n_gpus):
+def config_dict(w, n_gpus, shard=False):
     origin = (f"BASELINE.json configs[{list(workloads.CONFIGS).index(w.name[:4])}]" if w.name[:4] in workloads.CONFIGS
               else "linear-absorption variant of configs[1] (ground state + 7 sites, sigma_0(0) = mu_z|0><0|; not a BASELINE config)")
     return {"workload": f"{w.name}: {origin} "
@@ -153,7 +153,9 @@ def config_dict(w, n_gpus):
             "state_mb": round(w.state_bytes / 1e6, 1),
             "l2_policy": "state buffers (4 x %.0f MB) exceed the 126 MB L2; no flush needed" % (w.state_bytes / 1e6)
             if w.state_bytes > 130e6 else "state smaller than L2: L2 flushed by a 256 MB write between timed chunks",
-            "parallelism": "single GPU" if n_gpus == 1 else f"{n_gpus} independent replicas (P:507), no collective",
+            "parallelism": (f"one hierarchy sharded over {n_gpus} rank(s), halo all_to_all per stage (P:501)" if shard
+                            else "single GPU" if n_gpus == 1
+                            else f"{n_gpus} independent replicas (P:507), no collective"),
             "seed": workloads.SEED_FMO}
 
 
@@ -165,6 +167,9 @@ def main():
     ap.add_argument("--config", default="cfg2", choices=list(workloads.CONFIGS) + list(workloads.EXTRA))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "shard"],
+                    help="N > 1: independent replicas (default, weak scaling) or ONE hierarchy sharded over the "
+                         "ranks with a halo exchange per stage (strong scaling; paper_1803_03498_b200/sharded.py)")
     ap.add_argument("--option", action="append", default=[], help="name=value library option")
     args = ap.parse_args()
     w = workloads.get(args.config)
@@ -188,17 +193,25 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     opts = dict(kv.split("=") for kv in args.option)
     stream = torch.cuda.Stream(device=local_rank)
-    g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, device=local_rank, bath_state=w.bath_state,
-             **{k: int(v) for k, v in opts.items()})
+    shard = args.parallel == "shard"
+    if shard:
+        from paper_1803_03498_b200.sharded import ShardedHeom
+        g = ShardedHeom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, rank, world, device=local_rank,
+                        bath_state=w.bath_state, **{k: int(v) for k, v in opts.items()})
+    else:
+        g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, device=local_rank, bath_state=w.bath_state,
+                 **{k: int(v) for k, v in opts.items()})
     g.bind(stream=stream)
-    sigma0 = replicas.replica_sigma0(w, rank) if w.sigma0_matrix is None else w.sigma0()
+    sigma0 = replicas.replica_sigma0(w, rank) if (w.sigma0_matrix is None and not shard) else w.sigma0()
+    job = 1 if shard else world          # whole-job units: one hierarchy (shard) or one per rank (replicas)
     flush = None
     if w.state_bytes <= 130e6:
         flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=f"cuda:{local_rank}")
 
     # ---------------- kernel-resident timing: state already in HBM -----------------------
     g.set_state(sigma0)
-    g.rk4_steps(w.dt_fs, args.warmup)
+    with torch.cuda.stream(stream):
+        g.rk4_steps(w.dt_fs, args.warmup)
     g.sync()
     g.set_option("timing", 1)
     g.kernel_time()                      # reset the per-launch event list
@@ -229,9 +242,10 @@ def main():
     replicas.barrier(world); torch.cuda.synchronize()
     t0 = time.perf_counter()
     g.set_state(sigma0)
-    for _ in range(e_steps):
-        g.rk4_steps(w.dt_fs, 1)
-        pop_e, tr_e = g.populations()
+    with torch.cuda.stream(stream):
+        for _ in range(e_steps):
+            g.rk4_steps(w.dt_fs, 1)
+            pop_e, tr_e = g.populations()
     g.sync()
     e_dt = replicas.max_over_ranks(time.perf_counter() - t0, world)
     h2d = 16 * w.N * w.N / e_steps
@@ -239,9 +253,10 @@ def main():
 
     if rank == 0:
         peaks, which = measured_peaks()
-        value = 4.0 * w.nodes * args.steps * world / (ms * 1e-3)
-        alg_bytes_per_launch = 64.0 * w.N * w.N * w.nodes          # 16 S per step / 4 launches
-        alg_flops_per_launch = 8.0 * w.N ** 3 * w.nodes            # real H: 8 N^3 per node-update
+        value = 4.0 * w.nodes * args.steps * job / (ms * 1e-3)
+        launch_nodes = g.n_owned if shard else w.nodes             # shard: rank 0's owned nodes (ghost rows are overhead)
+        alg_bytes_per_launch = 64.0 * w.N * w.N * launch_nodes     # 16 S per step / 4 launches
+        alg_flops_per_launch = 8.0 * w.N ** 3 * launch_nodes       # real H: 8 N^3 per node-update
         avg_launch_s = (kern_ms / max(kern_n, 1)) * 1e-3
         kernel_name = g.kernel_name()
         ket_note = None
@@ -285,11 +300,11 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": config_dict(w, world),
-            "rk4_steps_per_s": args.steps * world / (ms * 1e-3),
+            "scaling": "strong" if shard else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(w, world, shard),
+            "rk4_steps_per_s": args.steps * job / (ms * 1e-3),
             "roofline": roof,
-            "e2e": {"value": 4.0 * w.nodes * e_steps * world / e_dt, "unit": UNIT,
+            "e2e": {"value": 4.0 * w.nodes * e_steps * job / e_dt, "unit": UNIT,
                     "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "what": "heom_set_state(HOST sigma_0) once, then per step heom_rk4_steps(dt,1) + "
                             "heom_populations -> HOST; host wall clock"},

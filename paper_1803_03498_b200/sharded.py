@@ -79,8 +79,19 @@ class ShardedHeom:
                     self.exchange(stage)
 
     def populations(self):
-        """Eq. 26 on the rank that owns sigma_0 (rank 0: the root is the first node of the order)."""
-        return self.g.populations()
+        """Eq. 26 from the rank's copy of sigma_0 (rank 0 owns it: the root is the first node of the order; ranks
+        that hold neither it nor a ghost of it return zeros)."""
+        from .binding import HeomError
+        try:
+            return self.g.populations()
+        except HeomError as e:
+            if e.status != -4:
+                raise
+            return np.zeros(self.g.N), 0j
+
+    def __getattr__(self, name):
+        # plumbing calls (sync, set_option, kernel_time, launch_count, kernel_name, ...) go to the partition context
+        return getattr(self.g, name)
 
 
 def exchange_plan_check(plans):
