@@ -172,14 +172,19 @@ class Heom:
     def workspace_bytes(self):
         return int(self._lib.heom_workspace_bytes(self._h))
 
-    def bind(self, stream=None):
-        """Allocate the workspace as a torch tensor on `device` and bind it (PyTorch = memory + stream)."""
+    def bind(self, stream=None, poison=False):
+        """Allocate the workspace as a torch tensor on `device` and bind it (PyTorch = memory + stream).
+        poison=True fills it with 0xFF bytes (NaNs, index -1) first, so that a read of memory the library never
+        wrote shows up in the results (tests)."""
         import torch
         if not torch.cuda.is_available():
             raise HeomError(HEOM_ECUDA, "no CUDA device: the HEOM path has no CPU fallback")
         dev = torch.device("cuda", self.device)
         nbytes = self.workspace_bytes()
         self._workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
+        if poison:
+            self._workspace.fill_(255)
+            torch.cuda.synchronize(dev)
         ptr = (self._workspace.data_ptr() + 255) // 256 * 256
         self._stream = stream if stream is not None else torch.cuda.current_stream(dev)
         self._ck(self._lib.heom_bind_workspace(self._h, ptr, nbytes, self._stream.cuda_stream))

@@ -206,7 +206,10 @@ Layout layout_of(const heom_ctx* c) {
 
 RhsParams base_params(const heom_ctx* c) {
   RhsParams p{};
-  p.N = c->h.N; p.M = c->h.M; p.W = dev_modes(c); p.D = c->h.D; p.nodes = (int)c->h.nodes;
+  p.N = c->h.N; p.M = c->h.M; p.W = dev_modes(c); p.D = c->h.D;
+  // a partition computes its OWNED rows only (the first n_owned local nodes); the ghost rows behind them are
+  // read by the gathers and written by the halo exchange, never by a kernel
+  p.nodes = c->partitioned ? (int)c->part.n_owned : (int)c->h.nodes;
   p.stride = c->stride;
   p.inv_hbar = 1.0 / kHbar;
   p.H = c->d_H; p.Tterm = c->d_T; p.damp = c->d_damp;

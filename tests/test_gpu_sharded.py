@@ -25,9 +25,9 @@ class LocalWorld:
         from paper_1803_03498_b200 import Heom
         self.world = world
         self.parts = [Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, partition=(r, world),
-                           bath_state=bath_state, **opts).bind() for r in range(world)]
+                           bath_state=bath_state, **opts).bind(poison=True) for r in range(world)]
         self.plans = [g.partition_plan() for g in self.parts]
-        self.send = [torch.empty((max(1, int(p[1].sum())), 2 * g.N * g.N), dtype=torch.float64, device="cuda")
+        self.send = [torch.full((max(1, int(p[1].sum())), 2 * g.N * g.N), float("nan"), dtype=torch.float64, device="cuda")
                      for g, p in zip(self.parts, self.plans)]
 
     def exchange(self, ptrs):
