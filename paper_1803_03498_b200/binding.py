@@ -27,6 +27,8 @@ SYMBOLS = [
 ]
 
 _lib = None
+import weakref  # noqa: E402
+POISONED = weakref.WeakSet()   # contexts bound with poison=True (the test suite checks their guard bytes)
 
 
 class HeomError(RuntimeError):
@@ -185,10 +187,22 @@ class Heom:
         if poison:
             self._workspace.fill_(255)
             torch.cuda.synchronize(dev)
+            POISONED.add(self)
         ptr = (self._workspace.data_ptr() + 255) // 256 * 256
         self._stream = stream if stream is not None else torch.cuda.current_stream(dev)
+        self._ws_end = ptr - self._workspace.data_ptr() + nbytes
         self._ck(self._lib.heom_bind_workspace(self._h, ptr, nbytes, self._stream.cuda_stream))
         return self
+
+    def workspace_guard_intact(self):
+        """After bind(poison=True): the slack bytes behind heom_workspace_bytes() still hold the poison pattern,
+        i.e. nothing wrote past the end of the workspace (tests)."""
+        import torch
+        if self._workspace is None:
+            return True
+        torch.cuda.synchronize(self._workspace.device)
+        tail = self._workspace[self._ws_end:]
+        return bool(tail.numel() > 0 and (tail == 255).all().item())
 
     def bind_raw(self, dev_ptr, nbytes, cuda_stream=0):
         self._ck(self._lib.heom_bind_workspace(self._h, dev_ptr, nbytes, cuda_stream))

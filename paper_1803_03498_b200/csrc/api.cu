@@ -194,11 +194,12 @@ Layout layout_of(const heom_ctx* c) {
   L.off_S0 = o; o += align_up(N * N * 16);
   L.off_send = o; o += align_up(c->part.send_idx.size() * 4 + 16);
   if (large_supported((int)N, (int)W)) {
-    // every valid link appears once as "+" and once as "-": count the "-" links of the host table
+    // CSR link list: one 16-byte entry per valid "+" and per valid "-" link (a partition's table has links for its
+    // owned rows only, so the two counts differ there)
     size_t links = 0;
-    for (size_t q = 0; q < c->h.minus.size(); ++q) links += c->h.minus[q] >= 0;
+    for (size_t q = 0; q < c->h.minus.size(); ++q) links += (c->h.minus[q] >= 0) + (c->h.plus[q] >= 0);
     L.off_lptr = o; o += align_up((nodes + 1) * 8);
-    L.off_lent = o; o += align_up(2 * links * 16 + 16);
+    L.off_lent = o; o += align_up(links * 16 + 16);
   }
   L.total = o;
   return L;

@@ -18,3 +18,14 @@ def oracle_lib():
     """Build (if stale) and load the CPU oracle."""
     from oracle import build_oracle
     return build_oracle.build()
+
+
+@pytest.fixture(autouse=True)
+def _workspace_guard(request):
+    """After every GPU test: no context bound with poison=True wrote past the end of its workspace."""
+    yield
+    if request.node.get_closest_marker("gpu") is None:
+        return
+    from paper_1803_03498_b200 import binding
+    for g in list(binding.POISONED):
+        assert g.workspace_guard_intact(), "a kernel or copy wrote past heom_workspace_bytes()"

@@ -23,7 +23,7 @@ STATE_TOL = 1e-10
 def _pair(w, **opts):
     from paper_1803_03498_b200 import Heom
     o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D)
-    g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, **opts).bind()
+    g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, **opts).bind(poison=w.state_bytes < 2e9)
     return o, g
 
 

@@ -95,6 +95,7 @@ def test_sharded_rk4_parity(name, D, steps, world, herm, form):
     for g, p in zip(lw.parts, lw.plans):
         loc = g.get_full_state()
         assert rel_err(loc, ref[p[0]]) < STATE_TOL
+        assert g.workspace_guard_intact()                           # nothing wrote past the workspace
 
 
 def test_sharded_world_1_equals_plain():

@@ -26,7 +26,7 @@ def _system(N, bath_state, seed):
 def _pair(H, lam, nu, T, K, D, bath_state, **opts):
     from paper_1803_03498_b200 import Heom
     o = Oracle(H, lam, nu, T, K, D, bath_state=bath_state)
-    g = Heom(H, lam, nu, T, K, D, bath_state=bath_state, **opts).bind()
+    g = Heom(H, lam, nu, T, K, D, bath_state=bath_state, **opts).bind(poison=True)
     return o, g
 
 
