@@ -163,7 +163,10 @@ heom_status heom_expectation(heom_ctx* ctx, const double* A, double* re, double*
  * (torch.distributed / NCCL all_to_all_single in paper_1803_03498_b200/sharded.py): per RK4 step
  *   for stage in 0..3: heom_rk4_stage; heom_stage_output -> buf; heom_pack_halo(buf -> send);
  *                      all-to-all: send rows -> the peers' ghost rows of buf
- * heom_set_state sets the rank's copy of sigma_0 (owned or ghost) if it holds one. */
+ * heom_set_state sets the rank's copy of sigma_0 (owned or ghost) if it holds one; heom_populations and
+ * heom_expectation return HEOM_ESTATE on a rank that holds none; heom_rk4_steps returns HEOM_ESTATE on a
+ * partition with world > 1 (it cannot exchange).  Kernels launch over the owned rows only.  Errors: rank/world out
+ * of range or world > number of nodes -> HEOM_EINVAL. */
 heom_status heom_create_partition(heom_ctx** out, int n_states, const double* H_cm, int n_baths,
                                   const int* bath_state, const double* lambda_cm, const double* nu_per_fs,
                                   double T_kelvin, int K, int D, int device, int rank, int world);

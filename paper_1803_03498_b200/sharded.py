@@ -91,6 +91,8 @@ class ShardedHeom:
 
     def __getattr__(self, name):
         # plumbing calls (sync, set_option, kernel_time, launch_count, kernel_name, ...) go to the partition context
+        if name == "g":
+            raise AttributeError(name)
         return getattr(self.g, name)
 
 
