@@ -117,3 +117,35 @@ def test_partition_refuses_unsplit_stepping():
     with pytest.raises(HeomError) as e:
         g.rk4_steps(1.0, 1)
     assert e.value.status == -4
+
+
+def test_sharded_class_nccl_world_1():
+    """ShardedHeom end to end through torch.distributed NCCL with a one-rank group on the one GPU there is: the
+    exchange call (views of the workspace tensor, split lists, in-place receive) is issued after every stage."""
+    import os
+    import socket
+    import torch.distributed as dist
+    from paper_1803_03498_b200.sharded import ShardedHeom
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        w = workloads.fmo_like().with_(D=3)
+        o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D)
+        sh = ShardedHeom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, 0, 1).bind()
+        assert sh.n_owned == o.nodes and sh.send_counts.sum() == 0
+        o.set_state(w.sigma0()); sh.set_state(w.sigma0())
+        for _ in range(40):
+            for stage in range(4):
+                sh.g.rk4_stage(w.dt_fs, stage)
+                sh.exchange(stage)                                  # nothing to move, but the collective runs
+        o.rk4_steps(w.dt_fs, 40)
+        got = sh.gather_state(o.nodes)
+        assert rel_err(got, o.get_full_state()) < STATE_TOL
+        pop, tr = sh.populations()
+        assert abs(tr - 1.0) < 1e-12
+    finally:
+        dist.destroy_process_group()
