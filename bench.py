@@ -274,7 +274,7 @@ def main():
         achieved = alg_bytes_per_launch / avg_launch_s / 1e9
         # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
         # (average over the 4 stage launches of one RK4 step), or null where no capture exists
-        ncu_traffic = {"cfg2_fmo7": (965.0e6, "profiles/r1c_cfg2_hpipe.md"),
+        ncu_traffic = {"cfg2_fmo7": (964.6e6, "profiles/r1d_cfg2_hpipe.md"),
                        "cfg3_deep7": (36.6e9, "profiles/r1c_cfg3_hpipe.md"),
                        "cfg5_large96": (94.4e9, "profiles/r1c_cfg5_large.md")}.get(w.name, (None, None))
         if w.N >= 32:
