@@ -149,3 +149,38 @@ def test_sharded_class_nccl_world_1():
         assert abs(tr - 1.0) < 1e-12
     finally:
         dist.destroy_process_group()
+
+
+def test_partition_launch_cost_follows_owned_rows():
+    """A partition launches over its owned rows only: on config 2 split 4 ways, rank 2 (1.44 ghosts per owned node)
+    must cost about a quarter of the full launch, not (1 + 1.44)/4 of it.  Prints the times."""
+    from paper_1803_03498_b200 import Heom
+    w = workloads.fmo_like()
+
+    def stage_ms(g, reps=40):
+        g.set_state(w.sigma0())
+        for s in range(4):
+            g.rk4_stage(w.dt_fs, s)                                 # warm-up (ghost rows stay as they are: timing only)
+        g.sync()
+        g.set_option("timing", 1); g.kernel_time()
+        for _ in range(reps):
+            for s in range(4):
+                g.rk4_stage(w.dt_fs, s)
+        ms, n = g.kernel_time()
+        g.set_option("timing", 0)
+        return ms / n
+
+    full = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, ket=0).bind()
+    t_full = stage_ms(full)
+    full.close()
+    out = []
+    for world, rank in ((2, 1), (4, 2), (8, 4)):
+        g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, partition=(rank, world)).bind()
+        t = stage_ms(g)
+        out.append((world, rank, g.owned(), g.nodes - g.owned(), t))
+        g.close()
+    print(f"\nPARTITION_COST cfg2 full launch {t_full*1e3:.1f} us; " +
+          "; ".join(f"world {wd} rank {r}: owned {o} ghosts {gh} launch {t*1e3:.1f} us ({t/t_full:.2f} of full, ideal {1/wd:.2f})"
+                    for wd, r, o, gh, t in out))
+    for wd, r, o, gh, t in out:
+        assert t < (1.0 / wd + 0.5 * gh / (o + gh) / wd + 0.12) * t_full
