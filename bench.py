@@ -202,7 +202,12 @@ def main():
         g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, device=local_rank, bath_state=w.bath_state,
                  **{k: int(v) for k, v in opts.items()})
     g.bind(stream=stream)
-    sigma0 = replicas.replica_sigma0(w, rank) if (w.sigma0_matrix is None and not shard) else w.sigma0()
+    if w.sigma0_matrix is None and not shard:
+        sigma0 = replicas.replica_sigma0(w, rank)
+    elif args.config == "absorb" and not shard:
+        sigma0 = workloads.absorption_fmo(p=(2 + rank) % 3).sigma0()   # replicas = polarisation directions (Eq. 55)
+    else:
+        sigma0 = w.sigma0()
     job = 1 if shard else world          # whole-job units: one hierarchy (shard) or one per rank (replicas)
     flush = None
     if w.state_bytes <= 130e6:

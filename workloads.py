@@ -124,13 +124,14 @@ def large():
                     0.5, 50)
 
 
-def absorption_fmo():
+def absorption_fmo(p=2):
     """Not a BASELINE config: the paper's linear-absorption use (Fig. 5: FMO at 77 K) on the FMO-like
-    stand-in.  cfg2's H with the ground state as state 0, its 7 baths on states 1..7, sigma_0(0) = mu_z |0><0|
-    (a non-Hermitian state: the general-state kernels), N = 8, W = 14, D = 8, the same 319 770 nodes."""
+    stand-in.  cfg2's H with the ground state as state 0, its 7 baths on states 1..7, sigma_0(0) = mu_p |0><0|
+    (p = 0, 1, 2: the polarisation directions of Eq. 55, independent replicas; default z), a non-Hermitian
+    single-column state, N = 8, W = 14, D = 8, the same 319 770 nodes."""
     w = fmo_like()
     H, bath_state, dip = with_ground_state(w)
-    mu = dipole_operator(dip, 2)
+    mu = dipole_operator(dip, int(p) % 3)
     s0 = np.zeros((8, 8), dtype=np.complex128)
     s0[:, 0] = mu[:, 0]
     return Workload("absorb_fmo8", H, 35.0, 50.0, 77.0, 1, 8, 1.0, 1000, tuple(bath_state), s0)
