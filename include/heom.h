@@ -77,18 +77,19 @@ void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
  *   "order"   device storage order of the nodes: 0 = pinned order, 1 = plain
  *             lexicographic (default 1)
  *   "kernel"  0 = generic element-per-thread kernel, 1 = auto (specialised
- *             kernels where available; default), 2 = as 1 without the persistent
- *             pipelined / tensor-core kernels (for comparison)
+ *             kernels where available; default), 2 = as 1 without the
+ *             whole-propagation kernel for tiny hierarchies (always 4 launches per step)
  *   "pade"    0 (default) = Matsubara poles and coefficients (Eq. 19-20); 1 = Pade poles (P:148-176
  *             Eq. 27-33, R11): the K poles beyond the Drude pole become xi_k/(beta hbar) with weights eta_k.
  *             Rebuilds the coefficients (heom_get_coefficients reports them)
  *   "l2_fetch" cudaLimitMaxL2FetchGranularity to request (32, 64, 128), 0 = leave it
  * and at any time:
  *   "rk4_form" how heom_rk4_steps groups the classical RK4 step (R6): 0 = the four
- *             classical stages; 1 or -1 (default) = the Taylor/Horner form v_s = (dt/s) L v_{s-1},
- *             y' = y + v1 + v2 + v3 + v4 -- identical for this linear autonomous right-hand side up
- *             to rounding, 14 instead of 16 state sizes of traffic -- where the kernel in use
- *             supports it (the pipelined small-N kernel and the large-N tensor-core kernel)
+ *             classical stages with a running sum (16 state sizes of traffic per step); 1 or -1
+ *             (default) = the Horner form w <- y + (dt/s) L w for s = 4, 3, 2, 1, y' = the last w --
+ *             the same polynomial in dt L for this linear autonomous right-hand side, equal up to
+ *             rounding, no running sum, 11 state sizes of traffic -- where the kernel in use
+ *             supports it (the pipelined small-N, the tensor-core and the column kernels)
  *   "warps_per_cta" warps per CTA of the pipelined small-N kernel, 0 = as many as fit (default)
  *   "timing"  1 = bracket every RHS launch with CUDA events (heom_kernel_time)
  *   "hermitian" 1 (default) = when heom_set_state / heom_set_full_state find the state
@@ -98,7 +99,7 @@ void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
  *   "ket"     1 (default) = when heom_set_state finds sigma_0 with exactly ONE non-zero column c, state c
  *             without a bath (heom_create_sites) and uncoupled in H (H[c][j] = 0 for j != c) -- the
  *             mu_p|0><0| state of linear absorption, P:301 -- every sigma_u keeps that shape, and the state is
- *             held and propagated as one N-vector per node (kernels_ket.cu; Taylor/Horner form of RK4).
+ *             held and propagated as one N-vector per node (kernels_ket.cu; Horner form of RK4).
  *             All getters still return full matrices.  0 = always full matrices.  Takes effect at the next
  *             heom_set_state; heom_set_full_state always selects full matrices. */
 heom_status heom_set_option(heom_ctx* ctx, const char* name, int value);
@@ -192,6 +193,11 @@ int64_t heom_launch_count(const heom_ctx* ctx); /* kernels launched so far */
 heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches);
 /* Name of the RHS kernel variant the bound configuration uses (static string). */
 const char* heom_kernel_name(const heom_ctx* ctx);
+/* Measured peak of `device` for the harness' roofline (no context needed; synchronises; allocates
+ * and frees its own scratch): kind 0 = FP64 FMA (register-resident DFMA chains), 1 = FP64 tensor core
+ * (mma.sync.m8n8k4.f64, SASS DMMA.8x8x4) -- *value in TFLOP/s; 2 = HBM copy bandwidth (read + write bytes of a
+ * 1 GiB device-to-device copy kernel) -- *value in GB/s.  Best of 5 timed repetitions after one warm-up. */
+heom_status heom_probe_peak(int device, int kind, double* value);
 /* Human-readable text of the last error on this context (ctx-owned). */
 const char* heom_last_error(const heom_ctx* ctx);
 

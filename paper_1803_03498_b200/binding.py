@@ -23,7 +23,7 @@ SYMBOLS = [
     "heom_get_tables", "heom_get_coefficients", "heom_workspace_bytes", "heom_bind_workspace",
     "heom_set_state", "heom_set_full_state", "heom_get_full_state", "heom_rhs", "heom_rk4_steps",
     "heom_sync", "heom_populations", "heom_launch_count", "heom_kernel_time", "heom_kernel_name",
-    "heom_last_error",
+    "heom_last_error", "heom_probe_peak",
 ]
 
 _lib = None
@@ -85,12 +85,24 @@ def load_library():
     lib.heom_kernel_name.restype = C.c_char_p
     lib.heom_last_error.argtypes = [P]
     lib.heom_last_error.restype = C.c_char_p
+    lib.heom_probe_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
     _lib = lib
     return lib
 
 
 def _dptr(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def probe_peak(kind, device=0):
+    """heom_probe_peak: measured FP64 FMA ("dfma") / FP64 tensor-core ("dmma") peak in TFLOP/s, or HBM copy
+    bandwidth ("hbm") in GB/s, of `device`."""
+    lib = load_library()
+    v = C.c_double()
+    rc = lib.heom_probe_peak(int(device), {"dfma": 0, "dmma": 1, "hbm": 2}[kind], C.byref(v))
+    if rc != 0:
+        raise HeomError(rc, "heom_probe_peak failed (no CUDA device?)")
+    return v.value
 
 
 class Heom:

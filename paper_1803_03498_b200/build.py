@@ -1,20 +1,23 @@
 """Build the CUDA library in-tree: paper_1803_03498_b200/libheom_b200.so (sm_100a only).
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the GPU box.
+Every source is compiled to its own object (in parallel, only when stale), then linked.
 """
 import glob
 import os
 import shutil
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libheom_b200.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-Xcompiler", "-fPIC,-fopenmp,-O2", "--shared",
+    "-Xcompiler", "-fPIC,-fopenmp,-O2",
 ]
 
 
@@ -29,9 +32,13 @@ def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cpp")))
 
 
-def deps():
-    return sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.hpp")) \
+def headers():
+    return glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.hpp")) \
         + glob.glob(os.path.join(INCLUDE, "*.h")) + [os.path.abspath(__file__)]
+
+
+def deps():
+    return sources() + headers()
 
 
 def build(force: bool = False, verbose: bool = False, extra=()) -> str:
@@ -39,15 +46,33 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
         return LIB
     if os.environ.get("HEOM_DEBUG"):
         extra = list(extra) + ["-DHEOM_DEBUG"]
-    cmd = [nvcc_path()] + NVCC_FLAGS + list(extra) + ["-I", INCLUDE, "-o", LIB] + sources() + ["-lgomp"]
-    if verbose:
-        cmd.insert(1, "-Xptxas")
-        cmd.insert(2, "-v")
-        print(" ".join(cmd))
-    subprocess.run(cmd, check=True)
+    os.makedirs(OBJ, exist_ok=True)
+    tag = os.path.join(OBJ, "flags.txt")
+    flags = " ".join(NVCC_FLAGS + list(extra))
+    if not os.path.exists(tag) or open(tag).read() != flags:
+        force = True
+    hdr_time = max(map(os.path.getmtime, headers()))
+    nvcc = nvcc_path()
+
+    def compile_one(src):
+        obj = os.path.join(OBJ, os.path.basename(src) + ".o")
+        if not force and os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(src), hdr_time):
+            return obj
+        cmd = [nvcc] + NVCC_FLAGS + list(extra) + (["-Xptxas", "-v"] if verbose else []) \
+            + ["-I", INCLUDE, "-c", "-o", obj, src]
+        if verbose:
+            print(" ".join(cmd))
+        subprocess.run(cmd, check=True)
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as pool:
+        objs = list(pool.map(compile_one, sources()))
+    subprocess.run([nvcc, "--shared", "-o", LIB] + objs + ["-lgomp"], check=True)
+    with open(tag, "w") as f:
+        f.write(flags)
     return LIB
 
 
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force="-f" in sys.argv or "-v" in sys.argv, verbose="-v" in sys.argv))

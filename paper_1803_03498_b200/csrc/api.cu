@@ -44,17 +44,11 @@ struct heom_ctx {
   int stride = 0;  // complex elements per node
   size_t state_bytes = 0;
   double2 *y = nullptr, *acc = nullptr, *xa = nullptr, *xb = nullptr;
-  int32_t *d_plus = nullptr, *d_minus = nullptr, *d_slot = nullptr, *d_links = nullptr;
-  int lrow = 0;
-  bool use_rows = false;
-  // Hermitian fast path (kernels_herm.cu)
+  int32_t *d_plus = nullptr, *d_minus = nullptr, *d_slot = nullptr;
+  // Hermitian fast path of the pipelined kernel
   int herm_opt = 1;          // option "hermitian": 1 = use it when the state is exactly Hermitian
-  bool use_herm = false;     // kernel available for this shape
   bool state_hermitian = false;
-  int32_t* d_linksH = nullptr;
-  double* d_coefH = nullptr;
-  int lrowH = 0;
-  // persistent pipelined Hermitian kernel (kernels_hpipe.cu)
+  // persistent pipelined kernel (kernels_hpipe.cu)
   bool use_hpipe = false;
   int32_t* d_linksP = nullptr;
   int lrowP = 0;
@@ -78,9 +72,7 @@ struct heom_ctx {
   size_t n_links = 0;
   unsigned long long* d_tickets = nullptr;   // work counter of the persistent kernel
   unsigned long long ticket_base = 0;
-  int acc_red = 1;           // option "acc_red": 1 (default) = Taylor stages 2-4 of the large-N kernel add to the running sum
-                             // with fire-and-forget global reductions, 0 = they load, add and store it
-  int rk4_form = -1;         // option "rk4_form": 0 classical stages, 1 Taylor/Horner (large-N kernel only), -1 auto
+  int rk4_form = -1;         // option "rk4_form": 0 classical stages, 1 Horner form (where the kernel supports it), -1 auto
   int l2_fetch = 0;          // option "l2_fetch": cudaLimitMaxL2FetchGranularity in bytes, 0 = leave the default
   int sms = 148;
   uint8_t* d_tuples = nullptr;
@@ -156,27 +148,41 @@ bool ensure_hierarchy(heom_ctx* c) {
 }
 
 int node_stride(int N) { return N * N; }
-// int32 entries per row of the combined link table: plus[W], minus[W], W tuple bytes, padded to 16 B
-int links_row(int W) { return (2 * W + (W + 3) / 4 + 3) / 4 * 4; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_links, off_linksH, off_coefH, off_linksP, off_Hs, off_delta, off_A, off_S0, off_send, off_lptr, off_lent, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_linksP, off_Hs, off_delta, off_A, off_S0, off_send, off_lptr, off_lent, total;
 };
+
+// Which kernel family the bound configuration will run (fixed by the shape and the "kernel" option), so that the
+// workspace holds the link tables of that family only (config 3: 1.1 GB of plain tables against 1.7 GB of meta rows).
+struct KernelChoice { bool hpipe, large, tiny, plain_tables; };
+KernelChoice kernel_choice(const heom_ctx* c) {
+  KernelChoice k{};
+  const int N = c->h.N, Wd = dev_modes(c), D = c->h.D;
+  const long long nodes = (long long)c->h.nodes;
+  k.large = c->kernel >= 1 && large_supported(N, Wd);
+  k.hpipe = c->kernel >= 1 && hpipe_supported(N, Wd, D, nodes);
+  k.tiny = c->kernel == 1 && !c->partitioned && tiny_supported(N, Wd, D, nodes);
+  k.plain_tables = k.tiny || !(k.large || k.hpipe);   // plus/minus/tuples [nodes][W]: generic and tiny kernels
+  return k;
+}
 
 Layout layout_of(const heom_ctx* c) {
   Layout L{};
   const size_t nodes = (size_t)c->h.nodes, W = (size_t)dev_modes(c), N = (size_t)c->h.N, D1 = (size_t)c->h.D + 1;
+  const KernelChoice kc = kernel_choice(c);
+  const size_t tab = kc.plain_tables ? nodes * W : 0;
   L.state = align_up(nodes * (size_t)node_stride((int)N) * sizeof(double2));
   size_t o = 0;
   L.off_y = o; o += L.state;
   L.off_acc = o; o += L.state;
   L.off_xa = o; o += L.state;
   L.off_xb = o; o += L.state;
-  L.off_plus = o; o += align_up(nodes * W * 4);
-  L.off_minus = o; o += align_up(nodes * W * 4);
+  L.off_plus = o; o += align_up(tab * 4);
+  L.off_minus = o; o += align_up(tab * 4);
   L.off_slot = o; o += align_up(nodes * 4);
-  L.off_tuples = o; o += align_up(nodes * W);
+  L.off_tuples = o; o += align_up(tab);
   L.off_damp = o; o += align_up((nodes + 1) * 8);
   L.off_H = o; o += align_up(N * N * 8);
   L.off_T = o; o += align_up(N * N * 8);
@@ -184,16 +190,13 @@ Layout layout_of(const heom_ctx* c) {
   L.off_amx = o; o += align_up(W * D1 * 8);
   L.off_amo = o; o += align_up(W * D1 * 8);
   L.off_scratch = o; o += align_up((N + 2) * 8 + 128);
-  L.off_links = o; o += align_up(nodes * (size_t)links_row((int)W) * 4);
-  L.off_linksH = o; o += align_up(nodes * (size_t)herm_links_row((int)N, c->h.M) * 4);
-  L.off_coefH = o; o += align_up(W * D1 * 32);
-  L.off_linksP = o; o += align_up(nodes * (size_t)hpipe_links_row((int)N, c->h.M) * 4);
+  L.off_linksP = o; o += align_up(kc.hpipe ? nodes * (size_t)hpipe_links_row((int)N, c->h.M) * 4 : 0);
   L.off_Hs = o; o += align_up(N * N * 8);
   L.off_delta = o; o += align_up(N * 8);
   L.off_A = o; o += align_up(N * N * 16);
   L.off_S0 = o; o += align_up(N * N * 16);
   L.off_send = o; o += align_up(c->part.send_idx.size() * 4 + 16);
-  if (large_supported((int)N, (int)W)) {
+  if (kc.large) {
     // CSR link list: one 16-byte entry per valid "+" and per valid "-" link (a partition's table has links for its
     // owned rows only, so the two counts differ there)
     size_t links = 0;
@@ -245,9 +248,6 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
                         ctx->cd.a_minus_o.data(), ctx->H.data(), ctx->cd.delta.data(),
                         ctx->herm_opt && ctx->state_hermitian, ctx->warps_per_cta, ctx->sms, ctx->d_tickets,
                         &ctx->ticket_base, ctx->stream));
-  else if (ctx->use_herm && ctx->herm_opt && ctx->state_hermitian)
-    CU(launch_rhs_herm(p, ctx->d_linksH, ctx->lrowH, ctx->d_coefH, ctx->H.data(), ctx->cd.delta.data(), ctx->stream));
-  else if (ctx->use_rows) CU(launch_rhs_rows(p, ctx->d_links, ctx->lrow, ctx->H.data(), ctx->stream));
   else CU(launch_rhs_generic(p, ctx->stream));
   ctx->launches += 1;
   if (ctx->timing) CU(cudaEventRecord(e1, ctx->stream));
@@ -274,38 +274,31 @@ heom_status sigma0_matrix(heom_ctx* ctx, const double2** out) {
 }
 
 // One fused RHS + RK4-stage launch (stage = 0..3) of the matrix kernels, in the form the kernel in use takes (R6):
-//  - Taylor/Horner (pipelined small-N and tensor-core kernels unless rk4_form = 0):
-//      v1 = dt f(y), v_s = (dt/s) f(v_{s-1}), y' = y + v1 + v2 + v3 + v4; the stages never read y: 14 state sizes
+//  - Horner (pipelined small-N and tensor-core kernels unless rk4_form = 0): w <- y + (dt/s) f(w), s = 4, 3, 2, 1,
+//      xa = y + dt/4 f(y) | xb = y + dt/3 f(xa) | xa = y + dt/2 f(xb) | y = y + dt f(xa)  (in place)
+//      no running sum: 2 + 3 + 3 + 3 = 11 state sizes of traffic per step, three buffers
 //  - classical: k1 = f(y); xa = y + dt/2 k1; acc = y + dt/6 k1 | k2 = f(xa); xb = y + dt/2 k2; acc += dt/3 k2 |
-//               k3 = f(xb); xa = y + dt k3; acc += dt/3 k3     | k4 = f(xa); y = acc + dt/6 k4
+//               k3 = f(xb); xa = y + dt k3; acc += dt/3 k3     | k4 = f(xa); y = acc + dt/6 k4     (16 state sizes)
 // After the stage the next stage's input is xa (stages 0, 2), xb (stage 1) or y (stage 3): heom_stage_output.
 heom_status launch_stage(heom_ctx* ctx, double dt, int stage) {
   RhsParams p = base_params(ctx);
   p.rhs_only = 0;
-  const bool taylor_large = ctx->use_large && ctx->rk4_form != 0;
-  const bool taylor_pipe = !taylor_large && ctx->use_hpipe && ctx->rk4_form != 0;
+  const bool horner = (ctx->use_large || ctx->use_hpipe) && ctx->rk4_form != 0;
   p.x = stage == 0 ? ctx->y : (stage == 2 ? ctx->xb : ctx->xa);
+  p.y = ctx->y;
+  if (horner) {
+    p.horner = 1;
+    p.out_x = stage == 3 ? ctx->y : (stage == 1 ? ctx->xb : ctx->xa);
+    p.acc_in = nullptr; p.out_acc = nullptr;
+    p.ax = dt / (double)(4 - stage);
+    p.bx = 0.0;
+    return launch_rhs(ctx, p);
+  }
   p.out_x = stage == 3 ? nullptr : (stage == 1 ? ctx->xb : ctx->xa);
   p.acc_in = stage == 0 ? ctx->y : ctx->acc;
-  if (taylor_large) {
-    /* acc = y + v1 is stored, v2..v4 are added to it by global reductions; y and acc then swap roles */
-    p.taylor = 1; p.y = nullptr; p.out_acc = ctx->acc;
-    p.acc_red = stage == 0 ? 0 : ctx->acc_red;
-    p.ax = p.bx = dt / (double)(stage + 1);
-    heom_status s = launch_rhs(ctx, p);
-    if (s != HEOM_OK) return s;
-    if (stage == 3) { double2* tmp = ctx->y; ctx->y = ctx->acc; ctx->acc = tmp; }
-    return HEOM_OK;
-  }
-  p.y = ctx->y;
   p.out_acc = stage == 3 ? ctx->y : ctx->acc;
-  if (taylor_pipe) {
-    p.taylor = 1;
-    p.ax = p.bx = dt / (double)(stage + 1);
-  } else {
-    p.ax = stage == 2 ? dt : dt / 2.0;
-    p.bx = (stage == 0 || stage == 3) ? dt / 6.0 : dt / 3.0;
-  }
+  p.ax = stage == 2 ? dt : dt / 2.0;
+  p.bx = (stage == 0 || stage == 3) ? dt / 6.0 : dt / 3.0;
   return launch_rhs(ctx, p);
 }
 
@@ -414,7 +407,6 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
     ctx->l2_fetch = value;
     return HEOM_OK;
   }
-  if (s == "acc_red") { ctx->acc_red = value ? 1 : 0; return HEOM_OK; }
   if (s == "ket") { ctx->ket_opt = value ? 1 : 0; return HEOM_OK; }   // takes effect at the next heom_set_state
   if (s == "rk4_form") {
     if (value < -1 || value > 1) return fail(ctx, HEOM_EINVAL, "rk4_form must be -1, 0 or 1");
@@ -517,16 +509,10 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->d_tickets = (unsigned long long*)(base + L.off_scratch + (((size_t)ctx->h.N + 2) * 8 + 63) / 64 * 64);
   ctx->ticket_base = 0;
   CU(cudaMemset(ctx->d_tickets, 0, 8));
-  ctx->d_links = (int32_t*)(base + L.off_links);
   const int Wd = dev_modes(ctx);
-  ctx->lrow = links_row(Wd);
-  ctx->use_rows = ctx->kernel >= 1 && rows_supported(ctx->h.N, Wd, ctx->h.D, ctx->lrow);
-  ctx->d_linksH = (int32_t*)(base + L.off_linksH);
-  ctx->d_coefH = (double*)(base + L.off_coefH);
-  ctx->lrowH = herm_links_row(ctx->h.N, ctx->h.M);
-  ctx->use_herm = ctx->kernel >= 1 && herm_supported(ctx->h.N, Wd, ctx->h.D);
-  ctx->use_large = ctx->kernel == 1 && large_supported(ctx->h.N, Wd);
-  ctx->use_tiny = ctx->kernel == 1 && !ctx->partitioned && tiny_supported(ctx->h.N, Wd, ctx->h.D, (long long)ctx->h.nodes);
+  const KernelChoice kc = kernel_choice(ctx);
+  ctx->use_large = kc.large;
+  ctx->use_tiny = kc.tiny;
   ctx->d_Hs = (double*)(base + L.off_Hs);
   ctx->d_delta = (double*)(base + L.off_delta);
   ctx->d_A = (double2*)(base + L.off_A);
@@ -539,7 +525,7 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->d_lent = (void*)(base + L.off_lent);
   ctx->d_linksP = (int32_t*)(base + L.off_linksP);
   ctx->lrowP = hpipe_links_row(ctx->h.N, ctx->h.M);
-  ctx->use_hpipe = ctx->kernel == 1 && hpipe_supported(ctx->h.N, Wd, ctx->h.D, (long long)ctx->h.nodes);
+  ctx->use_hpipe = kc.hpipe && !kc.large;
   {
     cudaDeviceProp prop;
     CU(cudaGetDeviceProperties(&prop, ctx->device));
@@ -571,23 +557,13 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
       }
       damp[s] = d;
     }
-    CU(cudaMemcpy(ctx->d_plus, tp.data(), nodes * W * 4, cudaMemcpyHostToDevice));
-    CU(cudaMemcpy(ctx->d_minus, tm.data(), nodes * W * 4, cudaMemcpyHostToDevice));
-    CU(cudaMemcpy(ctx->d_tuples, tt.data(), nodes * W, cudaMemcpyHostToDevice));
+    if (kc.plain_tables) {
+      CU(cudaMemcpy(ctx->d_plus, tp.data(), nodes * W * 4, cudaMemcpyHostToDevice));
+      CU(cudaMemcpy(ctx->d_minus, tm.data(), nodes * W * 4, cudaMemcpyHostToDevice));
+      CU(cudaMemcpy(ctx->d_tuples, tt.data(), nodes * W, cudaMemcpyHostToDevice));
+    }
     CU(cudaMemset(ctx->d_damp + nodes, 0, 8));
     CU(cudaMemcpy(ctx->d_damp, damp.data(), nodes * 8, cudaMemcpyHostToDevice));
-    if (ctx->use_rows) {
-      const size_t lrow = (size_t)ctx->lrow;
-      std::vector<int32_t> lk(nodes * lrow, 0);
-#pragma omp parallel for schedule(static)
-      for (int64_t s = 0; s < (int64_t)nodes; ++s) {
-        int32_t* row = &lk[(size_t)s * lrow];
-        std::memcpy(row, &tp[(size_t)s * W], W * 4);
-        std::memcpy(row + W, &tm[(size_t)s * W], W * 4);
-        std::memcpy(row + 2 * W, &tt[(size_t)s * W], W);
-      }
-      CU(cudaMemcpy(ctx->d_links, lk.data(), nodes * lrow * 4, cudaMemcpyHostToDevice));
-    }
     if (ctx->use_large) {
       // CSR link list in storage-slot order: "+" links first, then "-" links, of every node
       std::vector<int64_t> lptr(nodes + 1, 0);
@@ -621,22 +597,6 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
         hpipe_pack_links(h.N, h.M, h.D, &tp[(size_t)s * W], &tm[(size_t)s * W], &tt[(size_t)s * W], damp[(size_t)s], &lk[(size_t)s * lrow]);
       CU(cudaMemcpy(ctx->d_linksP, lk.data(), nodes * lrow * 4, cudaMemcpyHostToDevice));
     }
-    if (ctx->use_herm || ctx->use_hpipe) {
-      const size_t D1 = (size_t)h.D + 1;
-      std::vector<double> cf(W * D1 * 4, 0.0);
-      for (size_t q = 0; q < W * D1; ++q) {
-        cf[4 * q] = ctx->cd.a_plus[q]; cf[4 * q + 1] = ctx->cd.a_minus_x[q]; cf[4 * q + 2] = ctx->cd.a_minus_o[q];
-      }
-      CU(cudaMemcpy(ctx->d_coefH, cf.data(), W * D1 * 32, cudaMemcpyHostToDevice));
-    }
-    if (ctx->use_herm) {
-      const size_t lrow = (size_t)ctx->lrowH;
-      std::vector<int32_t> lk(nodes * lrow, 0);
-#pragma omp parallel for schedule(static)
-      for (int64_t s = 0; s < (int64_t)nodes; ++s)
-        herm_pack_links(h.N, h.M, &tp[(size_t)s * W], &tm[(size_t)s * W], &tt[(size_t)s * W], &lk[(size_t)s * lrow]);
-      CU(cudaMemcpy(ctx->d_linksH, lk.data(), nodes * lrow * 4, cudaMemcpyHostToDevice));
-    }
   } catch (const std::bad_alloc&) {
     return fail(ctx, HEOM_ENOMEM, "out of host memory while staging the device tables");
   }
@@ -647,6 +607,9 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   CU(cudaMemcpy(ctx->d_ap, ctx->cd.a_plus.data(), WD * 8, cudaMemcpyHostToDevice));
   CU(cudaMemcpy(ctx->d_amx, ctx->cd.a_minus_x.data(), WD * 8, cudaMemcpyHostToDevice));
   CU(cudaMemcpy(ctx->d_amo, ctx->cd.a_minus_o.data(), WD * 8, cudaMemcpyHostToDevice));
+  // the uploads above are pageable-memory copies on the legacy stream: they may return before the DMA has landed,
+  // and ctx->stream does not synchronise with the legacy stream -- wait for the device once, here
+  CU(cudaDeviceSynchronize());
   ctx->bound = true;
   ctx->have_state = false;
   return HEOM_OK;
@@ -773,29 +736,25 @@ heom_status heom_rhs(heom_ctx* ctx, double* dsigma) {
   return read_back(ctx, ctx->xa, ctx->xb, dsigma);
 }
 
-/* Classical RK4 (R6) with the stage combinations fused into the RHS epilogue (4 buffers):
- *   stage 1: k1 = f(y);   xa = y + dt/2 k1;  acc = y + dt/6 k1
- *   stage 2: k2 = f(xa);  xb = y + dt/2 k2;  acc += dt/3 k2
- *   stage 3: k3 = f(xb);  xa = y + dt   k3;  acc += dt/3 k3
- *   stage 4: k4 = f(xa);  y  = acc + dt/6 k4                                        */
+/* nsteps RK4 steps, four fused RHS + stage launches each (launch_stage above: Horner or classical form, R6). */
 heom_status heom_rk4_steps(heom_ctx* ctx, double dt, int nsteps) {
   if (!ctx || nsteps < 0 || !std::isfinite(dt)) return HEOM_EINVAL;
   if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
   RhsParams p = base_params(ctx);
   p.rhs_only = 0;
   if (ctx->ket_col >= 0) {
-    /* column-sparse state: Taylor/Horner form (R6) on the kets, 4 launches per step */
-    double2 *ky = ket_buf(ctx, KET_Y), *ka = ket_buf(ctx, KET_ACC), *kxa = ket_buf(ctx, KET_XA), *kxb = ket_buf(ctx, KET_XB);
-    p.taylor = 1;
+    /* column-sparse state: Horner form (R6) on the kets, 4 launches per step, three ket buffers */
+    double2 *ky = ket_buf(ctx, KET_Y), *kxa = ket_buf(ctx, KET_XA), *kxb = ket_buf(ctx, KET_XB);
+    p.horner = 1; p.y = ky;
     for (int step = 0; step < nsteps; ++step) {
       heom_status s;
-      p.x = ky; p.acc_in = ky; p.out_x = kxa; p.out_acc = ka; p.ax = p.bx = dt;          /* v1; acc = y + v1 */
+      p.x = ky; p.out_x = kxa; p.ax = dt / 4.0;
       if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-      p.x = kxa; p.acc_in = ka; p.out_x = kxb; p.ax = p.bx = dt / 2.0;                    /* v2; acc += v2 */
+      p.x = kxa; p.out_x = kxb; p.ax = dt / 3.0;
       if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-      p.x = kxb; p.out_x = kxa; p.ax = p.bx = dt / 3.0;                                   /* v3; acc += v3 */
+      p.x = kxb; p.out_x = kxa; p.ax = dt / 2.0;
       if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
-      p.x = kxa; p.out_x = nullptr; p.out_acc = ky; p.ax = p.bx = dt / 4.0;               /* y = acc + v4 */
+      p.x = kxa; p.out_x = ky; p.ax = dt;                /* in place: only node u reads y_u */
       if ((s = launch_rhs(ctx, p)) != HEOM_OK) return s;
     }
     return HEOM_OK;
@@ -830,7 +789,7 @@ heom_status heom_rk4_stage(heom_ctx* ctx, double dt, int stage) {
   if (!ctx || stage < 0 || stage > 3 || !std::isfinite(dt)) return HEOM_EINVAL;
   if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
   if (ctx->ket_col >= 0 || ctx->use_tiny)
-    return fail(ctx, HEOM_ESTATE, "stage-wise stepping is for the matrix kernels (set options ket=0, kernel=2)");
+    return fail(ctx, HEOM_ESTATE, "stage-wise stepping is for the matrix kernels (set options ket=0 and kernel=2)");
   return launch_stage(ctx, dt, stage);
 }
 
@@ -919,8 +878,7 @@ const char* heom_kernel_name(const heom_ctx* c) {
   if (c->ket_col >= 0) return "rhs_ket_kernel";
   if (c->use_large) return "rhs_large_kernel";
   if (c->use_hpipe) return (c->herm_opt && c->state_hermitian) ? "rhs_hpipe_kernel" : "rhs_hpipe_general_kernel";
-  if (c->use_herm && c->herm_opt && c->state_hermitian) return "rhs_herm_kernel";
-  return c->use_rows ? "rhs_rows_kernel" : "rhs_generic_kernel";
+  return "rhs_generic_kernel";
 }
 
 const char* heom_last_error(const heom_ctx* c) { return c ? c->err.c_str() : "null context"; }

@@ -31,32 +31,16 @@ struct RhsParams {
   double2* out_acc;       // acc_in + bx*k     (or, in RHS-only mode, k itself)
   double ax, bx;
   int rhs_only;           // 1: out_acc = k, nothing else read or written
-  // Taylor/Horner form of RK4 for a linear autonomous right-hand side (R6); honoured by the
-  // large-N kernel only (the others are always launched with both flags 0):
-  int taylor;             // 1: out_x = ax*k (y is not read)
-  int acc_red;            // 1: out_acc += bx*k by fire-and-forget global reductions (acc_in is not read)
+  // Horner form of RK4 for a linear autonomous right-hand side (R6): w <- y + (dt/s) L w, s = 4, 3, 2, 1.
+  // No running sum: acc_in / out_acc / bx are unused, out_x = y + ax*k (y may alias x: first stage; out_x may alias
+  // y: last stage, in place).  Honoured by the pipelined small-N, the tensor-core and the column kernels.
+  int horner;
 };
 
 // Generic kernel: any N <= 96, one thread per matrix element.
 cudaError_t launch_rhs_generic(const RhsParams& p, cudaStream_t s);
 // Shared-memory bytes the generic kernel needs (0 if N is unsupported).
 size_t rhs_generic_smem(int N);
-
-// Row-per-thread kernel for 2 <= N <= 16 (kernels_rows.cu).  links: DEVICE [nodes][lrow] int32 =
-// plus[W], minus[W], then the tuple bytes; H_host: HOST [N][N] (travels in the kernel parameters).
-bool rows_supported(int N, int W, int D, int lrow);
-cudaError_t launch_rhs_rows(const RhsParams& p, const int32_t* links, int lrow, const double* H_host,
-                            cudaStream_t s);
-
-// Hermitian-state kernel for 2 <= N <= 16 (kernels_herm.cu).  links: DEVICE [nodes][lrow] int32 in the
-// grouped layout written by herm_pack_links (per mode index kk: plus[N pad 4], minus[N pad 4], tuple
-// bytes [N pad 8]); coef: DEVICE [W][D+1][4] doubles = a+, a-x, a-o, 0.  H_host, delta_host: HOST.
-int herm_links_row(int N, int M);   // ints per row (multiple of 4), 0 if unsupported
-bool herm_supported(int N, int W, int D);
-void herm_pack_links(int N, int M, const int32_t* plus, const int32_t* minus, const uint8_t* tuple,
-                     int32_t* row);  // HOST: one node's row from its plus/minus/tuple entries [W]
-cudaError_t launch_rhs_herm(const RhsParams& p, const int32_t* links, int lrow, const double* coef,
-                            const double* H_host, const double* delta_host, cudaStream_t s);
 
 // Persistent TMA-pipelined kernel for 2 <= N <= 16 (kernels_hpipe.cu); hermitian = 1: the state is exactly
 // Hermitian (row-only gathers, exact Hermiticity preserved), 0: general state (row and column gathers).  links: DEVICE

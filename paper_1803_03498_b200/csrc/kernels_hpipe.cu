@@ -190,10 +190,10 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   const int npass = P.npass;
 
   const bool rhs_only = p.rhs_only != 0;
+  const bool horner = p.horner != 0;                  // out_x = y + ax*k, no running sum (R6)
   const bool y_is_x = (p.y == p.x), acc_is_x = (p.acc_in == p.x);
-  const bool need_A = !rhs_only && !acc_is_x;
-  const bool taylor = p.taylor != 0;                  // next stage input = ax*k (Taylor form): y is not read
-  const bool need_Y = !rhs_only && p.out_x != nullptr && !y_is_x && !taylor;
+  const bool need_A = !rhs_only && !horner && !acc_is_x;
+  const bool need_Y = !rhs_only && p.out_x != nullptr && !y_is_x;
   const bool write_x = !rhs_only && p.out_x != nullptr;
   const bool producer = lane == 0;
   const unsigned long long pol_stream = policy_evict_first(), pol_keep = policy_evict_last();
@@ -456,25 +456,23 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
       if (rhs_only) {
 #pragma unroll
         for (int i = 0; i < N; ++i) ac[i * N] = k[i];
+      } else if (horner) {                          // Horner stage: XA holds y (first stage: y = x); w' = y + ax k
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+          const double2 yv = xa[i * N];
+          xa[i * N] = make_double2(fma(p.ax, k[i].x, yv.x), fma(p.ax, k[i].y, yv.y));
+        }
       } else if (acc_is_x) {                        // stage 1: y = acc_in = x, still in XA
 #pragma unroll
         for (int i = 0; i < N; ++i) {
           const double2 yv = xa[i * N];
-          xa[i * N] = taylor ? make_double2(p.ax * k[i].x, p.ax * k[i].y)
-                             : make_double2(fma(p.ax, k[i].x, yv.x), fma(p.ax, k[i].y, yv.y));
+          xa[i * N] = make_double2(fma(p.ax, k[i].x, yv.x), fma(p.ax, k[i].y, yv.y));
           ac[i * N] = make_double2(fma(p.bx, k[i].x, yv.x), fma(p.bx, k[i].y, yv.y));
         }
       } else if (!write_x) {                        // stage 4: running sum only
 #pragma unroll
         for (int i = 0; i < N; ++i) {
           const double2 av = ac[i * N];
-          ac[i * N] = make_double2(fma(p.bx, k[i].x, av.x), fma(p.bx, k[i].y, av.y));
-        }
-      } else if (taylor) {                          // Taylor stages 2, 3: v_s = ax k
-#pragma unroll
-        for (int i = 0; i < N; ++i) {
-          const double2 av = ac[i * N];
-          xa[i * N] = make_double2(p.ax * k[i].x, p.ax * k[i].y);
           ac[i * N] = make_double2(fma(p.bx, k[i].x, av.x), fma(p.bx, k[i].y, av.y));
         }
       } else {                                      // classical stages 2, 3: y is in XA
@@ -491,7 +489,7 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     if (lane == 0) {
       const unsigned bx = (unsigned)ncnt * NN * 16;
       if (write_x) bulk_s2g(p.out_x + (size_t)n0 * NN, sXA, bx, pol_stream);
-      bulk_s2g(p.out_acc + (size_t)n0 * NN, sAC, bx, pol_stream);
+      if (!horner) bulk_s2g(p.out_acc + (size_t)n0 * NN, sAC, bx, pol_stream);
       bulk_commit();
     }
     if ((s ^= 1) == 0) ph ^= 1u;
@@ -553,9 +551,15 @@ cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, c
   if (grid < 1) grid = 1;
   P.tickets = tickets;
   P.ticket_base = *ticket_base;
-  *ticket_base += (unsigned long long)P.npass + 2ULL * grid * P.nwarps;   // two failing draws per warp
   rhs_hpipe_kernel<N, HERM><<<grid, P.nwarps * 32, smem, s>>>(P);
-  return cudaGetLastError();
+  const cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) {
+    *ticket_base += (unsigned long long)P.npass + 2ULL * grid * P.nwarps;   // two failing draws per warp
+  } else {                                 // nothing ran: keep host base and device counter in step
+    cudaMemsetAsync(tickets, 0, sizeof(unsigned long long), s);
+    *ticket_base = 0;
+  }
+  return e;
 }
 
 }  // namespace

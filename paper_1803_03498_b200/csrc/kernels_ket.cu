@@ -15,8 +15,8 @@
 //
 // Mapping: LP = 2, 4, 8 or 16 lanes per node (a power of two >= N), 32/LP nodes per warp; lane i holds v_u[i], the
 // commutator H v is N warp shuffles + FMAs with row i of H/hbar from shared memory, lane i gathers the 2M
-// neighbour elements of its own bath (16-byte loads, L2-resident), and the Taylor-form RK4 epilogue (DESIGN.md
-// R6) is fused: out_x = ax k, out_acc = acc_in + bx k.  The meta rows are the pipelined kernel's
+// neighbour elements of its own bath (16-byte loads, L2-resident), and the Horner-form RK4 epilogue (DESIGN.md
+// R6) is fused: out_x = y + ax k (y may alias x, out_x may alias y).  The meta rows are the pipelined kernel's
 // (hpipe_pack_links): neighbour offsets are slot*N*N, so the ket offset is off/N.
 #include "kernels.cuh"
 
@@ -30,12 +30,12 @@ constexpr int kKetThreads = 256;
 template <int N>
 struct KetParams {
   const double2* x;        // [nodes][N] stage input (gathered)
-  const double2* acc_in;   // [nodes][N] running sum to extend (may alias x)
-  double2* out_x;          // ax * k (null: not written)
-  double2* out_acc;        // acc_in + bx * k, or k itself when rhs_only
+  const double2* y;        // [nodes][N] step-start state (may alias x)
+  double2* out_x;          // y + ax * k
+  double2* out_acc;        // k itself when rhs_only
   const int32_t* links;    // hpipe meta rows [nodes][lrow]
   int lrow, nodes, M, col, rhs_only;
-  double ax, bx;
+  double ax;
   double hcc;              // H[c][c] / hbar
   double H[N * N];         // H / hbar
   double tdamp[N];         // (1 - delta_ic)(Delta_i + Delta_c)      Eq. 14 with Eq. 24
@@ -109,13 +109,12 @@ __global__ void __launch_bounds__(kKetThreads) rhs_ket_kernel(const __grid_const
     kr += fma(hd, v.x, ci);                                                  // -i (cr + i ci) = ci - i cr
     ki += fma(hd, v.y, -cr);
 
-    // ---- fused Taylor-form RK4 epilogue ----
+    // ---- fused Horner-form RK4 epilogue (R6): w' = y + ax k ----
     if (P.rhs_only) {
       P.out_acc[e] = make_double2(kr, ki);
     } else {
-      const double2 av = P.acc_in[e];
-      if (P.out_x) P.out_x[e] = make_double2(P.ax * kr, P.ax * ki);
-      P.out_acc[e] = make_double2(fma(P.bx, kr, av.x), fma(P.bx, ki, av.y));
+      const double2 yv = (P.y == P.x) ? v : P.y[e];
+      P.out_x[e] = make_double2(fma(P.ax, kr, yv.x), fma(P.ax, ki, yv.y));
     }
   }
 }
@@ -135,9 +134,9 @@ cudaError_t launch_ket_t(const RhsParams& p, const int32_t* links, int lrow, int
                          const double* a_minus_x, const double* a_minus_o, const double* H_host,
                          const double* delta_host, int sms, cudaStream_t s) {
   KetParams<N> P;
-  P.x = p.x; P.acc_in = p.acc_in; P.out_x = p.out_x; P.out_acc = p.out_acc;
+  P.x = p.x; P.y = p.y; P.out_x = p.out_x; P.out_acc = p.out_acc;
   P.links = links; P.lrow = lrow; P.nodes = p.nodes; P.M = p.M; P.col = col; P.rhs_only = p.rhs_only;
-  P.ax = p.ax; P.bx = p.bx;
+  P.ax = p.ax;
   P.hcc = H_host[col * N + col] * p.inv_hbar;
   for (int e = 0; e < N * N; ++e) P.H[e] = H_host[e] * p.inv_hbar;
   for (int e = 0; e < N; ++e) P.tdamp[e] = (e == col) ? 0.0 : delta_host[e] + delta_host[col];

@@ -150,7 +150,10 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
     if (warp == 0) {
       if (lane == 0) {
         next = draw();
-        if (next < nodes) lbulk_prefetch_l2(p.x + (size_t)next * NN, (unsigned)NN * 16);
+        if (next < nodes) {
+          lbulk_prefetch_l2(p.x + (size_t)next * NN, (unsigned)NN * 16);
+          if (p.horner && p.y != p.x) lbulk_prefetch_l2(p.y + (size_t)next * NN, (unsigned)NN * 16);
+        }
       }
       next = __shfl_sync(0xffffffffu, next, 0);
     }
@@ -280,33 +283,28 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
       if (p.rhs_only) {
 #pragma unroll
         for (int ct = 0; ct < CT; ++ct) p.out_acc[rbase + 4 * ct] = acc[rg][ct];
+      } else if (p.horner) {
+        // Horner stage (R6): w' = y + ax k; no running sum, nothing but y is loaded
+        double2 yv[CT];
+#pragma unroll
+        for (int ct = 0; ct < CT; ++ct) yv[ct] = p.y[rbase + 4 * ct];
+#pragma unroll
+        for (int ct = 0; ct < CT; ++ct) {
+          const double2 kv = acc[rg][ct];
+          p.out_x[rbase + 4 * ct] = make_double2(fma(p.ax, kv.x, yv[ct].x), fma(p.ax, kv.y, yv[ct].y));
+        }
       } else {
-        if (p.taylor && p.acc_red) {
-          // Taylor stage s >= 2: v_s = ax k is the next stage input and is added to the running sum by
-          // global reductions -- nothing is loaded, the traffic drains behind the next node's arithmetic
+        double2 yv[CT], av[CT];
 #pragma unroll
-          for (int ct = 0; ct < CT; ++ct) {
-            const double2 kv = acc[rg][ct];
-            if (p.out_x) p.out_x[rbase + 4 * ct] = make_double2(p.ax * kv.x, p.ax * kv.y);
-            double* dst = reinterpret_cast<double*>(p.out_acc + rbase + 4 * ct);
-            atomicAdd(dst, p.bx * kv.x);
-            atomicAdd(dst + 1, p.bx * kv.y);
-          }
-        } else {
-          double2 yv[CT], av[CT];
+        for (int ct = 0; ct < CT; ++ct) {
+          av[ct] = p.acc_in[rbase + 4 * ct];
+          if (p.out_x) yv[ct] = p.y[rbase + 4 * ct];
+        }
 #pragma unroll
-          for (int ct = 0; ct < CT; ++ct) {
-            av[ct] = p.acc_in[rbase + 4 * ct];
-            if (p.out_x && !p.taylor) yv[ct] = p.y[rbase + 4 * ct];
-          }
-#pragma unroll
-          for (int ct = 0; ct < CT; ++ct) {
-            const double2 kv = acc[rg][ct];
-            if (p.out_x)
-              p.out_x[rbase + 4 * ct] = p.taylor ? make_double2(p.ax * kv.x, p.ax * kv.y)
-                                                 : make_double2(fma(p.ax, kv.x, yv[ct].x), fma(p.ax, kv.y, yv[ct].y));
-            p.out_acc[rbase + 4 * ct] = make_double2(fma(p.bx, kv.x, av[ct].x), fma(p.bx, kv.y, av[ct].y));
-          }
+        for (int ct = 0; ct < CT; ++ct) {
+          const double2 kv = acc[rg][ct];
+          if (p.out_x) p.out_x[rbase + 4 * ct] = make_double2(fma(p.ax, kv.x, yv[ct].x), fma(p.ax, kv.y, yv[ct].y));
+          p.out_acc[rbase + 4 * ct] = make_double2(fma(p.bx, kv.x, av[ct].x), fma(p.bx, kv.y, av[ct].y));
         }
       }
     }
@@ -349,9 +347,15 @@ cudaError_t launch_large_t(const RhsParams& p, const int64_t* lptr, const int4* 
   if (grid < 1) grid = 1;
   P.tickets = tickets;
   P.ticket_base = *ticket_base;
-  *ticket_base += (unsigned long long)p.nodes + (unsigned long long)grid;   // one failing draw per CTA
   rhs_large_kernel<N><<<grid, C::THREADS, smem, s>>>(P);
-  return cudaGetLastError();
+  const cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) {
+    *ticket_base += (unsigned long long)p.nodes + (unsigned long long)grid;   // one failing draw per CTA
+  } else {                                 // nothing ran: keep host base and device counter in step
+    cudaMemsetAsync(tickets, 0, sizeof(unsigned long long), s);
+    *ticket_base = 0;
+  }
+  return e;
 }
 
 }  // namespace

@@ -64,19 +64,26 @@ class ShardedHeom:
 
     # -- propagation ----------------------------------------------------------------------------
     def exchange(self, stage):
-        """Refresh the ghost rows of the buffer the next stage reads."""
-        ptr = self.g.stage_output(stage)
-        buf = self.g.buffer_view(ptr)
-        if int(self.send_counts.sum()):
-            self.g.pack_halo(ptr, self._send.data_ptr())
-        halo_all_to_all(buf, self._send, self.n_owned, self.send_counts, self.recv_counts, self.group)
+        """Refresh the ghost rows of the buffer the next stage reads.  The library launches on the stream bound
+        with heom_bind_workspace; torch.distributed orders the NCCL collective against torch's CURRENT stream --
+        so the bound stream is made current here: the collective then runs after the pack kernel and before the
+        next stage kernel, whatever stream the caller is on."""
+        import torch
+        with torch.cuda.stream(self.g._stream):
+            ptr = self.g.stage_output(stage)
+            buf = self.g.buffer_view(ptr)
+            if int(self.send_counts.sum()):
+                self.g.pack_halo(ptr, self._send.data_ptr())
+            halo_all_to_all(buf, self._send, self.n_owned, self.send_counts, self.recv_counts, self.group)
 
     def rk4_steps(self, dt_fs, nsteps):
-        for _ in range(int(nsteps)):
-            for stage in range(4):
-                self.g.rk4_stage(dt_fs, stage)
-                if self.world > 1:
-                    self.exchange(stage)
+        import torch
+        with torch.cuda.stream(self.g._stream):
+            for _ in range(int(nsteps)):
+                for stage in range(4):
+                    self.g.rk4_stage(dt_fs, stage)
+                    if self.world > 1:
+                        self.exchange(stage)
 
     def populations(self):
         """Eq. 26 from the rank's copy of sigma_0 (rank 0 owns it: the root is the first node of the order; ranks

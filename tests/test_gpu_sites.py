@@ -37,7 +37,7 @@ CASES = [(2, [1], 1, 4), (3, [1, 2], 1, 3), (8, [1, 2, 3, 4, 5, 6, 7], 1, 3), (8
 
 
 @pytest.mark.parametrize("N,bath_state,K,D", CASES)
-@pytest.mark.parametrize("order,kernel", [(0, 1), (1, 1), (1, 2), (1, 0)])
+@pytest.mark.parametrize("order,kernel", [(0, 1), (1, 1), (1, 0)])
 def test_rhs_parity_site_map_random_state(N, bath_state, K, D, order, kernel):
     H, lam, nu = _system(N, bath_state, N + K + D)
     o, g = _pair(H, lam, nu, 150.0, K, D, bath_state, order=order, kernel=kernel)
@@ -50,7 +50,7 @@ def test_rhs_parity_site_map_random_state(N, bath_state, K, D, order, kernel):
     o.set_full_state(sth); g.set_full_state(sth)
     got = g.rhs()
     assert rel_err(got, o.rhs()) < RHS_TOL
-    if g.kernel_name() in ("rhs_hpipe_kernel", "rhs_herm_kernel"):
+    if g.kernel_name() == "rhs_hpipe_kernel":
         assert np.array_equal(got, np.conj(np.swapaxes(got, 1, 2)))
 
 

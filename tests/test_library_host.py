@@ -44,7 +44,7 @@ def test_tables_bit_exact_vs_oracle(N, K, D, order):
         assert a.dtype == b.dtype and np.array_equal(a, b)
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg4", "cfg5"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
 def test_tables_bit_exact_baseline_configs(name):
     w = workloads.get(name)
     o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D)
@@ -93,7 +93,7 @@ def test_option_validation_without_gpu():
         with pytest.raises(HeomError) as e:
             g.set_option(name, bad)
         assert e.value.status == -1
-    for name in ("timing", "hermitian", "acc_red", "pade"):
+    for name in ("timing", "hermitian", "ket", "pade"):
         g.set_option(name, 1)
         g.set_option(name, 0)
 

@@ -114,6 +114,8 @@ SURVEY_CHECKS = {
     (2, 1, 4): (5246, 2380, 13976, 122561, 6300, 122561),
     (7, 1, 8): (266843672200, 94646454840, 2067401366940, 8701842624013419,
                 709860620700, 3163845708648120),
+    (7, 1, 12): (307620673231800, 139078872118200, 2351115053793228, 10115670477738734324,
+                 1043092008913500, 4550830205369578669),          # cfg3: W = 14, D = 12, 9 657 700 nodes
     (96, 0, 3): (36002339968, 1084140288, 1983102012080, 107104809694540,
                  52602933936, 32955572434587),
 }
