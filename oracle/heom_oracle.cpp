@@ -25,6 +25,15 @@
  *   bath -> state
  *   map           : two-level absorber cumulant closed form; lambda = 0 per-site
  *                   equivalence; Eq. 48 block structure (tests/test_oracle_sites.py).
+ *   S(b) > 1, several baths per state, complex / time-dependent H
+ *   (oracle_create_general, oracle_set_hamiltonian, oracle_rk4_step_td;
+ *   tests/test_oracle_general.py): two-exciton coherences at J = 0 against the
+ *   product of one-exciton line shapes; a bath shared by two states (the shared
+ *   coupling cancels in their coherence; the printed and the operator form of the
+ *   Eq. 14 sum, R12, differ by exactly exp(-2 Delta t) there); gauge transform
+ *   H -> U H U^dagger with a diagonal unitary against the pinned real-H path;
+ *   lambda = 0 against scipy expm; resonantly driven two-level system (RWA) against
+ *   the rotating-frame Rabi formula.
  *   Parity unpinned: nothing in this file is without a pin, but configs 2-5 of
  *   BASELINE.json have no printed values anywhere (the paper prints none);
  *   they rest on the pins above evaluated at those shapes.
@@ -55,11 +64,18 @@ const double PI = 3.14159265358979323846;
 
 struct oracle_ctx {
   int N = 0;       /* system states (rows of every sigma_u)                   */
-  int B = 0;       /* baths; bath b couples to the projector |site[b]><site[b]|
-                      (S(b) = 1).  oracle_create: B = N, site[b] = b;
-                      oracle_create_sites: any injective map, e.g. a ground state
-                      without a bath for linear absorption      */
-  std::vector<int> site;        /* [B] bs(b): the state bath b couples to      */
+  int B = 0;       /* baths; bath b couples through the projectors |s><s| on the
+                      S(b) = bptr[b+1] - bptr[b] states bst[bptr[b]..] (P:84, P:119
+                      Eq. 18, Eq. 21).  oracle_create: B = N, one state each,
+                      bs(b) = b; oracle_create_sites: one state each, any injective
+                      map (a ground state without a bath);
+                      oracle_create_general: any lists ("multiple states can share
+                      one bath, or multiple baths can couple to the same state",
+                      P:84: the two-exciton manifold of Eq. 54)                */
+  std::vector<int> bptr;        /* [B+1] offsets into bst                       */
+  std::vector<int> bst;         /* states of every bath, bath after bath       */
+  int terminator_form = 0;      /* Eq. 14's sum over s: 0 = as printed,
+                                   sum_s V_s^x V_s^x; 1 = (sum_s V_s^x)^2 (R12)  */
   int K = 0;       /* Matsubara terms beyond the Drude pole                   */
   int M = 0;       /* modes per bath = K+1 = the paper's K             */
   int W = 0;       /* tuple length W = B*K_paper                        */
@@ -70,7 +86,11 @@ struct oracle_ctx {
   int threads = 0;
   int pade = 0;      /* 0 = Matsubara poles (Eq. 19-20), 1 = Pade poles (Eq. 27-33) */
   double T_kelvin = 0;
-  std::vector<double> H;        /* [N][N] cm^-1                               */
+  std::vector<double> H;        /* [N][N] cm^-1, real part (symmetric)         */
+  std::vector<double> Him;      /* [N][N] cm^-1, imaginary part (antisymmetric;
+                                   zero unless oracle_create_general /
+                                   oracle_set_hamiltonian gave one: RWA field
+                                   coupling, Eq. 51)                            */
   std::vector<double> lambda;   /* [B] cm^-1                                  */
   std::vector<double> nu;       /* [B] fs^-1                                  */
   double beta_hbar = 0;         /* beta*hbar = hbar/(k_B T), fs               */
@@ -309,7 +329,8 @@ inline double abs_c(const oracle_ctx* c, int l) {
 }
 
 /* ------------------------------------------------------------ right-hand side
- * d sigma_u / dt, Eq. 12-17, for one node u of the state `st`.               */
+ * d sigma_u / dt, Eq. 12-17, for one node u of the state `st`.  The sums over
+ * the S(b) states of a bath are written out as the paper prints them.        */
 void rhs_node(const oracle_ctx* c, const cplx* st, int64_t u, cplx* out) {
   const int N = c->N, M = c->M, W = c->W;
   const size_t NN = (size_t)N * N;
@@ -317,13 +338,13 @@ void rhs_node(const oracle_ctx* c, const cplx* st, int64_t u, cplx* out) {
   const cplx* s = st + (size_t)u * NN;
   const uint8_t* n = &c->tuples[(size_t)u * W];
 
-  /* Eq. 12:  -(i/hbar) [H, sigma_u] */
+  /* Eq. 12:  -(i/hbar) [H, sigma_u],  H = H_re + i H_im Hermitian */
   for (int i = 0; i < N; ++i)
     for (int j = 0; j < N; ++j) {
       cplx comm(0.0, 0.0);
       for (int m = 0; m < N; ++m)
-        comm += c->H[(size_t)i * N + m] * s[(size_t)m * N + j] -
-                s[(size_t)i * N + m] * c->H[(size_t)m * N + j];
+        comm += cplx(c->H[(size_t)i * N + m], c->Him[(size_t)i * N + m]) * s[(size_t)m * N + j] -
+                s[(size_t)i * N + m] * cplx(c->H[(size_t)m * N + j], c->Him[(size_t)m * N + j]);
       out[(size_t)i * N + j] = -(I / HBAR_CM_FS) * comm;
     }
 
@@ -332,33 +353,44 @@ void rhs_node(const oracle_ctx* c, const cplx* st, int64_t u, cplx* out) {
   for (int l = 0; l < W; ++l) damp += (double)n[l] * c->gamma[l];
   for (size_t e = 0; e < NN; ++e) out[e] -= damp * s[e];
 
-  /* Eq. 14:  - sum_b [ ... ] V_b^x V_b^x sigma_u   (S(b)=1, V_b = |bs(b)><bs(b)|) */
+  /* Eq. 14:  - sum_b sum_{s=1..S(b)} [ ... ] V_s^x V_s^x sigma_u  as printed (terminator_form 0), or with the
+   * operator of the bath squared, (sum_s V_s^x)^2 (terminator_form 1, R12); the same thing when S(b) = 1 */
   if (c->terminator)
     for (int b = 0; b < c->B; ++b)
       for (int i = 0; i < N; ++i)
-        for (int j = 0; j < N; ++j)
-          out[(size_t)i * N + j] -= c->delta[b] * VxVx(c->site[b], i, j) * s[(size_t)i * N + j];
+        for (int j = 0; j < N; ++j) {
+          double mask = 0.0;
+          if (c->terminator_form == 0) {
+            for (int q = c->bptr[b]; q < c->bptr[b + 1]; ++q) mask += VxVx(c->bst[q], i, j);
+          } else {
+            double v = 0.0;
+            for (int q = c->bptr[b]; q < c->bptr[b + 1]; ++q) v += Vx(c->bst[q], i, j);
+            mask = v * v;
+          }
+          out[(size_t)i * N + j] -= c->delta[b] * mask * s[(size_t)i * N + j];
+        }
 
-  /* Eq. 15 -> Eq. 35:  + sum_{b,k} i sqrt((n+1)|c|) V_b^x sigma^+_{(u,b,k)} */
+  /* Eq. 15 -> Eq. 35:  + sum_b sum_s sum_k i sqrt((n+1)|c|) V_s^x sigma^+_{(u,b,k)} */
   for (int l = 0; l < W; ++l) {
     const int32_t up = c->plus[(size_t)u * W + l];
     if (up < 0) continue; /* invalid link contributes nothing */
-    const int b = c->site[l / M];  /* Eq. 11, then bs(b) */
+    const int b = l / M;  /* Eq. 11 */
     const cplx* sp = st + (size_t)up * NN;
     const double f = c->scaling ? std::sqrt(((double)n[l] + 1.0) * abs_c(c, l)) : 1.0;
-    for (int i = 0; i < N; ++i)
-      for (int j = 0; j < N; ++j)
-        out[(size_t)i * N + j] += I * (f * Vx(b, i, j)) * sp[(size_t)i * N + j];
+    for (int q = c->bptr[b]; q < c->bptr[b + 1]; ++q)
+      for (int i = 0; i < N; ++i)
+        for (int j = 0; j < N; ++j)
+          out[(size_t)i * N + j] += I * (f * Vx(c->bst[q], i, j)) * sp[(size_t)i * N + j];
   }
 
-  /* Eq. 16-17 -> Eq. 36:  + sum_{b,k} sqrt(n/|c|) theta_MA(b,k) sigma^-_{(u,b,k)},
-   * theta_MA = i c V^x + delta_{k,0} (lambda_b nu_b / hbar) V^o.
+  /* Eq. 16-17 -> Eq. 36:  + sum_b sum_s sum_k sqrt(n/|c|) theta_MA(b,k) sigma^-_{(u,b,k)},
+   * theta_MA = i c V_s^x + delta_{k,0} (lambda_b nu_b / hbar) V_s^o.
    * Unscaled (Eq. 16) the prefactor is n.  |c| = 0 (lambda_b = 0): the bath is
    * decoupled and the term is dropped (limit of the printed 0/0). */
   for (int l = 0; l < W; ++l) {
     const int32_t um = c->minus[(size_t)u * W + l];
     if (um < 0) continue;
-    const int b = c->site[l / M], k = l % M;
+    const int b = l / M, k = l % M;
     const cplx* sm = st + (size_t)um * NN;
     double f;
     if (c->scaling) {
@@ -368,11 +400,12 @@ void rhs_node(const oracle_ctx* c, const cplx* st, int64_t u, cplx* out) {
       f = (double)n[l];
     }
     const double lam_nu = (k == 0) ? -c->c_im[l] : 0.0; /* lambda_b nu_b / hbar */
-    for (int i = 0; i < N; ++i)
-      for (int j = 0; j < N; ++j) {
-        const cplx theta = I * (c->c_re[l] * Vx(b, i, j)) + lam_nu * Vo(b, i, j);
-        out[(size_t)i * N + j] += f * theta * sm[(size_t)i * N + j];
-      }
+    for (int q = c->bptr[b]; q < c->bptr[b + 1]; ++q)
+      for (int i = 0; i < N; ++i)
+        for (int j = 0; j < N; ++j) {
+          const cplx theta = I * (c->c_re[l] * Vx(c->bst[q], i, j)) + lam_nu * Vo(c->bst[q], i, j);
+          out[(size_t)i * N + j] += f * theta * sm[(size_t)i * N + j];
+        }
   }
 }
 
@@ -386,27 +419,38 @@ void rhs_all(const oracle_ctx* c, const cplx* st, cplx* out) {
 
 extern "C" {
 
-int oracle_create_sites(oracle_ctx** out, int n_states, const double* H_cm, int n_baths,
-                        const int* bath_state, const double* lambda_cm, const double* nu_per_fs,
-                        double T_kelvin, int K, int D) {
-  if (!out || !H_cm || !lambda_cm || !nu_per_fs || !bath_state) return -1;
-  if (n_states < 1 || n_baths < 1 || n_baths > n_states || K < 0 || D < 0 || D > 255 || !(T_kelvin > 0.0)) return -1;
+int oracle_create_general(oracle_ctx** out, int n_states, const double* H_re_cm, const double* H_im_cm,
+                          int n_baths, const int* bath_ptr, const int* bath_states, const double* lambda_cm,
+                          const double* nu_per_fs, double T_kelvin, int K, int D) {
+  if (!out || !H_re_cm || !lambda_cm || !nu_per_fs || !bath_ptr || !bath_states) return -1;
+  if (n_states < 1 || n_baths < 1 || K < 0 || D < 0 || D > 255 || !(T_kelvin > 0.0)) return -1;
+  if (bath_ptr[0] != 0) return -1;
   for (int b = 0; b < n_baths; ++b) {
     if (!(lambda_cm[b] >= 0.0) || !(nu_per_fs[b] > 0.0)) return -1;
-    if (bath_state[b] < 0 || bath_state[b] >= n_states) return -1;
-    for (int b2 = 0; b2 < b; ++b2) if (bath_state[b2] == bath_state[b]) return -1;   /* one bath per state */
+    if (bath_ptr[b + 1] <= bath_ptr[b]) return -1;                       /* S(b) >= 1 */
+    for (int q = bath_ptr[b]; q < bath_ptr[b + 1]; ++q) {
+      if (bath_states[q] < 0 || bath_states[q] >= n_states) return -1;
+      for (int q2 = bath_ptr[b]; q2 < q; ++q2) if (bath_states[q2] == bath_states[q]) return -1;   /* a state once per bath */
+    }
   }
   for (int i = 0; i < n_states; ++i)
     for (int j = 0; j < n_states; ++j) {
-      if (!std::isfinite(H_cm[i * n_states + j])) return -1;
-      if (H_cm[i * n_states + j] != H_cm[j * n_states + i]) return -1;
+      if (!std::isfinite(H_re_cm[i * n_states + j])) return -1;
+      if (H_re_cm[i * n_states + j] != H_re_cm[j * n_states + i]) return -1;
+      if (H_im_cm) {
+        if (!std::isfinite(H_im_cm[i * n_states + j])) return -1;
+        if (H_im_cm[i * n_states + j] != -H_im_cm[j * n_states + i]) return -1;   /* Hermitian */
+      }
     }
   oracle_ctx* c = new (std::nothrow) oracle_ctx();
   if (!c) return -2;
   try {
     c->N = n_states; c->B = n_baths; c->K = K; c->M = K + 1; c->W = n_baths * (K + 1); c->D = D;
-    c->site.assign(bath_state, bath_state + n_baths);
-    c->H.assign(H_cm, H_cm + (size_t)n_states * n_states);
+    c->bptr.assign(bath_ptr, bath_ptr + n_baths + 1);
+    c->bst.assign(bath_states, bath_states + bath_ptr[n_baths]);
+    c->H.assign(H_re_cm, H_re_cm + (size_t)n_states * n_states);
+    c->Him.assign((size_t)n_states * n_states, 0.0);
+    if (H_im_cm) c->Him.assign(H_im_cm, H_im_cm + (size_t)n_states * n_states);
     c->lambda.assign(lambda_cm, lambda_cm + n_baths);
     c->nu.assign(nu_per_fs, nu_per_fs + n_baths);
     c->T_kelvin = T_kelvin;
@@ -422,6 +466,19 @@ int oracle_create_sites(oracle_ctx** out, int n_states, const double* H_cm, int 
   }
   *out = c;
   return 0;
+}
+
+/* One state per bath, all different: the S(b) = 1 special case of oracle_create_general. */
+int oracle_create_sites(oracle_ctx** out, int n_states, const double* H_cm, int n_baths,
+                        const int* bath_state, const double* lambda_cm, const double* nu_per_fs,
+                        double T_kelvin, int K, int D) {
+  if (!bath_state || n_baths < 1 || n_baths > n_states) return -1;
+  std::vector<int> ptr((size_t)n_baths + 1);
+  for (int b = 0; b <= n_baths; ++b) ptr[(size_t)b] = b;
+  for (int b = 0; b < n_baths; ++b)
+    for (int b2 = 0; b2 < b; ++b2) if (bath_state[b2] == bath_state[b]) return -1;   /* one bath per state */
+  return oracle_create_general(out, n_states, H_cm, nullptr, n_baths, ptr.data(), bath_state, lambda_cm,
+                               nu_per_fs, T_kelvin, K, D);
 }
 
 /* Per-site baths: one bath per state, bath b on state b (BASELINE.json's five configurations). */
@@ -440,6 +497,7 @@ int oracle_set_option(oracle_ctx* c, const char* name, int value) {
   const std::string s(name);
   if (s == "scaling") { if (value < 0 || value > 2) return -1; c->scaling = value; return 0; }
   if (s == "terminator") { c->terminator = value ? 1 : 0; return 0; }
+  if (s == "terminator_form") { if (value < 0 || value > 1) return -1; c->terminator_form = value; return 0; }
   if (s == "threads") { if (value < 0) return -1; c->threads = value; return 0; }
   if (s == "pade") { c->pade = value ? 1 : 0; return build_coefficients(c, c->T_kelvin); }
   return -1;
@@ -549,6 +607,49 @@ int oracle_rk4_steps(oracle_ctx* c, double dt, int nsteps) {
 #pragma omp parallel for schedule(static) num_threads(nt)
     for (size_t e = 0; e < total; ++e) { sum[e] += k[e]; y[e] += (dt / 6.0) * sum[e]; }
   }
+  return 0;
+}
+
+/* Replace the Hamiltonian (time-dependent H(t), Eq. 47-51: the caller evaluates the field). */
+int oracle_set_hamiltonian(oracle_ctx* c, const double* H_re_cm, const double* H_im_cm) {
+  if (!c || !H_re_cm) return -1;
+  const int N = c->N;
+  for (int i = 0; i < N; ++i)
+    for (int j = 0; j < N; ++j) {
+      if (!std::isfinite(H_re_cm[i * N + j]) || H_re_cm[i * N + j] != H_re_cm[j * N + i]) return -1;
+      if (H_im_cm && (!std::isfinite(H_im_cm[i * N + j]) || H_im_cm[i * N + j] != -H_im_cm[j * N + i])) return -1;
+    }
+  c->H.assign(H_re_cm, H_re_cm + (size_t)N * N);
+  c->Him.assign((size_t)N * N, 0.0);
+  if (H_im_cm) c->Him.assign(H_im_cm, H_im_cm + (size_t)N * N);
+  return 0;
+}
+
+/* One classical RK4 step of the NON-autonomous system d sigma/dt = L(H(t)) sigma:
+ *   k1 = f(t, y); k2 = f(t + dt/2, y + dt/2 k1); k3 = f(t + dt/2, y + dt/2 k2); k4 = f(t + dt, y + dt k3),
+ * with H(t), H(t + dt/2), H(t + dt) handed in (each as real and imaginary part; imaginary parts may be NULL).
+ * Leaves H(t + dt) set. */
+int oracle_rk4_step_td(oracle_ctx* c, double dt, const double* H0_re, const double* H0_im,
+                       const double* Hm_re, const double* Hm_im, const double* H1_re, const double* H1_im) {
+  if (!c || !std::isfinite(dt)) return -1;
+  if (!c->have_state) return -4;
+  const size_t total = c->y.size();
+  std::vector<cplx> x, k, sum;
+  try { x.resize(total); k.resize(total); sum.resize(total); }
+  catch (const std::bad_alloc&) { return -2; }
+  cplx* y = c->y.data();
+  int rc;
+  if ((rc = oracle_set_hamiltonian(c, H0_re, H0_im)) != 0) return rc;
+  rhs_all(c, y, k.data());                                     /* k1 */
+  for (size_t e = 0; e < total; ++e) { sum[e] = k[e]; x[e] = y[e] + (dt / 2.0) * k[e]; }
+  if ((rc = oracle_set_hamiltonian(c, Hm_re, Hm_im)) != 0) return rc;
+  rhs_all(c, x.data(), k.data());                              /* k2 */
+  for (size_t e = 0; e < total; ++e) { sum[e] += 2.0 * k[e]; x[e] = y[e] + (dt / 2.0) * k[e]; }
+  rhs_all(c, x.data(), k.data());                              /* k3 */
+  for (size_t e = 0; e < total; ++e) { sum[e] += 2.0 * k[e]; x[e] = y[e] + dt * k[e]; }
+  if ((rc = oracle_set_hamiltonian(c, H1_re, H1_im)) != 0) return rc;
+  rhs_all(c, x.data(), k.data());                              /* k4 */
+  for (size_t e = 0; e < total; ++e) { sum[e] += k[e]; y[e] += (dt / 6.0) * sum[e]; }
   return 0;
 }
 

@@ -46,6 +46,18 @@ int  oracle_create(oracle_ctx** out, int n_sites, const double* H_cm,
 int  oracle_create_sites(oracle_ctx** out, int n_states, const double* H_cm, int n_baths,
                          const int* bath_state, const double* lambda_cm, const double* nu_per_fs,
                          double T_kelvin, int K, int D);
+/* General system-bath operators ("Multiple states can share one bath, or multiple
+ * baths can couple to the same state (for instance a two-exciton state is coupled to two sites ...)"; the sums
+ * over s = 1..S(b) in Eq. 14-17; the two-exciton manifold of Eq. 54) and a complex Hermitian H (the
+ * RWA field coupling of Eq. 51):
+ *   bath b couples through the projectors on the S(b) = bath_ptr[b+1] - bath_ptr[b] >= 1 states
+ *   bath_states[bath_ptr[b] .. bath_ptr[b+1]) (0-based, a state at most once per bath; a state may appear in the
+ *   lists of several baths; bath_ptr[0] = 0);  H = H_re_cm + i H_im_cm, H_re symmetric, H_im antisymmetric
+ *   (H_im_cm may be NULL = real H).
+ * oracle_create_sites(...) == oracle_create_general with one state per bath. */
+int  oracle_create_general(oracle_ctx** out, int n_states, const double* H_re_cm, const double* H_im_cm,
+                           int n_baths, const int* bath_ptr, const int* bath_states, const double* lambda_cm,
+                           const double* nu_per_fs, double T_kelvin, int K, int D);
 void oracle_destroy(oracle_ctx* ctx);
 
 /* Options (set before any rhs/rk4 call; defaults in brackets):
@@ -53,6 +65,9 @@ void oracle_destroy(oracle_ctx* ctx);
  *               [1] = Eq. 35-36 with |c| = |Re c(b,k)|      (R5)
  *                2 = Eq. 35-36 with |c| = complex modulus of c(b,0)
  *   "terminator" [1] = Eq. 14 on, 0 = off
+ *   "terminator_form" the sum over the S(b) states of a bath in Eq. 14 (R12; no effect when S(b) = 1):
+ *               [0] = as printed, sum_s V_s^x V_s^x, mask (1 - delta_ij)(m_b(i) + m_b(j)), m_b = membership
+ *                1 = the bath's operator squared, (sum_s V_s^x)^2, mask (m_b(i) - m_b(j))^2
  *   "pade"       [0] = Matsubara poles and coefficients (Eq. 19-20), 1 = Pade (Eq. 27-33); rebuilds the
  *                coefficients, K keeps its meaning (number of poles beyond the Drude pole)
  *   "threads"    OpenMP threads for the loop over nodes [0 = runtime default];
@@ -91,6 +106,11 @@ int  oracle_rhs_nodes(oracle_ctx* ctx, const int64_t* node_ids, int64_t count,
                       double* out);
 /* Classical RK4, nsteps steps of dt_fs, in place. */
 int  oracle_rk4_steps(oracle_ctx* ctx, double dt_fs, int nsteps);
+/* Time-dependent H(t) (Eq. 47-51): replace the Hamiltonian (H_im_cm may be NULL) ... */
+int  oracle_set_hamiltonian(oracle_ctx* ctx, const double* H_re_cm, const double* H_im_cm);
+/* ... and one classical RK4 step of the non-autonomous system with H(t), H(t + dt/2), H(t + dt) handed in. */
+int  oracle_rk4_step_td(oracle_ctx* ctx, double dt_fs, const double* H0_re, const double* H0_im,
+                        const double* Hm_re, const double* Hm_im, const double* H1_re, const double* H1_im);
 /* Eq. 26: p_i = Re sigma_0[i][i], trace = sum_i sigma_0[i][i]. */
 int  oracle_populations(const oracle_ctx* ctx, double* pop, double* trace_re,
                         double* trace_im);

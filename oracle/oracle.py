@@ -27,6 +27,11 @@ def _load():
     lib.oracle_create_sites.argtypes = [C.POINTER(P), C.c_int, dp, C.c_int, C.POINTER(C.c_int), dp, dp,
                                         C.c_double, C.c_int, C.c_int]
     lib.oracle_create_sites.restype = C.c_int
+    lib.oracle_create_general.argtypes = [C.POINTER(P), C.c_int, dp, dp, C.c_int, C.POINTER(C.c_int),
+                                          C.POINTER(C.c_int), dp, dp, C.c_double, C.c_int, C.c_int]
+    lib.oracle_create_general.restype = C.c_int
+    lib.oracle_set_hamiltonian.argtypes = [P, dp, dp]
+    lib.oracle_rk4_step_td.argtypes = [P, C.c_double, dp, dp, dp, dp, dp, dp]
     lib.oracle_destroy.argtypes = [P]
     lib.oracle_destroy.restype = None
     lib.oracle_set_option.argtypes = [P, C.c_char_p, C.c_int]
@@ -65,17 +70,30 @@ class Oracle:
     """One truncated hierarchy on the CPU.  Arguments as heom_oracle.h."""
 
     def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, scaling=1, terminator=1,
-                 threads=0, pade=0, bath_state=None):
+                 threads=0, pade=0, bath_state=None, bath_states=None, terminator_form=0):
         """bath_state=None: one bath per state (oracle_create); else a list of the states the baths couple
-        to (oracle_create_sites), lambda_cm / nu_per_fs then have one entry per bath."""
+        to (oracle_create_sites), lambda_cm / nu_per_fs then have one entry per bath.
+        bath_states = list of lists: bath b couples to every state of bath_states[b] (oracle_create_general);
+        H_cm may then be complex Hermitian."""
         lib = _load()
-        H = np.ascontiguousarray(H_cm, dtype=np.float64)
+        Hc = np.asarray(H_cm)
+        H = np.ascontiguousarray(Hc.real, dtype=np.float64)
+        Him = np.ascontiguousarray(Hc.imag, dtype=np.float64) if np.iscomplexobj(Hc) else None
         self.N = H.shape[0]
-        self.B = self.N if bath_state is None else len(bath_state)
+        self.B = len(bath_states) if bath_states is not None else self.N if bath_state is None else len(bath_state)
         lam = np.ascontiguousarray(np.broadcast_to(lambda_cm, (self.B,)), dtype=np.float64)
         nu = np.ascontiguousarray(np.broadcast_to(nu_per_fs, (self.B,)), dtype=np.float64)
         h = C.c_void_p()
-        if bath_state is None:
+        if bath_states is not None or Him is not None:
+            if bath_states is None:
+                bath_states = [[b] for b in (range(self.N) if bath_state is None else bath_state)]
+            ptr = np.concatenate([[0], np.cumsum([len(x) for x in bath_states])]).astype(np.int32)
+            flat = np.array([s for x in bath_states for s in x], dtype=np.int32)
+            rc = lib.oracle_create_general(C.byref(h), self.N, _dptr(H), _dptr(Him) if Him is not None else None,
+                                           self.B, ptr.ctypes.data_as(C.POINTER(C.c_int)),
+                                           flat.ctypes.data_as(C.POINTER(C.c_int)), _dptr(lam), _dptr(nu),
+                                           float(T_kelvin), int(K), int(D))
+        elif bath_state is None:
             rc = lib.oracle_create(C.byref(h), self.N, _dptr(H), _dptr(lam), _dptr(nu),
                                    float(T_kelvin), int(K), int(D))
         else:
@@ -89,7 +107,8 @@ class Oracle:
         self.K, self.D = int(K), int(D)
         self.nodes = int(lib.oracle_num_nodes(h))
         self.W = int(lib.oracle_num_modes(h))
-        for name, v in (("scaling", scaling), ("terminator", terminator), ("threads", threads), ("pade", pade)):
+        for name, v in (("scaling", scaling), ("terminator", terminator), ("threads", threads), ("pade", pade),
+                        ("terminator_form", terminator_form)):
             self._ck(lib.oracle_set_option(h, name.encode(), int(v)))
 
     def _ck(self, rc):
@@ -149,6 +168,25 @@ class Oracle:
 
     def rk4_steps(self, dt_fs, nsteps):
         self._ck(self._lib.oracle_rk4_steps(self._h, float(dt_fs), int(nsteps)))
+
+    @staticmethod
+    def _parts(H):
+        Hc = np.asarray(H)
+        re = np.ascontiguousarray(Hc.real, dtype=np.float64)
+        im = np.ascontiguousarray(Hc.imag, dtype=np.float64) if np.iscomplexobj(Hc) else None
+        return re, im
+
+    def set_hamiltonian(self, H):
+        re, im = self._parts(H)
+        self._ck(self._lib.oracle_set_hamiltonian(self._h, _dptr(re), _dptr(im) if im is not None else None))
+
+    def rk4_step_td(self, dt_fs, H0, Hm, H1):
+        """One classical RK4 step with H(t) = H0, H(t + dt/2) = Hm, H(t + dt) = H1."""
+        parts = [self._parts(H) for H in (H0, Hm, H1)]
+        args = []
+        for re, im in parts:
+            args += [_dptr(re), _dptr(im) if im is not None else None]
+        self._ck(self._lib.oracle_rk4_step_td(self._h, float(dt_fs), *args))
 
     def populations(self):
         pop = np.empty(self.N)

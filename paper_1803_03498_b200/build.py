@@ -67,7 +67,7 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
 
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as pool:
         objs = list(pool.map(compile_one, sources()))
-    subprocess.run([nvcc, "--shared", "-o", LIB] + objs + ["-lgomp"], check=True)
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "--shared", "-o", LIB] + objs + ["-lgomp"], check=True)
     with open(tag, "w") as f:
         f.write(flags)
     return LIB

@@ -116,7 +116,7 @@ def test_dimer_1000_steps(kernel):
 
 
 @pytest.mark.parametrize("name,D,steps", [("cfg2", 4, 300), ("cfg3", 5, 100), ("cfg4", 4, 200),
-                                          ("cfg5", 1, 50), ("cfg5", 2, 10)])
+                                          ("cfg5", 1, 50), ("cfg5", 2, 3)])
 @pytest.mark.parametrize("order,kernel,herm,form", [(0, 1, 1, -1), (1, 1, 1, -1), (1, 1, 1, 0), (1, 1, 0, -1),
                                                     (1, 1, 0, 0), (1, 0, 0, -1)])
 def test_rk4_parity_reduced_depth(name, D, steps, order, kernel, herm, form):
