@@ -32,9 +32,9 @@ import workloads  # noqa: E402
 METRIC = "heom_node_updates_per_s"
 UNIT = "node-updates/s"
 # per_config: steps per chunk of the short runs of the non-headline configs
-SHORT_STEPS = {"cfg1": 1000, "cfg2": 200, "cfg3": 8, "cfg4": 50, "cfg5": 2, "absorb": 200}
+SHORT_STEPS = {"cfg1": 1000, "cfg2": 200, "cfg3": 8, "cfg4": 50, "cfg5": 2, "absorb": 200, "twoex": 50}
 SEEDS = {"cfg1": None, "cfg2": workloads.SEED_FMO, "cfg3": workloads.SEED_FMO, "cfg4": workloads.SEED_LHCII,
-         "cfg5": workloads.SEED_LARGE, "absorb": workloads.SEED_FMO}
+         "cfg5": workloads.SEED_LARGE, "absorb": workloads.SEED_FMO, "twoex": workloads.SEED_FMO}
 
 
 def measured_peaks():
@@ -117,7 +117,8 @@ def oracle_throughput(w, target_seconds=15.0):
     right-hand-side evaluations (oracle_rhs_nodes) of a seeded sample of nodes of the full hierarchy,
     i.e. node-updates without the RK4 combination."""
     from oracle.oracle import Oracle
-    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, bath_state=w.bath_state)
+    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, bath_state=w.bath_state,
+               bath_states=w.bath_states)
     o.set_state(w.sigma0())
     if w.state_bytes <= 2e9:
         t0 = time.perf_counter(); o.rk4_steps(w.dt_fs, 1); t1 = time.perf_counter() - t0
@@ -143,7 +144,8 @@ def run_reference(args, w):
         return
     # each "step" of the reference arm is a bounded sample: one oracle RK4 step of the full hierarchy
     from oracle.oracle import Oracle
-    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, bath_state=w.bath_state)
+    o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, bath_state=w.bath_state,
+               bath_states=w.bath_states)
     o.set_state(w.sigma0())
     t0 = time.perf_counter(); o.rk4_steps(w.dt_fs, 1); t1 = time.perf_counter() - t0
     budget = 150.0
@@ -166,6 +168,7 @@ def run_reference(args, w):
 
 def config_dict(w, key, n_gpus, shard=False):
     origin = (f"BASELINE.json configs[{list(workloads.CONFIGS).index(key)}]" if key in workloads.CONFIGS
+              else "two-exciton space of configs[1]'s H (29 states, P:471-481, Eq. 54; not a BASELINE config)" if key == "twoex"
               else "linear-absorption variant of configs[1] (ground state + 7 sites, sigma_0(0) = mu_z|0><0|; not a BASELINE config)")
     return {"workload": f"{w.name}: {origin} "
                         f"N={w.N} K={w.K} D={w.D} T={w.T_kelvin:g}K nodes={w.nodes} dt={w.dt_fs}fs",
@@ -203,7 +206,7 @@ def run_config(key, args, steps, ctx, with_e2e=True, with_cpu=True, options=None
                         bath_state=w.bath_state, **opts)
     else:
         g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, device=local_rank, bath_state=w.bath_state,
-                 **opts)
+                 bath_states=w.bath_states, **opts)
     g.bind(stream=stream)
     if w.sigma0_matrix is None and not shard:
         sigma0 = replicas.replica_sigma0(w, rank)
@@ -281,7 +284,8 @@ def run_config(key, args, steps, ctx, with_e2e=True, with_cpu=True, options=None
 
     peaks, which = measured_peaks()
     value = 4.0 * w.nodes * steps * job / (ms * 1e-3)
-    horner = kernel_name in ("rhs_hpipe_kernel", "rhs_hpipe_general_kernel", "rhs_large_kernel", "rhs_ket_kernel") \
+    horner = kernel_name in ("rhs_hpipe_kernel", "rhs_hpipe_general_kernel", "rhs_large_kernel", "rhs_ket_kernel",
+                             "rhs_mma_kernel") \
         and opts.get("rk4_form", -1) != 0
     # fused classical RK4 moves 16 state sizes per step = 64 N^2 bytes per node-update; the Horner form
     # the kernels run by default (R6) moves 2 + 3 + 3 + 3 = 11 state sizes = 44 N^2 bytes per node-update

@@ -71,6 +71,28 @@ heom_status heom_create(heom_ctx** out, int n_sites, const double* H_cm,
 heom_status heom_create_sites(heom_ctx** out, int n_states, const double* H_cm, int n_baths,
                               const int* bath_state, const double* lambda_cm, const double* nu_per_fs,
                               double T_kelvin, int K, int D, int device);
+/* General system-bath operators and complex H.  P:84: "Multiple states can share one bath,
+ * or multiple baths can couple to the same state (for instance a two-exciton state is coupled to two sites ...)":
+ * the sums over s = 1..S(b) of Eq. 14-17; the two-exciton manifold of Eq. 54 (P:279-281,
+ * N_states = 1 + N + N(N-1)/2); the RWA field coupling of Eq. 51, which makes H complex Hermitian.
+ *   bath_ptr    HOST [n_baths+1], bath_ptr[0] = 0, increasing: bath b couples through the projectors on the
+ *               S(b) = bath_ptr[b+1] - bath_ptr[b] >= 1 states bath_states[bath_ptr[b] .. bath_ptr[b+1])
+ *   bath_states HOST, 0-based; a state at most once per bath; a state may be listed by several baths
+ *   H_re_cm     HOST [n_states][n_states] symmetric; H_im_cm HOST antisymmetric or NULL (real H).  A context
+ *               created with H_im_cm != NULL accepts complex Hamiltonians in heom_set_hamiltonian later.
+ * n_states <= 96.  With one state per bath, all different, and H_im_cm = NULL this IS heom_create_sites (same
+ * kernels); otherwise the general kernels run (kernels_mma.cu for 17 <= n_states <= 96, else the generic kernel),
+ * one GPU.  Option "terminator_form" (below) selects how Eq. 14 sums over the states of a bath (R12).
+ * Errors: bad lists, non-Hermitian H -> HEOM_EINVAL. */
+heom_status heom_create_general(heom_ctx** out, int n_states, const double* H_re_cm, const double* H_im_cm,
+                                int n_baths, const int* bath_ptr, const int* bath_states, const double* lambda_cm,
+                                const double* nu_per_fs, double T_kelvin, int K, int D, int device);
+/* Replace the Hamiltonian: time-dependent H(t) (Eq. 47-51; the caller evaluates the field).  HOST arrays as
+ * above; H_im_cm != NULL needs a context created by heom_create_general with H_im_cm != NULL.  Stream-ordered:
+ * launches enqueued before the call use the old H.  A time-dependent RK4 step is heom_set_hamiltonian(H(t));
+ * heom_rk4_stage(dt, 0); heom_set_hamiltonian(H(t + dt/2)); stages 1, 2; heom_set_hamiltonian(H(t + dt)); stage 3,
+ * with option "rk4_form" = 0 (the Horner form holds for a time-independent H only). */
+heom_status heom_set_hamiltonian(heom_ctx* ctx, const double* H_re_cm, const double* H_im_cm);
 void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
 
 /* Options, to be set before heom_bind_workspace:
@@ -82,6 +104,10 @@ void heom_destroy(heom_ctx* ctx); /* NULL-safe; does not free the workspace */
  *   "pade"    0 (default) = Matsubara poles and coefficients (Eq. 19-20); 1 = Pade poles (P:148-176
  *             Eq. 27-33, R11): the K poles beyond the Drude pole become xi_k/(beta hbar) with weights eta_k.
  *             Rebuilds the coefficients (heom_get_coefficients reports them)
+ *   "terminator_form" how Eq. 14 sums over the S(b) states of a bath (R12; no effect when S(b) = 1):
+ *             0 (default) = as printed, sum_s V_s^x V_s^x, i.e. the mask (1 - delta_ij)(q_b(i) + q_b(j)) with q_b the
+ *             0/1 membership of the bath's state set; 1 = the bath's operator squared, (sum_s V_s^x)^2, i.e. the mask
+ *             (q_b(i) - q_b(j))^2
  *   "l2_fetch" cudaLimitMaxL2FetchGranularity to request (32, 64, 128), 0 = leave it
  * and at any time:
  *   "rk4_form" how heom_rk4_steps groups the classical RK4 step (R6): 0 = the four

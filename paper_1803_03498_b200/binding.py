@@ -23,7 +23,7 @@ SYMBOLS = [
     "heom_get_tables", "heom_get_coefficients", "heom_workspace_bytes", "heom_bind_workspace",
     "heom_set_state", "heom_set_full_state", "heom_get_full_state", "heom_rhs", "heom_rk4_steps",
     "heom_sync", "heom_populations", "heom_launch_count", "heom_kernel_time", "heom_kernel_name",
-    "heom_last_error", "heom_probe_peak",
+    "heom_last_error", "heom_probe_peak", "heom_create_general", "heom_set_hamiltonian",
 ]
 
 _lib = None
@@ -52,6 +52,9 @@ def load_library():
                                       C.c_int, C.c_int, C.c_int]
     lib.heom_create_partition.argtypes = [C.POINTER(P), C.c_int, dp, C.c_int, C.POINTER(C.c_int), dp, dp, C.c_double,
                                           C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
+    lib.heom_create_general.argtypes = [C.POINTER(P), C.c_int, dp, dp, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int),
+                                        dp, dp, C.c_double, C.c_int, C.c_int, C.c_int]
+    lib.heom_set_hamiltonian.argtypes = [P, dp, dp]
     lib.heom_partition_owned.argtypes = [P]
     lib.heom_partition_owned.restype = C.c_int64
     lib.heom_partition_plan.argtypes = [P, P, P, P, P]
@@ -109,22 +112,37 @@ class Heom:
     """One truncated hierarchy bound to one GPU stream.  Mirrors include/heom.h one to one."""
 
     def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, device=0, bath_state=None, partition=None,
-                 **options):
+                 bath_states=None, **options):
         """bath_state=None: heom_create (one bath per state); else heom_create_sites with the listed states
         (lambda_cm, nu_per_fs then have one entry per bath).  partition=(rank, world): heom_create_partition --
-        this context holds rank's part of the hierarchy (owned + ghost nodes)."""
+        this context holds rank's part of the hierarchy (owned + ghost nodes).
+        bath_states = list of lists (bath b couples to every state of bath_states[b]) and/or a complex H_cm:
+        heom_create_general."""
         self._lib = load_library()
         self._h = None
-        H = np.ascontiguousarray(H_cm, dtype=np.float64)
+        Hc = np.asarray(H_cm)
+        H = np.ascontiguousarray(Hc.real, dtype=np.float64)
+        Him = np.ascontiguousarray(Hc.imag, dtype=np.float64) if np.iscomplexobj(Hc) else None
         if H.ndim != 2 or H.shape[0] != H.shape[1]:
             raise ValueError("H_cm must be square")
         self.N = H.shape[0]
-        self.B = self.N if bath_state is None else len(bath_state)
+        self.B = len(bath_states) if bath_states is not None else self.N if bath_state is None else len(bath_state)
         lam = np.ascontiguousarray(np.broadcast_to(lambda_cm, (self.B,)), dtype=np.float64)
         nu = np.ascontiguousarray(np.broadcast_to(nu_per_fs, (self.B,)), dtype=np.float64)
         h = C.c_void_p()
         self.partition = partition
-        if partition is not None:
+        if bath_states is not None or Him is not None:
+            if partition is not None:
+                raise ValueError("general contexts are single-GPU")
+            if bath_states is None:
+                bath_states = [[b] for b in (range(self.N) if bath_state is None else bath_state)]
+            ptr = np.concatenate([[0], np.cumsum([len(x) for x in bath_states])]).astype(np.int32)
+            flat = np.array([int(q) for x in bath_states for q in x], dtype=np.int32)
+            rc = self._lib.heom_create_general(C.byref(h), self.N, _dptr(H), _dptr(Him) if Him is not None else None,
+                                               self.B, ptr.ctypes.data_as(C.POINTER(C.c_int)),
+                                               flat.ctypes.data_as(C.POINTER(C.c_int)), _dptr(lam), _dptr(nu),
+                                               float(T_kelvin), int(K), int(D), int(device))
+        elif partition is not None:
             states = list(range(self.N)) if bath_state is None else bath_state
             bs = (C.c_int * self.B)(*[int(x) for x in states])
             rc = self._lib.heom_create_partition(C.byref(h), self.N, _dptr(H), self.B, bs, _dptr(lam), _dptr(nu),
@@ -246,6 +264,20 @@ class Heom:
 
     def rk4_steps(self, dt_fs, nsteps):
         self._ck(self._lib.heom_rk4_steps(self._h, float(dt_fs), int(nsteps)))
+
+    def set_hamiltonian(self, H_cm):
+        """heom_set_hamiltonian: replace H (complex Hermitian allowed on contexts created with a complex H)."""
+        Hc = np.asarray(H_cm)
+        re = np.ascontiguousarray(Hc.real, dtype=np.float64)
+        im = np.ascontiguousarray(Hc.imag, dtype=np.float64) if np.iscomplexobj(Hc) else None
+        self._ck(self._lib.heom_set_hamiltonian(self._h, _dptr(re), _dptr(im) if im is not None else None))
+
+    def rk4_step_td(self, dt_fs, H0, Hm, H1):
+        """One RK4 step with a time-dependent Hamiltonian H(t) = H0, H(t + dt/2) = Hm, H(t + dt) = H1 (heom.h:
+        heom_set_hamiltonian + heom_rk4_stage; needs option rk4_form = 0).  Argument marshalling only."""
+        self.set_hamiltonian(H0); self.rk4_stage(dt_fs, 0)
+        self.set_hamiltonian(Hm); self.rk4_stage(dt_fs, 1); self.rk4_stage(dt_fs, 2)
+        self.set_hamiltonian(H1); self.rk4_stage(dt_fs, 3)
 
     def sync(self):
         self._ck(self._lib.heom_sync(self._h))

@@ -25,6 +25,18 @@ struct heom_ctx {
   std::vector<int> site;            // [B] state of bath b
   std::vector<int> bath_of;         // [N] bath of state s, -1 = none
   Coefficients cd;                  // the same coefficients in the kernels' per-state mode indexing [Wd] / [N]
+  // General system-bath operators (heom_create_general): bath b couples through the projectors on the states
+  // bst[bptr[b]..bptr[b+1]) (the sums over s of Eq. 14-17), H may be complex Hermitian (Eq. 51).  Such a
+  // context keeps the HOST mode indexing on the device (l = b*M + k, Wd = B*M) and runs the general kernels.
+  bool general = false;             // = need_general || (mma_opt == 1 && eligible)
+  bool need_general = false;        // the lists or a complex H ask for it
+  int mma_opt = -1;                 // option "mma": -1 auto, 0 never for site-map contexts, 1 whenever eligible
+  std::vector<int> bptr, bst;       // bath -> states (always filled)
+  std::vector<int> sptr, sbl;       // state -> baths (CSR)
+  std::vector<uint32_t> bmask;      // [B][4] membership bits of the bath's states
+  bool use_mma = false;
+  std::vector<double> Him;          // [N][N] imaginary part of H (general contexts created with one; else empty)
+  int terminator_form = 0;          // option "terminator_form" (R12)
   std::vector<double> lambda, nu;   // bath parameters (kept for the "pade" option)
   double T_kelvin = 0;
   int pade = 0;
@@ -59,6 +71,9 @@ struct heom_ctx {
   int64_t* d_lptr = nullptr;
   void* d_lent = nullptr;
   double *d_Hs = nullptr, *d_delta = nullptr;
+  double* d_Him = nullptr;          // general contexts: imaginary part of H (cm^-1)
+  int32_t *d_sptr = nullptr, *d_sbl = nullptr;
+  uint32_t* d_bmask = nullptr;
   double2* d_A = nullptr;    // operator of heom_expectation
   // column-sparse states (kernels_ket.cu): sigma_u = v_u e_col^T, selected by heom_set_state after an exact check
   int ket_opt = 1;           // option "ket": 1 = use the column kernel when the conditions hold, 0 = never
@@ -102,13 +117,29 @@ heom_status cuda_fail(heom_ctx* c, cudaError_t e, const char* where) {
     if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);       \
   } while (0)
 
-int dev_modes(const heom_ctx* c) { return c->h.N * c->h.M; }
+int dev_modes(const heom_ctx* c) { return c->general ? c->h.W : c->h.N * c->h.M; }
 // storage slot of the hierarchy's root node sigma_0 (-1: a partition that does not hold it)
 int64_t root_slot(const heom_ctx* c) { return c->partitioned ? c->part.root : (int64_t)c->h.slot_of[0]; }   // Wd: mode columns of the device tables
 
 // c->cd, c->Tterm from c->c and the bath -> state map
 void expand_coefficients(heom_ctx* c) {
   const int N = c->h.N, M = c->h.M, D1 = c->h.D + 1, Wd = N * M;
+  if (c->general) {
+    // host mode indexing on the device; Eq. 14's mask from the membership q_b of every bath: as printed
+    // sum_s V_s^x V_s^x = (1 - delta_ij)(q_b(i) + q_b(j)), or (sum_s V_s^x)^2 = (q_b(i) - q_b(j))^2 (R12)
+    c->cd = c->c;
+    c->Tterm.assign((size_t)N * N, 0.0);
+    for (int b = 0; b < c->B; ++b) {
+      std::vector<int> q((size_t)N, 0);
+      for (int e = c->bptr[(size_t)b]; e < c->bptr[(size_t)b + 1]; ++e) q[(size_t)c->bst[(size_t)e]] = 1;
+      for (int i = 0; i < N; ++i)
+        for (int j = 0; j < N; ++j) {
+          const int m = c->terminator_form ? (q[i] - q[j]) * (q[i] - q[j]) : (i != j) * (q[i] + q[j]);
+          c->Tterm[(size_t)i * N + j] += c->c.delta[(size_t)b] * m;
+        }
+    }
+    return;
+  }
   Coefficients& d = c->cd;
   d.beta_hbar = c->c.beta_hbar;
   d.gamma.assign((size_t)Wd, 0.0); d.c_re.assign((size_t)Wd, 0.0); d.c_im.assign((size_t)Wd, 0.0);
@@ -134,6 +165,16 @@ void expand_coefficients(heom_ctx* c) {
       if (i != j) c->Tterm[(size_t)i * N + j] = d.delta[(size_t)i] + d.delta[(size_t)j];  // Eq. 14 + 24
 }
 
+// site-map contexts may run in the general representation (host mode indexing, membership bits) to reach the
+// tensor-core kernel of kernels_mma.cu; partitions keep the per-state representation
+void update_general(heom_ctx* c) {
+  const int N = c->h.N;
+  const bool eligible = !c->partitioned && N >= 17 && N <= 96 && !c->bmask.empty();
+  const bool want = c->mma_opt == 1 || (c->mma_opt == -1 && !large_supported(N, N * c->h.M));
+  c->general = c->need_general || (eligible && want);
+  expand_coefficients(c);
+}
+
 bool ensure_hierarchy(heom_ctx* c) {
   if (c->hierarchy_built && c->built_order == c->order) return true;
   std::string err;
@@ -151,20 +192,21 @@ int node_stride(int N) { return N * N; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_linksP, off_Hs, off_delta, off_A, off_S0, off_send, off_lptr, off_lent, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_linksP, off_Hs, off_delta, off_Him, off_gen, off_A, off_S0, off_send, off_lptr, off_lent, total;
 };
 
 // Which kernel family the bound configuration will run (fixed by the shape and the "kernel" option), so that the
 // workspace holds the link tables of that family only (config 3: 1.1 GB of plain tables against 1.7 GB of meta rows).
-struct KernelChoice { bool hpipe, large, tiny, plain_tables; };
+struct KernelChoice { bool hpipe, large, tiny, mma, plain_tables; };
 KernelChoice kernel_choice(const heom_ctx* c) {
   KernelChoice k{};
   const int N = c->h.N, Wd = dev_modes(c), D = c->h.D;
   const long long nodes = (long long)c->h.nodes;
-  k.large = c->kernel >= 1 && large_supported(N, Wd);
-  k.hpipe = c->kernel >= 1 && hpipe_supported(N, Wd, D, nodes);
-  k.tiny = c->kernel == 1 && !c->partitioned && tiny_supported(N, Wd, D, nodes);
-  k.plain_tables = k.tiny || !(k.large || k.hpipe);   // plus/minus/tuples [nodes][W]: generic and tiny kernels
+  k.large = c->kernel >= 1 && !c->general && large_supported(N, Wd);
+  k.hpipe = c->kernel >= 1 && !c->general && hpipe_supported(N, Wd, D, nodes);
+  k.tiny = c->kernel == 1 && !c->general && !c->partitioned && tiny_supported(N, Wd, D, nodes);
+  k.mma = c->kernel >= 1 && c->general && mma_supported(N, Wd, c->B, !c->Him.empty());
+  k.plain_tables = k.tiny || !(k.large || k.hpipe || k.mma);   // plus/minus/tuples [nodes][W]: generic and tiny kernels
   return k;
 }
 
@@ -193,10 +235,12 @@ Layout layout_of(const heom_ctx* c) {
   L.off_linksP = o; o += align_up(kc.hpipe ? nodes * (size_t)hpipe_links_row((int)N, c->h.M) * 4 : 0);
   L.off_Hs = o; o += align_up(N * N * 8);
   L.off_delta = o; o += align_up(N * 8);
+  L.off_Him = o; o += align_up(N * N * 8);
+  L.off_gen = o; o += align_up((N + 1) * 4) + align_up(c->sbl.size() * 4 + 16) + align_up((size_t)c->B * 16 + 16);
   L.off_A = o; o += align_up(N * N * 16);
   L.off_S0 = o; o += align_up(N * N * 16);
   L.off_send = o; o += align_up(c->part.send_idx.size() * 4 + 16);
-  if (kc.large) {
+  if (kc.large || kc.mma) {
     // CSR link list: one 16-byte entry per valid "+" and per valid "-" link (a partition's table has links for its
     // owned rows only, so the two counts differ there)
     size_t links = 0;
@@ -219,6 +263,10 @@ RhsParams base_params(const heom_ctx* c) {
   p.H = c->d_H; p.Tterm = c->d_T; p.damp = c->d_damp;
   p.plus = c->d_plus; p.minus = c->d_minus; p.tuples = c->d_tuples;
   p.a_plus = c->d_ap; p.a_minus_x = c->d_amx; p.a_minus_o = c->d_amo;
+  if (c->general) {
+    p.gen = 1; p.B = c->B; p.sptr = c->d_sptr; p.sbl = c->d_sbl; p.bmask = c->d_bmask;
+    p.Him = c->Him.empty() ? nullptr : c->d_Him;
+  }
   return p;
 }
 
@@ -239,6 +287,9 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
   if (ctx->ket_col >= 0)
     CU(launch_rhs_ket(p, ctx->d_linksP, ctx->lrowP, ctx->ket_col, ctx->cd.a_plus.data(), ctx->cd.a_minus_x.data(),
                       ctx->cd.a_minus_o.data(), ctx->H.data(), ctx->cd.delta.data(), ctx->sms, ctx->stream));
+  else if (ctx->use_mma)
+    CU(launch_rhs_mma(p, ctx->d_lptr, ctx->d_lent, ctx->cd.a_plus.data(), ctx->cd.a_minus_x.data(),
+                      ctx->cd.a_minus_o.data(), ctx->sms, ctx->d_tickets, &ctx->ticket_base, ctx->stream));
   else if (ctx->use_large)
     CU(launch_rhs_large(p, ctx->d_lptr, ctx->d_lent, ctx->d_Hs, ctx->d_delta, ctx->cd.a_plus.data(),
                         ctx->cd.a_minus_x.data(), ctx->cd.a_minus_o.data(), ctx->sms, ctx->d_tickets,
@@ -283,7 +334,7 @@ heom_status sigma0_matrix(heom_ctx* ctx, const double2** out) {
 heom_status launch_stage(heom_ctx* ctx, double dt, int stage) {
   RhsParams p = base_params(ctx);
   p.rhs_only = 0;
-  const bool horner = (ctx->use_large || ctx->use_hpipe) && ctx->rk4_form != 0;
+  const bool horner = (ctx->use_large || ctx->use_hpipe || ctx->use_mma) && ctx->rk4_form != 0;
   p.x = stage == 0 ? ctx->y : (stage == 2 ? ctx->xb : ctx->xa);
   p.y = ctx->y;
   if (horner) {
@@ -306,34 +357,68 @@ heom_status launch_stage(heom_ctx* ctx, double dt, int stage) {
 
 extern "C" {
 
-static heom_status create_impl(heom_ctx** out, int n_states, const double* H_cm, int n_baths, const int* bath_state,
-                               const double* lambda_cm, const double* nu_per_fs, double T_kelvin, int K, int D,
-                               int device, int rank, int world) {
+static heom_status create_impl(heom_ctx** out, int n_states, const double* H_cm, const double* H_im_cm, int n_baths,
+                               const int* bath_ptr, const int* bath_states, const double* lambda_cm,
+                               const double* nu_per_fs, double T_kelvin, int K, int D, int device, int rank, int world) {
   if (!out) return HEOM_EINVAL;
   *out = nullptr;
   if (world < 0 || (world > 0 && (rank < 0 || rank >= world))) return HEOM_EINVAL;
-  if (!H_cm || !lambda_cm || !nu_per_fs || !bath_state || n_states < 1 || n_baths < 1 || n_baths > n_states ||
+  if (!H_cm || !lambda_cm || !nu_per_fs || !bath_ptr || !bath_states || n_states < 1 || n_baths < 1 ||
       K < 0 || D < 0 || D > 255 || device < 0)
     return HEOM_EINVAL;
   for (int i = 0; i < n_states; ++i)
     for (int j = 0; j < n_states; ++j) {
       const double a = H_cm[(size_t)i * n_states + j], b = H_cm[(size_t)j * n_states + i];
       if (!std::isfinite(a) || a != b) return HEOM_EINVAL;
+      if (H_im_cm) {
+        const double c = H_im_cm[(size_t)i * n_states + j], d = H_im_cm[(size_t)j * n_states + i];
+        if (!std::isfinite(c) || c != -d) return HEOM_EINVAL;                      // Hermitian
+      }
     }
+  if (bath_ptr[0] != 0) return HEOM_EINVAL;
   std::vector<int> bath_of((size_t)n_states, -1);
+  bool general = H_im_cm != nullptr;
   for (int b = 0; b < n_baths; ++b) {
-    const int s = bath_state[b];
-    if (s < 0 || s >= n_states || bath_of[(size_t)s] >= 0) return HEOM_EINVAL;   // one bath per state at most
-    bath_of[(size_t)s] = b;
+    if (bath_ptr[b + 1] <= bath_ptr[b]) return HEOM_EINVAL;                        // S(b) >= 1
+    if (bath_ptr[b + 1] - bath_ptr[b] > 1) general = true;
+    for (int e = bath_ptr[b]; e < bath_ptr[b + 1]; ++e) {
+      const int s = bath_states[e];
+      if (s < 0 || s >= n_states) return HEOM_EINVAL;
+      for (int e2 = bath_ptr[b]; e2 < e; ++e2) if (bath_states[e2] == s) return HEOM_EINVAL;   // a state once per bath
+      if (bath_of[(size_t)s] >= 0) general = true;                                 // several baths on one state
+      bath_of[(size_t)s] = b;
+    }
   }
+  if (general && (world > 0 || n_states > 128)) return HEOM_EINVAL;   // general contexts: one GPU, 128 membership bits
   heom_ctx* c = new (std::nothrow) heom_ctx();
   if (!c) return HEOM_ENOMEM;
   c->device = device;
   c->partitioned = world > 0;
   c->part_rank = rank; c->part_world = world > 0 ? world : 1;
   c->B = n_baths;
-  c->site.assign(bath_state, bath_state + n_baths);
-  c->bath_of = bath_of;
+  c->general = c->need_general = general;
+  c->bptr.assign(bath_ptr, bath_ptr + n_baths + 1);
+  c->bst.assign(bath_states, bath_states + bath_ptr[n_baths]);
+  if (!general) {
+    c->site.assign(bath_states, bath_states + n_baths);
+    c->bath_of = bath_of;
+  }
+  if (n_states <= 128) {
+    std::vector<std::vector<int>> of((size_t)n_states);
+    c->bmask.assign((size_t)n_baths * 4, 0u);
+    for (int b = 0; b < n_baths; ++b)
+      for (int e = bath_ptr[b]; e < bath_ptr[b + 1]; ++e) {
+        const int s = bath_states[e];
+        of[(size_t)s].push_back(b);
+        c->bmask[(size_t)b * 4 + (s >> 5)] |= 1u << (s & 31);
+      }
+    c->sptr.assign(1, 0);
+    for (int s = 0; s < n_states; ++s) {
+      c->sbl.insert(c->sbl.end(), of[(size_t)s].begin(), of[(size_t)s].end());
+      c->sptr.push_back((int)c->sbl.size());
+    }
+    if (H_im_cm) c->Him.assign(H_im_cm, H_im_cm + (size_t)n_states * n_states);
+  }
   c->h.N = n_states; c->h.K = K; c->h.M = K + 1; c->h.W = n_baths * (K + 1); c->h.D = D;
   std::string err;
   if (!build_coefficients(n_baths, K, D, lambda_cm, nu_per_fs, T_kelvin, 0, c->c, err)) {
@@ -344,7 +429,7 @@ static heom_status create_impl(heom_ctx** out, int n_states, const double* H_cm,
   c->nu.assign(nu_per_fs, nu_per_fs + n_baths);
   c->T_kelvin = T_kelvin;
   c->H.assign(H_cm, H_cm + (size_t)n_states * n_states);
-  expand_coefficients(c);
+  update_general(c);
   if (!ensure_hierarchy(c)) {
     const bool oom = c->err.find("memory") != std::string::npos;
     delete c;
@@ -354,17 +439,37 @@ static heom_status create_impl(heom_ctx** out, int n_states, const double* H_cm,
   return HEOM_OK;
 }
 
+static heom_status create_sites_impl(heom_ctx** out, int n_states, const double* H_cm, int n_baths,
+                                     const int* bath_state, const double* lambda_cm, const double* nu_per_fs,
+                                     double T_kelvin, int K, int D, int device, int rank, int world) {
+  if (out) *out = nullptr;
+  if (!bath_state || n_baths < 1 || n_baths > n_states) return HEOM_EINVAL;
+  std::vector<int> ptr((size_t)n_baths + 1);
+  for (int b = 0; b <= n_baths; ++b) ptr[(size_t)b] = b;
+  for (int b = 0; b < n_baths; ++b)
+    for (int b2 = 0; b2 < b; ++b2) if (bath_state[b2] == bath_state[b]) return HEOM_EINVAL;   // one bath per state at most
+  return create_impl(out, n_states, H_cm, nullptr, n_baths, ptr.data(), bath_state, lambda_cm, nu_per_fs, T_kelvin, K, D,
+                     device, rank, world);
+}
+
 heom_status heom_create_sites(heom_ctx** out, int n_states, const double* H_cm, int n_baths, const int* bath_state,
                               const double* lambda_cm, const double* nu_per_fs, double T_kelvin, int K, int D,
                               int device) {
-  return create_impl(out, n_states, H_cm, n_baths, bath_state, lambda_cm, nu_per_fs, T_kelvin, K, D, device, 0, 0);
+  return create_sites_impl(out, n_states, H_cm, n_baths, bath_state, lambda_cm, nu_per_fs, T_kelvin, K, D, device, 0, 0);
+}
+
+heom_status heom_create_general(heom_ctx** out, int n_states, const double* H_re_cm, const double* H_im_cm, int n_baths,
+                                const int* bath_ptr, const int* bath_states, const double* lambda_cm,
+                                const double* nu_per_fs, double T_kelvin, int K, int D, int device) {
+  return create_impl(out, n_states, H_re_cm, H_im_cm, n_baths, bath_ptr, bath_states, lambda_cm, nu_per_fs, T_kelvin, K, D,
+                     device, 0, 0);
 }
 
 heom_status heom_create_partition(heom_ctx** out, int n_states, const double* H_cm, int n_baths, const int* bath_state,
                                   const double* lambda_cm, const double* nu_per_fs, double T_kelvin, int K, int D,
                                   int device, int rank, int world) {
   if (world < 1) return HEOM_EINVAL;
-  return create_impl(out, n_states, H_cm, n_baths, bath_state, lambda_cm, nu_per_fs, T_kelvin, K, D, device, rank, world);
+  return create_sites_impl(out, n_states, H_cm, n_baths, bath_state, lambda_cm, nu_per_fs, T_kelvin, K, D, device, rank, world);
 }
 
 int64_t heom_partition_owned(const heom_ctx* c) { return !c ? -1 : (c->partitioned ? c->part.n_owned : c->h.nodes); }
@@ -419,6 +524,20 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
     return HEOM_OK;
   }
   if (ctx->bound) return fail(ctx, HEOM_ESTATE, "option must be set before heom_bind_workspace");
+  if (s == "mma") {
+    // site-map contexts (one state per bath, real H) on the general tensor-core kernel: -1 = where no other
+    // specialised kernel exists (17 <= N <= 96 except 32, 64, 96), 0 = never, 1 = whenever 17 <= N <= 96
+    if (value < -1 || value > 1) return fail(ctx, HEOM_EINVAL, "mma must be -1, 0 or 1");
+    ctx->mma_opt = value;
+    update_general(ctx);
+    return HEOM_OK;
+  }
+  if (s == "terminator_form") {
+    if (value != 0 && value != 1) return fail(ctx, HEOM_EINVAL, "terminator_form must be 0 or 1");
+    ctx->terminator_form = value;
+    expand_coefficients(ctx);
+    return HEOM_OK;
+  }
   if (s == "pade") {
     Coefficients nc;
     std::string err;
@@ -512,9 +631,20 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   const int Wd = dev_modes(ctx);
   const KernelChoice kc = kernel_choice(ctx);
   ctx->use_large = kc.large;
+  ctx->use_mma = kc.mma;
   ctx->use_tiny = kc.tiny;
   ctx->d_Hs = (double*)(base + L.off_Hs);
   ctx->d_delta = (double*)(base + L.off_delta);
+  ctx->d_Him = (double*)(base + L.off_Him);
+  ctx->d_sptr = (int32_t*)(base + L.off_gen);
+  ctx->d_sbl = (int32_t*)(base + L.off_gen + align_up(((size_t)ctx->h.N + 1) * 4));
+  ctx->d_bmask = (uint32_t*)((char*)ctx->d_sbl + align_up(ctx->sbl.size() * 4 + 16));
+  if (ctx->general) {
+    CU(cudaMemcpy(ctx->d_sptr, ctx->sptr.data(), ctx->sptr.size() * 4, cudaMemcpyHostToDevice));
+    if (!ctx->sbl.empty()) CU(cudaMemcpy(ctx->d_sbl, ctx->sbl.data(), ctx->sbl.size() * 4, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(ctx->d_bmask, ctx->bmask.data(), ctx->bmask.size() * 4, cudaMemcpyHostToDevice));
+    if (!ctx->Him.empty()) CU(cudaMemcpy(ctx->d_Him, ctx->Him.data(), ctx->Him.size() * 8, cudaMemcpyHostToDevice));
+  }
   ctx->d_A = (double2*)(base + L.off_A);
   ctx->d_S0 = (double2*)(base + L.off_S0);
   ctx->d_send = (int32_t*)(base + L.off_send);
@@ -544,8 +674,8 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
     for (int64_t u = 0; u < (int64_t)nodes; ++u) {
       const size_t s = (size_t)h.slot_of[(size_t)u];
       double d = 0.0;
-      for (size_t l = 0; l < W; ++l) {      // device mode column l = state*M + k
-        const int bath = ctx->bath_of[l / Mm];
+      for (size_t l = 0; l < W; ++l) {      // device mode column l = state*M + k (general contexts: l = b*M + k)
+        const int bath = ctx->general ? (int)(l / Mm) : ctx->bath_of[l / Mm];
         if (bath < 0) { tp[s * W + l] = -1; tm[s * W + l] = -1; tt[s * W + l] = 0; continue; }
         const size_t lh = (size_t)bath * Mm + l % Mm;   // host mode index (Eq. 10)
         const int32_t a = h.plus[(size_t)u * Wh + lh], b = h.minus[(size_t)u * Wh + lh];
@@ -564,7 +694,7 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
     }
     CU(cudaMemset(ctx->d_damp + nodes, 0, 8));
     CU(cudaMemcpy(ctx->d_damp, damp.data(), nodes * 8, cudaMemcpyHostToDevice));
-    if (ctx->use_large) {
+    if (ctx->use_large || ctx->use_mma) {
       // CSR link list in storage-slot order: "+" links first, then "-" links, of every node
       std::vector<int64_t> lptr(nodes + 1, 0);
       for (size_t s = 0; s < nodes; ++s) {
@@ -633,7 +763,7 @@ heom_status heom_set_state(heom_ctx* ctx, const double* sigma0) {
     ctx->state_hermitian = herm;
   }
   ctx->ket_col = -1;
-  if (ctx->ket_opt && ctx->use_hpipe && !ctx->use_tiny && !ctx->partitioned && ket_supported(ctx->h.N, dev_modes(ctx), ctx->h.D)) {
+  if (ctx->ket_opt && !ctx->general && ctx->use_hpipe && !ctx->use_tiny && !ctx->partitioned && ket_supported(ctx->h.N, dev_modes(ctx), ctx->h.D)) {
     // column-sparse state?  exactly one non-zero column c, state c without a bath and uncoupled in H
     const int N = ctx->h.N;
     int col = -1, ncols = 0;
@@ -818,6 +948,44 @@ heom_status heom_sync(heom_ctx* ctx) {
   return HEOM_OK;
 }
 
+heom_status heom_set_hamiltonian(heom_ctx* ctx, const double* H_re_cm, const double* H_im_cm) {
+  if (!ctx || !H_re_cm) return HEOM_EINVAL;
+  const int N = ctx->h.N;
+  if (H_im_cm && ctx->Him.empty())
+    return fail(ctx, HEOM_EINVAL, "a complex H needs a context created by heom_create_general with H_im_cm != NULL");
+  for (int i = 0; i < N; ++i)
+    for (int j = 0; j < N; ++j) {
+      const double a = H_re_cm[(size_t)i * N + j], b = H_re_cm[(size_t)j * N + i];
+      if (!std::isfinite(a) || a != b) return fail(ctx, HEOM_EINVAL, "H_re must be finite and symmetric");
+      if (H_im_cm) {
+        const double c = H_im_cm[(size_t)i * N + j], d = H_im_cm[(size_t)j * N + i];
+        if (!std::isfinite(c) || c != -d) return fail(ctx, HEOM_EINVAL, "H_im must be finite and antisymmetric");
+      }
+    }
+  if (ctx->ket_col >= 0) {
+    for (int j = 0; j < N; ++j)
+      if (j != ctx->ket_col && H_re_cm[(size_t)ctx->ket_col * N + j] != 0.0)
+        return fail(ctx, HEOM_ESTATE, "the column-sparse state needs its state uncoupled in H (set option ket=0)");
+  }
+  ctx->H.assign(H_re_cm, H_re_cm + (size_t)N * N);
+  if (!ctx->Him.empty()) {
+    if (H_im_cm) ctx->Him.assign(H_im_cm, H_im_cm + (size_t)N * N);
+    else std::fill(ctx->Him.begin(), ctx->Him.end(), 0.0);
+  }
+  if (ctx->bound) {
+    // stream-ordered: launches already enqueued keep the old H, later ones see the new one
+    CU(cudaMemcpyAsync(ctx->d_H, ctx->H.data(), (size_t)N * N * 8, cudaMemcpyHostToDevice, ctx->stream));
+    if (!ctx->Him.empty())
+      CU(cudaMemcpyAsync(ctx->d_Him, ctx->Him.data(), (size_t)N * N * 8, cudaMemcpyHostToDevice, ctx->stream));
+    if (ctx->use_large) {
+      std::vector<double> Hs(ctx->H);
+      for (double& v : Hs) v *= 1.0 / kHbar;
+      CU(cudaMemcpyAsync(ctx->d_Hs, Hs.data(), Hs.size() * 8, cudaMemcpyHostToDevice, ctx->stream));
+    }
+  }
+  return HEOM_OK;
+}
+
 heom_status heom_populations(heom_ctx* ctx, double* pop, double* trace_re, double* trace_im) {
   if (!ctx) return HEOM_EINVAL;
   if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
@@ -876,6 +1044,7 @@ heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches)
 const char* heom_kernel_name(const heom_ctx* c) {
   if (!c) return "none";
   if (c->ket_col >= 0) return "rhs_ket_kernel";
+  if (c->use_mma) return "rhs_mma_kernel";
   if (c->use_large) return "rhs_large_kernel";
   if (c->use_hpipe) return (c->herm_opt && c->state_hermitian) ? "rhs_hpipe_kernel" : "rhs_hpipe_general_kernel";
   return "rhs_generic_kernel";

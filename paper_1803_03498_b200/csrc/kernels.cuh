@@ -35,6 +35,15 @@ struct RhsParams {
   // No running sum: acc_in / out_acc / bx are unused, out_x = y + ax*k (y may alias x: first stage; out_x may alias
   // y: last stage, in place).  Honoured by the pipelined small-N, the tensor-core and the column kernels.
   int horner;
+  // General system-bath operators (heom_create_general; generic and mma kernels): modes are indexed l = b*M + k
+  // over the B baths (W = B*M), bath b couples through the projectors on the states whose bit is set in
+  // bmask[b][0..3] (sums over s of Eq. 14-17), and H = H + i Him may be complex Hermitian (Eq. 51).
+  int gen;                  // 1: general context
+  int B;                    // baths
+  const int32_t* sptr;      // [N+1] CSR offsets: baths that state s belongs to
+  const int32_t* sbl;       // bath indices
+  const uint32_t* bmask;    // [B][4]
+  const double* Him;        // [N][N] cm^-1 or null (real H)
 };
 
 // Generic kernel: any N <= 96, one thread per matrix element.
@@ -66,6 +75,14 @@ cudaError_t launch_rhs_large(const RhsParams& p, const int64_t* lptr, const void
                              const double* delta_dev, const double* a_plus, const double* a_minus_x,
                              const double* a_minus_o, int sms, unsigned long long* tickets,
                              unsigned long long* ticket_base, cudaStream_t s);
+
+// Tensor-core kernel for 17 <= N <= 96 and general system-bath operators (kernels_mma.cu): p.gen = 1 with the bath
+// membership bits, p.Him != null selects the complex-H instantiation; CSR link list as for the large kernel with
+// mode indices l = b*M + k; a_*: HOST [W][D+1]; tickets as for hpipe.
+bool mma_supported(int N, int W, int B, bool cplx);
+cudaError_t launch_rhs_mma(const RhsParams& p, const int64_t* lptr, const void* lent, const double* a_plus,
+                           const double* a_minus_x, const double* a_minus_o, int sms, unsigned long long* tickets,
+                           unsigned long long* ticket_base, cudaStream_t s);
 
 // Whole-propagation kernel for tiny hierarchies (kernels_tiny.cu): nsteps classical RK4 steps of the state p.x
 // (DEVICE, storage-slot order, updated in place) inside ONE launch of one CTA; tables as for the generic kernel.

@@ -44,7 +44,7 @@ rhs_generic_kernel(const RhsParams p) {
     const int s = s0 + g;
     const double2* sig = sS + g * NN;
 
-    // Eq. 12: -(i/hbar)(H sigma - sigma H), H real
+    // Eq. 12: -(i/hbar)(H sigma - sigma H), H real symmetric (+ i Him, antisymmetric, for general contexts)
     double cr = 0.0, ci = 0.0;
     for (int m = 0; m < N; ++m) {
       const double him = sH[i * N + m], hmj = sH[m * N + j];
@@ -52,9 +52,17 @@ rhs_generic_kernel(const RhsParams p) {
       cr = fma(him, a.x, cr); ci = fma(him, a.y, ci);
       cr = fma(-hmj, b.x, cr); ci = fma(-hmj, b.y, ci);
     }
+    if (p.Him) {
+      for (int m = 0; m < N; ++m) {
+        const double gim = __ldg(p.Him + i * N + m), gmj = __ldg(p.Him + m * N + j);
+        const double2 a = sig[m * N + j], b = sig[i * N + m];
+        cr = fma(-gim, a.y, cr); ci = fma(gim, a.x, ci);      // i g (a.x + i a.y)
+        cr = fma(gmj, b.y, cr); ci = fma(-gmj, b.x, ci);
+      }
+    }
     double kr = ci * p.inv_hbar, ki = -cr * p.inv_hbar;
 
-    // Eq. 13 + Eq. 14 (mask Eq. 24)
+    // Eq. 13 + Eq. 14 (mask Eq. 24; general contexts: the table holds the sum over the baths' states, R12)
     const double2 own = sig[q];
     const double dd = p.damp[s] + p.Tterm[q];
     kr = fma(-dd, own.x, kr); ki = fma(-dd, own.y, ki);
@@ -62,52 +70,42 @@ rhs_generic_kernel(const RhsParams p) {
     const int32_t* pl = p.plus + (size_t)s * W;
     const int32_t* mi = p.minus + (size_t)s * W;
     const uint8_t* tu = p.tuples + (size_t)s * W;
-    if (i != j) {
-      // bath b = i: V^x = +1, V^o = 1
+    // the M modes of one bath (mode columns c*M .. c*M + M - 1) acting on element (i,j) with the mask values
+    // vx = V^x (Eq. 23) and vo = V^o (Eq. 25) summed over the bath's states
+    auto couple = [&](int c, double vx, double vo) {
       for (int k = 0; k < M; ++k) {
-        const int l = i * M + k;
+        const int l = c * M + k;
         const int n = tu[l];
         const int up = pl[l], dn = mi[l];
-        if (up >= 0) {  // Eq. 15/35: + i a+ sigma^+
-          const double a = p.a_plus[l * D1 + n];
+        if (up >= 0 && vx != 0.0) {  // Eq. 15/35: + i a+ V^x sigma^+
+          const double a = vx * p.a_plus[l * D1 + n];
           const double2 v = ldg2(p.x + (size_t)up * p.stride + q);
           kr = fma(-a, v.y, kr); ki = fma(a, v.x, ki);
         }
-        if (dn >= 0) {  // Eq. 16-17/36: (i a-x + a-o) sigma^-
-          const double ax = p.a_minus_x[l * D1 + n], ao = p.a_minus_o[l * D1 + n];
+        if (dn >= 0) {  // Eq. 16-17/36: (i a-x V^x + a-o V^o) sigma^-
+          const double ax = vx * p.a_minus_x[l * D1 + n], ao = vo * p.a_minus_o[l * D1 + n];
           const double2 v = ldg2(p.x + (size_t)dn * p.stride + q);
           kr = fma(ao, v.x, kr); kr = fma(-ax, v.y, kr);
           ki = fma(ao, v.y, ki); ki = fma(ax, v.x, ki);
         }
       }
-      // bath b = j: V^x = -1, V^o = 1
-      for (int k = 0; k < M; ++k) {
-        const int l = j * M + k;
-        const int n = tu[l];
-        const int up = pl[l], dn = mi[l];
-        if (up >= 0) {
-          const double a = p.a_plus[l * D1 + n];
-          const double2 v = ldg2(p.x + (size_t)up * p.stride + q);
-          kr = fma(a, v.y, kr); ki = fma(-a, v.x, ki);
-        }
-        if (dn >= 0) {
-          const double ax = p.a_minus_x[l * D1 + n], ao = p.a_minus_o[l * D1 + n];
-          const double2 v = ldg2(p.x + (size_t)dn * p.stride + q);
-          kr = fma(ao, v.x, kr); kr = fma(ax, v.y, kr);
-          ki = fma(ao, v.y, ki); ki = fma(-ax, v.x, ki);
-        }
+    };
+    if (p.gen) {
+      // baths whose state set contains i: q_i = 1, V^x = 1 - q_j, V^o = 1 + q_j; then those that contain j only
+      for (int e = p.sptr[i]; e < p.sptr[i + 1]; ++e) {
+        const int b = p.sbl[e];
+        const double qj = (double)((p.bmask[b * 4 + (j >> 5)] >> (j & 31)) & 1u);
+        couple(b, 1.0 - qj, 1.0 + qj);
       }
+      for (int e = p.sptr[j]; e < p.sptr[j + 1]; ++e) {
+        const int b = p.sbl[e];
+        if (!((p.bmask[b * 4 + (i >> 5)] >> (i & 31)) & 1u)) couple(b, -1.0, 1.0);
+      }
+    } else if (i != j) {
+      couple(i, 1.0, 1.0);    // the bath of state i acts on row i
+      couple(j, -1.0, 1.0);   // the bath of state j on column j
     } else {
-      // diagonal: V^x = 0, V^o = 2 (bath b = i = j only)
-      for (int k = 0; k < M; ++k) {
-        const int l = i * M + k;
-        const int dn = mi[l];
-        if (dn >= 0) {
-          const double ao = 2.0 * p.a_minus_o[l * D1 + tu[l]];
-          const double2 v = ldg2(p.x + (size_t)dn * p.stride + q);
-          kr = fma(ao, v.x, kr); ki = fma(ao, v.y, ki);
-        }
-      }
+      couple(i, 0.0, 2.0);    // diagonal: V^x = 0, V^o = 2
     }
 
     // fused RK4 stage epilogue

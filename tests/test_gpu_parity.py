@@ -150,7 +150,8 @@ def test_pade_coefficients_parity(name, D, K, T):
     for q, (a, b) in enumerate(zip(g.coefficients(), o.coefficients())):
         assert np.allclose(a, b, rtol=1e-12, atol=1e-15)
     o.set_state(w.sigma0()); g.set_state(w.sigma0())
-    o.rk4_steps(0.25, 200); g.rk4_steps(0.25, 200)
+    steps = 40 if w.N >= 32 else 200
+    o.rk4_steps(0.25, steps); g.rk4_steps(0.25, steps)
     ref, got = o.get_full_state(), g.get_full_state()
     assert rel_err(got, ref) < STATE_TOL
     pop, tr = g.populations()
@@ -282,7 +283,7 @@ def test_cfg5_full_size_rhs_and_stepping(capsys):
     o, g = _pair(w)
     for a, b in zip(g.tables(), o.tables()):
         assert np.array_equal(a, b)
-    st = workloads.random_state(o.nodes, w.N, seed=29)
+    st = workloads.random_state(o.nodes, w.N, seed=29, tile=2048)
     o.set_full_state(st); g.set_full_state(st)
     del st
     rng = np.random.default_rng(4)

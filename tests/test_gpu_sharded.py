@@ -72,7 +72,7 @@ class LocalWorld:
 
 
 @pytest.mark.parametrize("name,D,steps,world", [("cfg2", 4, 100, 2), ("cfg2", 4, 60, 5), ("cfg3", 5, 60, 3),
-                                                ("cfg4", 3, 60, 4), ("cfg5", 1, 20, 2), ("cfg5", 2, 6, 3),
+                                                ("cfg4", 3, 60, 4), ("cfg5", 1, 20, 2), ("cfg5", 2, 2, 3),
                                                 ("cfg1", 4, 200, 3)])
 @pytest.mark.parametrize("herm,form", [(1, -1), (0, -1), (1, 0)])
 def test_sharded_rk4_parity(name, D, steps, world, herm, form):

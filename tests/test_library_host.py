@@ -137,3 +137,22 @@ def test_site_map_validation():
     for bad in ([1, 1], [3], [-1], [0, 1, 2, 0], []):
         with pytest.raises(HeomError):
             Heom(H, 35.0, 0.02, 300.0, 0, 2, bath_state=bad)
+
+
+def test_general_create_validation_without_gpu():
+    """heom_create_general argument checking and host tables (no CUDA call)."""
+    H = np.zeros((4, 4))
+    g = Heom(H, [35.0, 20.0], [0.02, 0.03], 300.0, 1, 3, bath_states=[[1, 3], [2, 3]])
+    o = Oracle(H, [35.0, 20.0], [0.02, 0.03], 300.0, 1, 3, bath_states=[[1, 3], [2, 3]])
+    assert g.nodes == o.nodes and g.W == o.W == 4
+    for a, b in zip(g.tables(), o.tables()):
+        assert np.array_equal(a, b)
+    for bad in ([[1, 1]], [[4]], [[0], []]):
+        with pytest.raises(HeomError):
+            Heom(H, [35.0] * len(bad), [0.02] * len(bad), 300.0, 1, 2, bath_states=bad)
+    with pytest.raises(HeomError):
+        Heom(np.array([[0, 1j], [1j, 0]]), [35.0], [0.02], 300.0, 1, 2, bath_states=[[0]])   # not Hermitian
+    for name, good, bad in [("terminator_form", 1, 2)]:
+        g.set_option(name, good)
+        with pytest.raises(HeomError):
+            g.set_option(name, bad)

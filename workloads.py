@@ -35,6 +35,7 @@ class Workload:
     steps: int
     bath_state: tuple = None      # None: one bath per state; else the states the baths couple to (heom_create_sites)
     sigma0_matrix: np.ndarray = None   # None: |1><1|
+    bath_states: tuple = None     # lists of states per bath (heom_create_general): S(b) >= 1, shared states
 
     @property
     def N(self):
@@ -42,6 +43,8 @@ class Workload:
 
     @property
     def B(self):
+        if self.bath_states is not None:
+            return len(self.bath_states)
         return self.N if self.bath_state is None else len(self.bath_state)
 
     @property
@@ -137,21 +140,42 @@ def absorption_fmo(p=2):
     return Workload("absorb_fmo8", H, 35.0, 50.0, 77.0, 1, 8, 1.0, 1000, tuple(bath_state), s0)
 
 
+def two_exciton_fmo(D=5, K=1, T=77.0):
+    """Not a BASELINE config: the paper's transient-absorption state space (ground state, 7 one-exciton
+    and 21 two-exciton states of FMO = 29 states, Eq. 54) on the FMO-like stand-in H of cfg2; bath a couples to |a>
+    and to the six |ab>.  sigma_0(0) = |1><1| (one-exciton state of site 1).  Defaults: 7 baths x 2 modes,
+    D = 5: 11 628 nodes of 29 x 29 (156 MB per state buffer)."""
+    H, S, _ = two_exciton_manifold(_fmo_like_H())
+    s0 = np.zeros(H.shape, dtype=np.complex128)
+    s0[1, 1] = 1.0
+    return Workload("twoex_fmo29", H, 35.0, 50.0, T, K, D, 0.2, 200, None, s0, tuple(tuple(x) for x in S))
+
+
 CONFIGS = {
     "cfg1": dimer, "cfg2": fmo_like, "cfg3": deep, "cfg4": lhcii_like, "cfg5": large,
 }
-EXTRA = {"absorb": absorption_fmo}
+EXTRA = {"absorb": absorption_fmo, "twoex": two_exciton_fmo}
 
 
 def get(name):
     return (CONFIGS.get(name) or EXTRA[name])()
 
 
-def random_state(nodes, N, seed, hermitian=False):
+def random_state(nodes, N, seed, hermitian=False, tile=0):
     """A dense seeded test state [nodes][N][N] complex128 with O(1) entries
-    (for single-RHS parity, where every term of the equation must be exercised)."""
+    (for single-RHS parity, where every term of the equation must be exercised).
+    tile > 0 (very large states): `tile` random nodes repeated, node u scaled by 1 + (u mod 97)/100 -- every node
+    still differs from its neighbours, at a fraction of the generation time."""
     rng = np.random.default_rng(seed)
     out = np.empty((nodes, N, N), dtype=np.complex128)
+    if tile > 0:
+        blk = rng.standard_normal((tile, N, N)) + 1j * rng.standard_normal((tile, N, N))
+        if hermitian:
+            blk = 0.5 * (blk + np.conj(np.swapaxes(blk, 1, 2)))
+        for a in range(0, nodes, tile):
+            b = min(nodes, a + tile)
+            out[a:b] = blk[:b - a] * (1.0 + (np.arange(a, b) % 97) / 100.0)[:, None, None]
+        return out
     chunk = max(1, (1 << 22) // (N * N))
     for a in range(0, nodes, chunk):
         b = min(nodes, a + chunk)
@@ -191,3 +215,34 @@ def dipole_operator(dipoles, p):
     mu[1:, 0] = dipoles[:, p]
     mu[0, 1:] = dipoles[:, p]
     return mu
+
+
+def two_exciton_manifold(H_sites):
+    """Input construction for the paper's two-exciton space (Eq. 54: N_states = 1 + N + N(N-1)/2; P:84:
+    "a two-exciton state is coupled to two sites"): states 0 = ground, 1..N = |a>, then |ab> (a < b) in
+    row-major pair order.  Frenkel-exciton matrix elements: <ab|H|ab> = eps_a + eps_b, <ab|H|ac> = J_bc for pairs
+    that share one site, zero otherwise; the manifolds are not coupled by the field-free H.  Bath a (site a's
+    bath) couples to |a> and to every |ab>.  Returns (H [Ns][Ns], bath_states list of lists, pair index list)."""
+    N = H_sites.shape[0]
+    pairs = [(a, b) for a in range(N) for b in range(a + 1, N)]
+    Ns = 1 + N + len(pairs)
+    H = np.zeros((Ns, Ns))
+    H[1:N + 1, 1:N + 1] = H_sites
+    for p, (a, b) in enumerate(pairs):
+        for q, (c, d) in enumerate(pairs):
+            if p == q:
+                H[1 + N + p, 1 + N + q] = H_sites[a, a] + H_sites[b, b]
+            else:
+                shared = {a, b} & {c, d}
+                if len(shared) == 1:
+                    (x,) = {a, b} - shared
+                    (y,) = {c, d} - shared
+                    H[1 + N + p, 1 + N + q] = H_sites[x, y]
+    bath_states = [[1 + a] + [1 + N + p for p, pr in enumerate(pairs) if a in pr] for a in range(N)]
+    return H, bath_states, pairs
+
+
+def rwa_field_hamiltonian(H0, mu_plus, field):
+    """H(t) of Eq. 51 for one polarisation: H0 - (mu^+ E^-(t) + mu^- E^+(t)), E^- = conj(E^+); `field` = E^+(t) as a
+    complex number (envelope times carrier phase, Eq. 50), mu_plus = sum_a d_a |a><0| (Eq. 48), real."""
+    return H0.astype(np.complex128) - (mu_plus * np.conj(field) + mu_plus.T * field)
