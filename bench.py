@@ -285,7 +285,7 @@ def run_config(key, args, steps, ctx, with_e2e=True, with_cpu=True, options=None
     peaks, which = measured_peaks()
     value = 4.0 * w.nodes * steps * job / (ms * 1e-3)
     horner = kernel_name in ("rhs_hpipe_kernel", "rhs_hpipe_general_kernel", "rhs_large_kernel", "rhs_ket_kernel",
-                             "rhs_mma_kernel") \
+                             "rhs_mma_kernel", "rhs_large_herm_kernel") \
         and opts.get("rk4_form", -1) != 0
     # fused classical RK4 moves 16 state sizes per step = 64 N^2 bytes per node-update; the Horner form
     # the kernels run by default (R6) moves 2 + 3 + 3 + 3 = 11 state sizes = 44 N^2 bytes per node-update
@@ -317,10 +317,17 @@ def run_config(key, args, steps, ctx, with_e2e=True, with_cpu=True, options=None
         # arithmetic-bound (N/8 = 12 flop/B at N = 96): FP64 tensor-core (DMMA) roofline, peak measured in this process
         fp = ctx["fp64"]
         tf = alg_flops_per_launch / avg_launch_s / 1e12
+        # Hermitian states: the kernel forms H sigma only and takes k = Z + Z^dagger (4 N^3 executed flops)
+        exe_flops = alg_flops_per_launch * (0.5 if kernel_name == "rhs_large_herm_kernel" else 1.0)
         roof = {"bound": "alu", "achieved": tf, "peak": fp["dmma_tflops"], "unit": "TFLOP/s",
                 "frac": tf / fp["dmma_tflops"], "peak_source": "measured: " + fp["how"],
                 "dfma_peak_tflops": fp["dfma_tflops"],
                 "algorithmic_flops_per_launch": alg_flops_per_launch,
+                "executed_flops_per_launch": exe_flops,
+                "achieved_executed": exe_flops / avg_launch_s / 1e12,
+                "frac_executed": exe_flops / avg_launch_s / 1e12 / fp["dmma_tflops"],
+                "definition": "achieved = SURVEY 8(d) algorithmic flops (8 N^3 per node-update, real H) / launch time; "
+                              "*_executed = tensor-core flops the kernel issues (4 N^3 when the state is Hermitian)",
                 "hbm_GBs_at_executed_bytes": exe_bytes_per_launch / avg_launch_s / 1e9}
     else:
         exe = exe_bytes_per_launch / avg_launch_s / 1e9

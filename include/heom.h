@@ -212,6 +212,23 @@ heom_status heom_stage_output(heom_ctx* ctx, int stage, void** dev_ptr);
  * nodes of N*N complex128. */
 heom_status heom_pack_halo(heom_ctx* ctx, const void* src_dev, void* dst_dev);
 
+/* Slice halo: a neighbour gather reads of a ghost only row s -- and, unless the state is exactly Hermitian and a
+ * row-gather kernel runs, column s -- where s is the state of the bath through which the ghost is reached (the masks
+ * of Eq. 23, 25): 16 N (or 32 N) bytes per (ghost, state) pair instead of 16 N^2 per ghost.  The (node, state) pairs
+ * are unique and sorted by (peer, global node order, state) on both sides, so sender and receiver agree without
+ * communication.  Per stage: heom_rk4_stage; heom_stage_output -> buf; heom_pack_halo_slices(buf -> send);
+ * all-to-all of the packed pairs (heom_halo_slice_elements() complex128 each) ; heom_unpack_halo_slices(recv -> buf).
+ *   send_counts, recv_counts HOST int64 [world]: pairs per peer; send_node / send_state HOST int32 [sum send_counts]:
+ *   local OWNED node index and state; recv_node / recv_state HOST int32 [sum recv_counts]: local GHOST node index
+ *   and state.  Any pointer may be NULL. */
+heom_status heom_partition_plan_slices(const heom_ctx* ctx, int64_t* send_counts, int64_t* recv_counts,
+                                       int32_t* send_node, int32_t* send_state, int32_t* recv_node, int32_t* recv_state);
+int heom_halo_slice_elements(const heom_ctx* ctx);   /* N (row) or 2N (row, then column) complex128 per pair, now */
+/* dst_dev[q] = the slices of pair q of src_dev (a state buffer); DEVICE pointers; kernel on the bound stream. */
+heom_status heom_pack_halo_slices(heom_ctx* ctx, const void* src_dev, void* dst_dev);
+/* scatter the received pairs (DEVICE, in recv order) into the ghost nodes of state_dev. */
+heom_status heom_unpack_halo_slices(heom_ctx* ctx, const void* src_dev, void* state_dev);
+
 /* Introspection for the harness. */
 int64_t heom_launch_count(const heom_ctx* ctx); /* kernels launched so far */
 /* With option "timing"=1: sum of CUDA-event durations of the RHS/stage kernels

@@ -24,6 +24,7 @@ SYMBOLS = [
     "heom_set_state", "heom_set_full_state", "heom_get_full_state", "heom_rhs", "heom_rk4_steps",
     "heom_sync", "heom_populations", "heom_launch_count", "heom_kernel_time", "heom_kernel_name",
     "heom_last_error", "heom_probe_peak", "heom_create_general", "heom_set_hamiltonian",
+    "heom_partition_plan_slices", "heom_halo_slice_elements", "heom_pack_halo_slices", "heom_unpack_halo_slices",
 ]
 
 _lib = None
@@ -58,6 +59,10 @@ def load_library():
     lib.heom_partition_owned.argtypes = [P]
     lib.heom_partition_owned.restype = C.c_int64
     lib.heom_partition_plan.argtypes = [P, P, P, P, P]
+    lib.heom_partition_plan_slices.argtypes = [P, P, P, P, P, P, P]
+    lib.heom_halo_slice_elements.argtypes = [P]
+    lib.heom_pack_halo_slices.argtypes = [P, P, P]
+    lib.heom_unpack_halo_slices.argtypes = [P, P, P]
     lib.heom_rk4_stage.argtypes = [P, C.c_double, C.c_int]
     lib.heom_stage_output.argtypes = [P, C.c_int, C.POINTER(P)]
     lib.heom_pack_halo.argtypes = [P, P, P]
@@ -302,6 +307,28 @@ class Heom:
         idx = np.empty(int(sc.sum()), dtype=np.int32)
         self._ck(self._lib.heom_partition_plan(self._h, None, None, None, idx.ctypes.data if idx.size else None))
         return gid, sc, rc_, idx
+
+    def partition_plan_slices(self):
+        """(send_counts, recv_counts, send_node, send_state, recv_node, recv_state) of the slice halo."""
+        world = self.partition[1]
+        sc = np.empty(world, dtype=np.int64); rc_ = np.empty(world, dtype=np.int64)
+        self._ck(self._lib.heom_partition_plan_slices(self._h, sc.ctypes.data, rc_.ctypes.data, None, None, None, None))
+        sn = np.empty(int(sc.sum()), dtype=np.int32); ss = np.empty_like(sn)
+        rn = np.empty(int(rc_.sum()), dtype=np.int32); rs = np.empty_like(rn)
+        self._ck(self._lib.heom_partition_plan_slices(self._h, None, None, sn.ctypes.data if sn.size else None,
+                                                      ss.ctypes.data if ss.size else None,
+                                                      rn.ctypes.data if rn.size else None,
+                                                      rs.ctypes.data if rs.size else None))
+        return sc, rc_, sn, ss, rn, rs
+
+    def halo_slice_elements(self):
+        return int(self._lib.heom_halo_slice_elements(self._h))
+
+    def pack_halo_slices(self, src_ptr, dst_ptr):
+        self._ck(self._lib.heom_pack_halo_slices(self._h, int(src_ptr), int(dst_ptr)))
+
+    def unpack_halo_slices(self, src_ptr, state_ptr):
+        self._ck(self._lib.heom_unpack_halo_slices(self._h, int(src_ptr), int(state_ptr)))
 
     def rk4_stage(self, dt_fs, stage):
         self._ck(self._lib.heom_rk4_stage(self._h, float(dt_fs), int(stage)))

@@ -84,11 +84,13 @@ struct heom_ctx {
   int part_rank = 0, part_world = 1;
   Partition part;
   int32_t* d_send = nullptr; // DEVICE copy of part.send_idx
+  int32_t *d_spn = nullptr, *d_sps = nullptr, *d_rpn = nullptr, *d_rps = nullptr;   // slice-halo pair lists
   size_t n_links = 0;
   unsigned long long* d_tickets = nullptr;   // work counter of the persistent kernel
   unsigned long long ticket_base = 0;
   int rk4_form = -1;         // option "rk4_form": 0 classical stages, 1 Horner form (where the kernel supports it), -1 auto
   int l2_fetch = 0;          // option "l2_fetch": cudaLimitMaxL2FetchGranularity in bytes, 0 = leave the default
+  int l2_persist = 0;        // option "l2_persist": percent of the device's maximum persisting-L2 carve-out to request
   int sms = 148;
   uint8_t* d_tuples = nullptr;
   double *d_damp = nullptr, *d_H = nullptr, *d_T = nullptr, *d_ap = nullptr, *d_amx = nullptr,
@@ -180,7 +182,7 @@ bool ensure_hierarchy(heom_ctx* c) {
   std::string err;
   const int n_states = c->h.N;
   bool ok = build_hierarchy(c->B, c->h.K, c->h.D, c->partitioned ? 1 : c->order, c->h, err);   // tuples over the B*M modes
-  if (ok && c->partitioned) ok = restrict_hierarchy(c->h, c->part_rank, c->part_world, c->part, err);
+  if (ok && c->partitioned) ok = restrict_hierarchy(c->h, c->part_rank, c->part_world, c->site, c->part, err);
   c->h.N = n_states;
   if (!ok) { c->err = err; return false; }
   c->hierarchy_built = true;
@@ -192,7 +194,7 @@ int node_stride(int N) { return N * N; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_linksP, off_Hs, off_delta, off_Him, off_gen, off_A, off_S0, off_send, off_lptr, off_lent, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_linksP, off_Hs, off_delta, off_Him, off_gen, off_A, off_S0, off_send, off_pairs, off_lptr, off_lent, total;
 };
 
 // Which kernel family the bound configuration will run (fixed by the shape and the "kernel" option), so that the
@@ -240,6 +242,7 @@ Layout layout_of(const heom_ctx* c) {
   L.off_A = o; o += align_up(N * N * 16);
   L.off_S0 = o; o += align_up(N * N * 16);
   L.off_send = o; o += align_up(c->part.send_idx.size() * 4 + 16);
+  L.off_pairs = o; o += 2 * align_up(c->part.send_pair_node.size() * 4 + 16) + 2 * align_up(c->part.recv_pair_node.size() * 4 + 16);
   if (kc.large || kc.mma) {
     // CSR link list: one 16-byte entry per valid "+" and per valid "-" link (a partition's table has links for its
     // owned rows only, so the two counts differ there)
@@ -292,8 +295,8 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
                       ctx->cd.a_minus_o.data(), ctx->sms, ctx->d_tickets, &ctx->ticket_base, ctx->stream));
   else if (ctx->use_large)
     CU(launch_rhs_large(p, ctx->d_lptr, ctx->d_lent, ctx->d_Hs, ctx->d_delta, ctx->cd.a_plus.data(),
-                        ctx->cd.a_minus_x.data(), ctx->cd.a_minus_o.data(), ctx->sms, ctx->d_tickets,
-                        &ctx->ticket_base, ctx->stream));
+                        ctx->cd.a_minus_x.data(), ctx->cd.a_minus_o.data(), ctx->herm_opt && ctx->state_hermitian,
+                        ctx->sms, ctx->d_tickets, &ctx->ticket_base, ctx->stream));
   else if (ctx->use_hpipe)
     CU(launch_rhs_hpipe(p, ctx->d_linksP, ctx->lrowP, ctx->cd.a_plus.data(), ctx->cd.a_minus_x.data(),
                         ctx->cd.a_minus_o.data(), ctx->H.data(), ctx->cd.delta.data(),
@@ -507,6 +510,11 @@ heom_status heom_set_option(heom_ctx* ctx, const char* name, int value) {
   const std::string s(name);
   if (s == "timing") { ctx->timing = value ? 1 : 0; return HEOM_OK; }
   if (s == "hermitian") { ctx->herm_opt = value ? 1 : 0; return HEOM_OK; }
+  if (s == "l2_persist") {
+    if (value < 0 || value > 100) return fail(ctx, HEOM_EINVAL, "l2_persist must be 0..100 (percent of the maximum)");
+    ctx->l2_persist = value;
+    return HEOM_OK;
+  }
   if (s == "l2_fetch") {
     if (value != 0 && value != 32 && value != 64 && value != 128) return fail(ctx, HEOM_EINVAL, "l2_fetch must be 0, 32, 64 or 128");
     ctx->l2_fetch = value;
@@ -606,6 +614,11 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
     return fail(ctx, HEOM_ECUDA, std::string("no usable CUDA device: ") + cudaGetErrorString(e));
   CU(cudaSetDevice(ctx->device));
   if (ctx->l2_fetch) CU(cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)ctx->l2_fetch));
+  if (ctx->l2_persist) {
+    cudaDeviceProp pr;
+    CU(cudaGetDeviceProperties(&pr, ctx->device));
+    CU(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)pr.persistingL2CacheMaxSize / 100 * (size_t)ctx->l2_persist));
+  }
   ctx->stream = (cudaStream_t)cuda_stream;
   ctx->stride = node_stride(ctx->h.N);
   ctx->state_bytes = L.state;
@@ -650,6 +663,20 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->d_send = (int32_t*)(base + L.off_send);
   if (!ctx->part.send_idx.empty())
     CU(cudaMemcpy(ctx->d_send, ctx->part.send_idx.data(), ctx->part.send_idx.size() * 4, cudaMemcpyHostToDevice));
+  {
+    const Partition& q = ctx->part;
+    const size_t ns = align_up(q.send_pair_node.size() * 4 + 16), nr = align_up(q.recv_pair_node.size() * 4 + 16);
+    ctx->d_spn = (int32_t*)(base + L.off_pairs); ctx->d_sps = (int32_t*)(base + L.off_pairs + ns);
+    ctx->d_rpn = (int32_t*)(base + L.off_pairs + 2 * ns); ctx->d_rps = (int32_t*)(base + L.off_pairs + 2 * ns + nr);
+    if (!q.send_pair_node.empty()) {
+      CU(cudaMemcpy(ctx->d_spn, q.send_pair_node.data(), q.send_pair_node.size() * 4, cudaMemcpyHostToDevice));
+      CU(cudaMemcpy(ctx->d_sps, q.send_pair_state.data(), q.send_pair_state.size() * 4, cudaMemcpyHostToDevice));
+    }
+    if (!q.recv_pair_node.empty()) {
+      CU(cudaMemcpy(ctx->d_rpn, q.recv_pair_node.data(), q.recv_pair_node.size() * 4, cudaMemcpyHostToDevice));
+      CU(cudaMemcpy(ctx->d_rps, q.recv_pair_state.data(), q.recv_pair_state.size() * 4, cudaMemcpyHostToDevice));
+    }
+  }
   ctx->ket_col = -1;
   ctx->d_lptr = (int64_t*)(base + L.off_lptr);
   ctx->d_lent = (void*)(base + L.off_lent);
@@ -941,6 +968,47 @@ heom_status heom_pack_halo(heom_ctx* ctx, const void* src_dev, void* dst_dev) {
   return HEOM_OK;
 }
 
+heom_status heom_partition_plan_slices(const heom_ctx* c, int64_t* send_counts, int64_t* recv_counts,
+                                       int32_t* send_node, int32_t* send_state, int32_t* recv_node, int32_t* recv_state) {
+  if (!c || !c->partitioned) return HEOM_EINVAL;
+  const Partition& q = c->part;
+  if (send_counts) std::memcpy(send_counts, q.send_pair_counts.data(), q.send_pair_counts.size() * 8);
+  if (recv_counts) std::memcpy(recv_counts, q.recv_pair_counts.data(), q.recv_pair_counts.size() * 8);
+  if (send_node && !q.send_pair_node.empty()) std::memcpy(send_node, q.send_pair_node.data(), q.send_pair_node.size() * 4);
+  if (send_state && !q.send_pair_state.empty()) std::memcpy(send_state, q.send_pair_state.data(), q.send_pair_state.size() * 4);
+  if (recv_node && !q.recv_pair_node.empty()) std::memcpy(recv_node, q.recv_pair_node.data(), q.recv_pair_node.size() * 4);
+  if (recv_state && !q.recv_pair_state.empty()) std::memcpy(recv_state, q.recv_pair_state.data(), q.recv_pair_state.size() * 4);
+  return HEOM_OK;
+}
+
+int heom_halo_slice_elements(const heom_ctx* c) {
+  if (!c) return -1;
+  /* rows only while the state is exactly Hermitian and the row-gather kernels run, rows + columns otherwise */
+  return (c->herm_opt && c->state_hermitian && (c->use_hpipe || c->use_large)) ? c->h.N : 2 * c->h.N;
+}
+
+heom_status heom_pack_halo_slices(heom_ctx* ctx, const void* src_dev, void* dst_dev) {
+  if (!ctx || !src_dev || !dst_dev) return HEOM_EINVAL;
+  if (!ctx->bound || !ctx->partitioned) return fail(ctx, HEOM_ESTATE, "not a bound partition");
+  const long long pairs = (long long)ctx->part.send_pair_node.size();
+  if (pairs == 0) return HEOM_OK;
+  CU(launch_halo_slices((double2*)src_dev, (double2*)dst_dev, ctx->d_spn, ctx->d_sps, pairs, ctx->h.N,
+                        heom_halo_slice_elements(ctx) == 2 * ctx->h.N, 1, ctx->stream));
+  ctx->launches += 1;
+  return HEOM_OK;
+}
+
+heom_status heom_unpack_halo_slices(heom_ctx* ctx, const void* src_dev, void* state_dev) {
+  if (!ctx || !src_dev || !state_dev) return HEOM_EINVAL;
+  if (!ctx->bound || !ctx->partitioned) return fail(ctx, HEOM_ESTATE, "not a bound partition");
+  const long long pairs = (long long)ctx->part.recv_pair_node.size();
+  if (pairs == 0) return HEOM_OK;
+  CU(launch_halo_slices((double2*)state_dev, (double2*)src_dev, ctx->d_rpn, ctx->d_rps, pairs, ctx->h.N,
+                        heom_halo_slice_elements(ctx) == 2 * ctx->h.N, 0, ctx->stream));
+  ctx->launches += 1;
+  return HEOM_OK;
+}
+
 heom_status heom_sync(heom_ctx* ctx) {
   if (!ctx) return HEOM_EINVAL;
   if (!ctx->bound) return fail(ctx, HEOM_ESTATE, "no workspace bound");
@@ -1045,7 +1113,7 @@ const char* heom_kernel_name(const heom_ctx* c) {
   if (!c) return "none";
   if (c->ket_col >= 0) return "rhs_ket_kernel";
   if (c->use_mma) return "rhs_mma_kernel";
-  if (c->use_large) return "rhs_large_kernel";
+  if (c->use_large) return (c->herm_opt && c->state_hermitian) ? "rhs_large_herm_kernel" : "rhs_large_kernel";
   if (c->use_hpipe) return (c->herm_opt && c->state_hermitian) ? "rhs_hpipe_kernel" : "rhs_hpipe_general_kernel";
   return "rhs_generic_kernel";
 }

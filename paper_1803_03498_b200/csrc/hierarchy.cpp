@@ -1,6 +1,7 @@
 // hierarchy.cpp -- see hierarchy.hpp.  Host only, integer + a little fp64.
 #include "hierarchy.hpp"
 
+#include <algorithm>
 #include <cmath>
 #include <limits>
 #include <utility>
@@ -128,7 +129,8 @@ bool build_hierarchy(int N, int K, int D, int order, Hierarchy& h, std::string& 
   return true;
 }
 
-bool restrict_hierarchy(Hierarchy& h, int rank, int world, Partition& part, std::string& err) {
+bool restrict_hierarchy(Hierarchy& h, int rank, int world, const std::vector<int>& state_of_bath, Partition& part,
+                        std::string& err) {
   if (world < 1 || rank < 0 || rank >= world) { err = "invalid rank/world"; return false; }
   const int64_t nodes = h.nodes;
   const int W = h.W;
@@ -145,6 +147,10 @@ bool restrict_hierarchy(Hierarchy& h, int rank, int world, Partition& part, std:
   // nodes every peer needs: those with a neighbour in the peer's range
   std::vector<uint8_t> is_ghost((size_t)nodes, 0);
   std::vector<std::vector<int32_t>> send((size_t)world);
+  // slice halo pairs as (peer, global slot, state) keys: what I receive (ghost t read through a bath on state st)
+  // and what I send (my node s read by a node of peer p through a bath on state st; link symmetry)
+  struct PairKey { int peer; int64_t slot; int state; };
+  std::vector<PairKey> rpairs, spairs;
   for (int64_t s = s0; s < s1; ++s) {
     const int64_t u = h.node_at[(size_t)s];
     int last_peer = -1;
@@ -157,6 +163,9 @@ bool restrict_hierarchy(Hierarchy& h, int rank, int world, Partition& part, std:
         if (t >= s0 && t < s1) continue;
         is_ghost[(size_t)t] = 1;
         const int p = owner_of(t);
+        const int st = state_of_bath[(size_t)(l / h.M)];
+        rpairs.push_back({p, t, st});
+        spairs.push_back({p, s, st});
         if (p != last_peer) {
           bool seen = false;
           for (int q : peers) seen = seen || q == p;
@@ -204,6 +213,23 @@ bool restrict_hierarchy(Hierarchy& h, int rank, int world, Partition& part, std:
     }
   }
   part.root = local_of[(size_t)h.slot_of[0]];
+  auto finish = [&](std::vector<PairKey>& v, std::vector<int64_t>& counts, std::vector<int32_t>& node,
+                    std::vector<int32_t>& state) {
+    std::sort(v.begin(), v.end(), [](const PairKey& a, const PairKey& b) {
+      return a.peer != b.peer ? a.peer < b.peer : (a.slot != b.slot ? a.slot < b.slot : a.state < b.state);
+    });
+    v.erase(std::unique(v.begin(), v.end(), [](const PairKey& a, const PairKey& b) {
+              return a.peer == b.peer && a.slot == b.slot && a.state == b.state; }), v.end());
+    counts.assign((size_t)world, 0);
+    node.clear(); state.clear();
+    for (const PairKey& k : v) {
+      counts[(size_t)k.peer] += 1;
+      node.push_back(local_of[(size_t)k.slot]);
+      state.push_back(k.state);
+    }
+  };
+  finish(spairs, part.send_pair_counts, part.send_pair_node, part.send_pair_state);
+  finish(rpairs, part.recv_pair_counts, part.recv_pair_node, part.recv_pair_state);
   h = std::move(loc);
   return true;
 }

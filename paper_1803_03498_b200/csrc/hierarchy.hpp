@@ -39,12 +39,20 @@ struct Partition {
   std::vector<int64_t> recv_counts;  // [world] ghosts owned by peer p (contiguous in the ghost region)
   std::vector<int32_t> send_idx;     // [sum send_counts] local indices, grouped by peer, ascending
   int64_t root = -1;                 // local index of the hierarchy's root node (n = 0), -1 if not local
+  // Slice halo: a gather reads of a ghost only row s (and, for states that are not Hermitian, column s) of the
+  // states s = state of the bath through which the ghost is reached (Eq. 23, 25).  (node, state) pairs, unique,
+  // sorted by (peer, global slot, state): the same order on the sending and on the receiving side.
+  std::vector<int64_t> send_pair_counts, recv_pair_counts;   // [world]
+  std::vector<int32_t> send_pair_node, send_pair_state;      // local OWNED index, state; grouped by peer
+  std::vector<int32_t> recv_pair_node, recv_pair_state;      // local GHOST index (>= n_owned), state; grouped by peer
 };
 
 // Replaces `h` (a full hierarchy built with order = 1) by the rank's local hierarchy: tuples and link tables of the
 // n_owned + n_ghost local nodes with local indices (ghost rows: every link invalid; they are never the result of
 // a computation, only copies), slot_of = node_at = identity.
-bool restrict_hierarchy(Hierarchy& h, int rank, int world, Partition& part, std::string& err);
+// state_of_bath: [B] state bath b couples to (tuple position l belongs to bath l / M).
+bool restrict_hierarchy(Hierarchy& h, int rank, int world, const std::vector<int>& state_of_bath, Partition& part,
+                        std::string& err);
 
 struct Coefficients {
   double beta_hbar = 0;            // fs

@@ -67,13 +67,14 @@ cudaError_t launch_rhs_hpipe(const RhsParams& p, const int32_t* links, int lrow,
                              const double* delta_host, int hermitian, int warps, int sms,
                              unsigned long long* tickets, unsigned long long* ticket_base, cudaStream_t s);
 
-// Tensor-core (DMMA) kernel for N = 32, 64, 96 (kernels_large.cu), any state.  lptr: DEVICE [nodes+1] CSR
+// Tensor-core (DMMA) kernel for N = 32, 64, 96 (kernels_large.cu), any state; hermitian = 1: the state is exactly
+// Hermitian (one product H sigma instead of two, row-only gathers, exact Hermiticity preserved).  lptr: DEVICE [nodes+1] CSR
 // offsets; lent: DEVICE int4 link entries {neighbour slot, mode l, 0 "+" | 1 "-", n_l}; Hs_dev: DEVICE
 // [N][N] = H/hbar; delta_dev: DEVICE [N]; a_*: HOST coupling tables [W][D+1]; tickets as for hpipe.
 bool large_supported(int N, int W);
 cudaError_t launch_rhs_large(const RhsParams& p, const int64_t* lptr, const void* lent, const double* Hs_dev,
                              const double* delta_dev, const double* a_plus, const double* a_minus_x,
-                             const double* a_minus_o, int sms, unsigned long long* tickets,
+                             const double* a_minus_o, int hermitian, int sms, unsigned long long* tickets,
                              unsigned long long* ticket_base, cudaStream_t s);
 
 // Tensor-core kernel for 17 <= N <= 96 and general system-bath operators (kernels_mma.cu): p.gen = 1 with the bath
@@ -109,6 +110,11 @@ cudaError_t launch_ket_expand(const double2* ket, double2* dst, long long nodes,
 // dst[q][0..NN) = src[idx[q]*stride + 0..NN): the send buffer of a halo exchange
 cudaError_t launch_pack_rows(const double2* src, double2* dst, const int32_t* idx, long long rows, int NN, int stride,
                              cudaStream_t s);
+
+// slice halo: pair q = (node[q], st[q]) <-> packed[q][0..per), per = N (row st) or 2N (row st, then column st);
+// to_packed = 1 gathers from the state buffer, 0 scatters into it
+cudaError_t launch_halo_slices(double2* state, double2* packed, const int32_t* node, const int32_t* st, long long pairs,
+                               int N, int with_cols, int to_packed, cudaStream_t s);
 
 // out[0], out[1] = Tr(A sigma_0) (re, im); A: DEVICE [N][N] complex128
 cudaError_t launch_expectation(const double2* node0, const double2* A, int N, double* out, cudaStream_t s);

@@ -230,6 +230,33 @@ cudaError_t launch_pack_rows(const double2* src, double2* dst, const int32_t* id
   return cudaGetLastError();
 }
 
+// slice halo: pair q = (node, state st) moves row st of the node -- and, with_cols, column st
+// behind it -- between the state buffer and a packed buffer of `per` = N or 2N elements per pair
+__global__ void halo_slices_kernel(double2* __restrict__ state, double2* __restrict__ packed,
+                                   const int32_t* __restrict__ node, const int32_t* __restrict__ st, long long pairs,
+                                   int N, int per, int to_packed) {
+  const long long total = pairs * per;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
+       t += (long long)gridDim.x * blockDim.x) {
+    const long long q = t / per;
+    const int e = (int)(t - q * per);
+    const size_t base = (size_t)node[q] * N * N;
+    const size_t el = e < N ? base + (size_t)st[q] * N + e : base + (size_t)(e - N) * N + st[q];
+    if (to_packed) packed[t] = state[el];
+    else state[el] = packed[t];
+  }
+}
+
+cudaError_t launch_halo_slices(double2* state, double2* packed, const int32_t* node, const int32_t* st, long long pairs,
+                               int N, int with_cols, int to_packed, cudaStream_t s) {
+  const int per = with_cols ? 2 * N : N;
+  long long blocks = (pairs * per + 255) / 256;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  if (blocks < 1) blocks = 1;
+  halo_slices_kernel<<<(int)blocks, 256, 0, s>>>(state, packed, node, st, pairs, N, per, to_packed);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_expectation(const double2* node0, const double2* A, int N, double* out, cudaStream_t s) {
   expectation_kernel<<<1, 32, 0, s>>>(node0, A, N, out);
   return cudaGetLastError();

@@ -18,6 +18,13 @@
 //     sigma_{u +- e_l} (Eq. 15-17 / 35-36) are added from a compact per-node link list with predicated
 //     global loads of the neighbour's row b and column b (Eq. 23, 25); the RK4 update reads y / acc and
 //     writes the next stage input / running sum straight from the fragment layout (64-byte segments).
+//   * HERM = true (the state is exactly Hermitian, checked in api.cu, never assumed): the hierarchical Liouvillian
+//     maps Hermitian ADOs to Hermitian ADOs, so k_u = Z + Z^dagger with
+//       Z = -(i/hbar) H sigma_u - (d_u + T)/2 o sigma_u + sum_l (a-o + i a) P_b sigma_{u +- e_l}   (P_b keeps row b)
+//     as in kernels_hpipe.cu: only P1 = H sigma runs on the tensor cores (4 N^3 instead of 8 N^3 flop), only ROWS
+//     of the neighbours are gathered (contiguous), and Z is transposed through the sigma tile's shared memory
+//     once the contraction is done with it.  Element (j,i) is produced by exactly the conjugate operations of
+//     (i,j): the state stays bit-exactly Hermitian.
 #include "kernels.cuh"
 
 #include <cmath>
@@ -92,7 +99,7 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
 }
 __device__ __forceinline__ double neg(double v) { return -v; }
 
-template <int N>
+template <int N, bool HERM>
 __global__ void __launch_bounds__(LargeCfg<N>::THREADS, 1)
 rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
   using C = LargeCfg<N>;
@@ -104,6 +111,8 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
   double* sDelta = reinterpret_cast<double*>(sS + N * SS);                    // [N]
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(sDelta + N);
   int* sNode = reinterpret_cast<int*>(bar + 1);
+  double* sSqrt = reinterpret_cast<double*>(sNode + 2);                       // [258] sqrt(n), n = 0..D+1 <= 256
+  for (int e = threadIdx.x; e < 258; e += C::THREADS) sSqrt[e] = sqrt((double)e);
 
   for (int e = threadIdx.x; e < NN; e += C::THREADS) sH[(e / N) * HS + (e % N)] = P.Hs[e];
   for (int e = threadIdx.x; e < N; e += C::THREADS) sDelta[e] = P.delta[e];
@@ -150,10 +159,7 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
     if (warp == 0) {
       if (lane == 0) {
         next = draw();
-        if (next < nodes) {
-          lbulk_prefetch_l2(p.x + (size_t)next * NN, (unsigned)NN * 16);
-          if (p.horner && p.y != p.x) lbulk_prefetch_l2(p.y + (size_t)next * NN, (unsigned)NN * 16);
-        }
+        if (next < nodes) lbulk_prefetch_l2(p.x + (size_t)next * NN, (unsigned)NN * 16);
       }
       next = __shfl_sync(0xffffffffu, next, 0);
     }
@@ -186,6 +192,7 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
           for (int rg = 0; rg < RG; ++rg) dmma(acc[rg][ct].x, acc[rg][ct].y, hA[rg].y, b1);
         }
       }
+      if (!HERM)
 #pragma unroll
       for (int h = 0; h < 2; ++h) {  // P2: natural k, two sub-steps of 4
         const int mm = m0 + 4 * h;
@@ -207,7 +214,12 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
       }
     }
 
+    // Horner stage: this node's y is needed by the epilogue -- pull it into L2 now (prefetching it a whole node
+    // ahead made it compete with the sigma tiles for L2: 1.5x the DRAM reads, profiles/r2_cfg5_large.md)
+    if (warp == 1 && lane == 0 && p.horner && p.y != p.x) lbulk_prefetch_l2(p.y + (size_t)node * NN, (unsigned)NN * 16);
+
     // ---- k = -i C - (d_u + T) o sigma (Eq. 13-14, mask Eq. 24), in the fragment layout ------------
+    //      (HERM: Z = -i P1 - (d_u + T)/2 o sigma)
     const double dd = p.damp[node];
 #pragma unroll
     for (int rg = 0; rg < RG; ++rg) {
@@ -216,21 +228,24 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
       for (int ct = 0; ct < CT; ++ct) {
         const int col = j0w + 4 * ct + t;
         const double2 sv = sS[row * SS + col];
-        const double dt = dd + (row == col ? 0.0 : sDelta[row] + sDelta[col]);
+        double dt = dd + (row == col ? 0.0 : sDelta[row] + sDelta[col]);
+        if (HERM) dt *= 0.5;
         const double2 c = acc[rg][ct];
         acc[rg][ct] = make_double2(fma(-dt, sv.x, c.y), fma(-dt, sv.y, -c.x));
       }
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncthreads();                                  // every warp is done with the node's sigma
-
-    // ---- next node: start its TMA load (from L2) behind the rest of this node's work --------------
-    if (warp == 0) {
-      if (lane == 0) *sNode = next;
-      load_sigma(next);
+    if (!HERM) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      __syncthreads();                                // every warp is done with the node's sigma
+      // ---- next node: start its TMA load (from L2) behind the rest of this node's work ------------
+      if (warp == 0) {
+        if (lane == 0) *sNode = next;
+        load_sigma(next);
+      }
     }
 
     // ---- couplings to sigma_{u +- e_l}: row b and column b of the neighbour (Eq. 15-17, 23, 25, 35-36) --
+    //      (HERM: the row part only, added to Z; Z^dagger supplies the column part)
     {
       const int64_t e0 = P.lptr[node], e1 = P.lptr[node + 1];
       for (int64_t e = e0; e < e1; ++e) {
@@ -239,10 +254,10 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
         // row factor fr (elements (b, j)) and column factor fc (elements (i, b)) of this link
         double frx, fry, fcy;
         if (ent.z == 0) {                             // "+":  i a+ (delta_ib - delta_bj)
-          const double a = sqrt((double)(ent.w + 1)) * P.cP[l];
+          const double a = sSqrt[ent.w + 1] * P.cP[l];
           frx = 0.0; fry = a; fcy = -a;
         } else {                                      // "-":  i a-x (delta_ib - delta_bj) + a-o (delta_ib + delta_bj)
-          const double sn = sqrt((double)ent.w);
+          const double sn = sSqrt[ent.w];
           frx = sn * P.cO[l]; fry = sn * P.cX[l]; fcy = -fry;
         }
         const double2* nb = p.x + (size_t)ent.x * NN;
@@ -259,7 +274,7 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
             }
           }
         }
-        if (b >= j0w && b < j0w + C::CWc) {           // warp-uniform: this warp owns part of column b
+        if (!HERM && b >= j0w && b < j0w + C::CWc) {  // warp-uniform: this warp owns part of column b
 #pragma unroll
           for (int ct = 0; ct < CT; ++ct) {
             if (j0w + 4 * ct + t == b) {
@@ -272,6 +287,30 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
             }
           }
         }
+      }
+    }
+
+    if (HERM) {
+      // ---- k = Z + Z^dagger through the sigma tile's shared memory (the contraction is done with it) ----
+      __syncthreads();                                // every warp is done with the node's sigma
+#pragma unroll
+      for (int rg = 0; rg < RG; ++rg)
+#pragma unroll
+        for (int ct = 0; ct < CT; ++ct) sS[(i0w + 8 * rg + rho) * SS + j0w + 4 * ct + t] = acc[rg][ct];
+      __syncthreads();
+#pragma unroll
+      for (int rg = 0; rg < RG; ++rg)
+#pragma unroll
+        for (int ct = 0; ct < CT; ++ct) {
+          const double2 zt = sS[(j0w + 4 * ct + t) * SS + i0w + 8 * rg + rho];     // Z[col][row]
+          acc[rg][ct].x += zt.x;
+          acc[rg][ct].y -= zt.y;
+        }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      __syncthreads();                                // the tile may be overwritten
+      if (warp == 0) {
+        if (lane == 0) *sNode = next;
+        load_sigma(next);
       }
     }
 
@@ -314,10 +353,10 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
 template <int N>
 size_t large_smem() {
   using C = LargeCfg<N>;
-  return (size_t)N * C::HS * 8 + (size_t)N * C::SS * 16 + (size_t)N * 8 + 8 + 16;
+  return (size_t)N * C::HS * 8 + (size_t)N * C::SS * 16 + (size_t)N * 8 + 8 + 16 + 258 * 8;
 }
 
-template <int N>
+template <int N, bool HERM>
 cudaError_t launch_large_t(const RhsParams& p, const int64_t* lptr, const int4* lent, const double* Hs_dev,
                            const double* delta_dev, const double* a_plus, const double* a_minus_x,
                            const double* a_minus_o, int sms, unsigned long long* tickets,
@@ -334,12 +373,12 @@ cudaError_t launch_large_t(const RhsParams& p, const int64_t* lptr, const int4* 
     P.cO[l] = on ? a_minus_o[(size_t)l * D1 + 1] : 0.0;
   }
   const size_t smem = large_smem<N>();
-  static bool configured_on[64] = {};     // per device: the attribute belongs to the device's context
+  static bool configured_on[64] = {};     // per device: the attribute belongs to the device's context (one flag per instantiation)
   int dev_ = 0;
   cudaGetDevice(&dev_);
   bool& configured = configured_on[dev_ & 63];
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(rhs_large_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(rhs_large_kernel<N, HERM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
@@ -347,7 +386,7 @@ cudaError_t launch_large_t(const RhsParams& p, const int64_t* lptr, const int4* 
   if (grid < 1) grid = 1;
   P.tickets = tickets;
   P.ticket_base = *ticket_base;
-  rhs_large_kernel<N><<<grid, C::THREADS, smem, s>>>(P);
+  rhs_large_kernel<N, HERM><<<grid, C::THREADS, smem, s>>>(P);
   const cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) {
     *ticket_base += (unsigned long long)p.nodes + (unsigned long long)grid;   // one failing draw per CTA
@@ -364,15 +403,20 @@ bool large_supported(int N, int W) { return (N == 32 || N == 64 || N == 96) && W
 
 cudaError_t launch_rhs_large(const RhsParams& p, const int64_t* lptr, const void* lent, const double* Hs_dev,
                              const double* delta_dev, const double* a_plus, const double* a_minus_x,
-                             const double* a_minus_o, int sms, unsigned long long* tickets,
+                             const double* a_minus_o, int hermitian, int sms, unsigned long long* tickets,
                              unsigned long long* ticket_base, cudaStream_t s) {
   const int4* le = reinterpret_cast<const int4*>(lent);
+#define HEOM_LARGE_CASE(n)                                                                                              \
+  case n:                                                                                                               \
+    return hermitian ? launch_large_t<n, true>(p, lptr, le, Hs_dev, delta_dev, a_plus, a_minus_x, a_minus_o, sms,       \
+                                               tickets, ticket_base, s)                                                 \
+                     : launch_large_t<n, false>(p, lptr, le, Hs_dev, delta_dev, a_plus, a_minus_x, a_minus_o, sms,      \
+                                                tickets, ticket_base, s);
   switch (p.N) {
-    case 32: return launch_large_t<32>(p, lptr, le, Hs_dev, delta_dev, a_plus, a_minus_x, a_minus_o, sms, tickets, ticket_base, s);
-    case 64: return launch_large_t<64>(p, lptr, le, Hs_dev, delta_dev, a_plus, a_minus_x, a_minus_o, sms, tickets, ticket_base, s);
-    case 96: return launch_large_t<96>(p, lptr, le, Hs_dev, delta_dev, a_plus, a_minus_x, a_minus_o, sms, tickets, ticket_base, s);
+    HEOM_LARGE_CASE(32) HEOM_LARGE_CASE(64) HEOM_LARGE_CASE(96)
     default: return cudaErrorInvalidValue;
   }
+#undef HEOM_LARGE_CASE
 }
 
 }  // namespace heom

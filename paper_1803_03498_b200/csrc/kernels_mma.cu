@@ -33,14 +33,18 @@ namespace {
 
 constexpr int kMmaMaxModes = 288;   // W of the constant-bank coupling tables
 constexpr int kMmaMaxBaths = 96;
+constexpr int kMmaStaged = 64;      // link entries of a node staged in shared memory (the rest is read from global)
 
 template <int NP>
 struct MmaCfg {
-  static constexpr int WR = (NP == 96) ? 3 : NP / 16;   // warp grid WR x WC
+#ifndef HEOM_MMA_ROWS
+#define HEOM_MMA_ROWS 16
+#endif
+  static constexpr int WR = (NP == 96) ? 3 : NP / HEOM_MMA_ROWS;   // warp grid WR x WC (16-row warp tiles; 8-row tiles measured 1.4x slower: no A-fragment reuse)
   static constexpr int WC = (NP == 96) ? 4 : 2;
   static constexpr int WARPS = WR * WC;
   static constexpr int THREADS = WARPS * 32;
-  static constexpr int RW = NP / WR;                  // rows per warp (16 or 32)
+  static constexpr int RW = NP / WR;                  // rows per warp (16, or 32 for NP = 96)
   static constexpr int CWc = NP / WC;                 // complex columns per warp
   static constexpr int RG = RW / 8;                   // 8-row groups per warp
   static constexpr int CT = CWc / 4;                  // 4-complex-column tiles per warp (P1 n-tiles)
@@ -54,7 +58,8 @@ struct MmaCfg {
 template <int NP, bool CPLX>
 constexpr size_t mma_smem_bytes() {
   using C = MmaCfg<NP>;
-  return (size_t)NP * C::HS * 8 * (CPLX ? 2 : 1) + (size_t)NP * C::SS * 16 + (size_t)kMmaMaxBaths * 16 + 8 + 16;
+  return (size_t)NP * C::HS * 8 * (CPLX ? 2 : 1) + (size_t)NP * C::SS * 16 + (size_t)kMmaMaxBaths * 16 +
+         2 * ((size_t)kMmaStaged * 16 + 32) + 8 + 16 + 258 * 8;
 }
 template <int NP, bool CPLX>
 constexpr int mma_ctas_per_sm() {
@@ -118,8 +123,13 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
   double* sHi = sH + (CPLX ? NP * HS : 0);                                    // [NP][HS]  Im H / hbar (CPLX)
   double2* sS = reinterpret_cast<double2*>(sHi + NP * HS);                    // [NP][SS]  sigma of the node
   unsigned* sMask = reinterpret_cast<unsigned*>(sS + NP * SS);                // [kMmaMaxBaths][4] membership bits
-  unsigned long long* bar = reinterpret_cast<unsigned long long*>(sMask + 4 * kMmaMaxBaths);
+  // per node parity: {damping rate d_u, first entry e0, entry count} and the first kMmaStaged link entries
+  unsigned char* sLinkBase = reinterpret_cast<unsigned char*>(sMask + 4 * kMmaMaxBaths);
+  constexpr int kLinkBuf = kMmaStaged * 16 + 32;
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(sLinkBase + 2 * kLinkBuf);
   int* sNode = reinterpret_cast<int*>(bar + 1);
+  double* sSqrt = reinterpret_cast<double*>(sNode + 4);                       // [258] sqrt(n), n = 0..D+1 <= 256
+  for (int e = threadIdx.x; e < 258; e += C::THREADS) sSqrt[e] = sqrt((double)e);
 
   for (int e = threadIdx.x; e < NP * HS; e += C::THREADS) {
     const int i = e / HS, j = e % HS;
@@ -153,12 +163,40 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
     const unsigned long long tk = atomicAdd(P.tickets, 1ULL) - P.ticket_base;
     return tk < (unsigned long long)nodes ? (int)tk : nodes;
   };
+  // warp 0 stages a node's header and link entries: fetch() early (registers), publish() behind a CTA barrier
+  struct Staged { double dd; long long e0; int cnt; int4 ent[2]; };
+  auto fetch = [&](int node) {
+    Staged st;
+    st.dd = 0.0; st.e0 = 0; st.cnt = 0;
+    st.ent[0] = make_int4(0, 0, 0, 0); st.ent[1] = make_int4(0, 0, 0, 0);
+    if (node < nodes) {
+      st.e0 = P.lptr[node];
+      st.cnt = (int)(P.lptr[node + 1] - st.e0);
+      st.dd = p.damp[node];
+      if (lane < st.cnt && lane < kMmaStaged) st.ent[0] = __ldg(P.lent + st.e0 + lane);
+      if (lane + 32 < st.cnt && lane + 32 < kMmaStaged) st.ent[1] = __ldg(P.lent + st.e0 + lane + 32);
+    }
+    return st;
+  };
+  auto publish = [&](const Staged& st, int buf) {
+    unsigned char* base = sLinkBase + buf * kLinkBuf;
+    if (lane == 0) {
+      *reinterpret_cast<double*>(base) = st.dd;
+      *reinterpret_cast<long long*>(base + 8) = st.e0;
+      *reinterpret_cast<int*>(base + 16) = st.cnt;
+    }
+    int4* ents = reinterpret_cast<int4*>(base + 32);
+    ents[lane] = st.ent[0];
+    ents[lane + 32] = st.ent[1];
+  };
   if (warp == 0) {
     int first = 0;
     if (lane == 0) { first = draw(); *sNode = first; }
     first = __shfl_sync(0xffffffffu, first, 0);
     load_sigma(first);
+    publish(fetch(first), 0);
   }
+  __syncthreads();
 
   // Eq. 14 table values of this thread's elements are the same for every node: hoisted when the tile is small
   constexpr bool T_IN_REGS = RG * CT <= 12;
@@ -174,12 +212,14 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
   }
 
   unsigned ph = 0;
+  int lbuf = 0;                                       // link-staging buffer of the node in flight
   for (;;) {
     mmbar_wait(bar, ph);                              // sigma of the node has landed (or there is no node)
     ph ^= 1u;
     const int node = *reinterpret_cast<volatile int*>(sNode);
     if (node >= nodes) break;
     int next = nodes;
+    Staged nst;
     if (warp == 0) {
       if (lane == 0) {
         next = draw();
@@ -189,6 +229,7 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
         }
       }
       next = __shfl_sync(0xffffffffu, next, 0);
+      nst = fetch(next);                              // in flight behind this node's contraction
     }
 
     // ---- C = (H/hbar) sigma - sigma (H/hbar) on the FP64 tensor cores (Eq. 12) --------------------
@@ -211,25 +252,39 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
           hA[rg] = *reinterpret_cast<const double2*>(sH + hA_off + rg * 8 * HS + m0);
           if (CPLX) gA[rg] = *reinterpret_cast<const double2*>(sHi + hA_off + rg * 8 * HS + m0);
         }
+        // all B fragments first, then the two k-halves one after the other: RG*CT independent DMMAs lie between two
+        // updates of the same accumulator
+        double b0[CT], b1[CT];
 #pragma unroll
         for (int ct = 0; ct < CT; ++ct) {
-          const double b0 = sBcol[(size_t)(m0 * SS + 4 * ct) * 2];
-          const double b1 = sBcol[(size_t)((m0 + 1) * SS + 4 * ct) * 2];
+          b0[ct] = sBcol[(size_t)(m0 * SS + 4 * ct) * 2];
+          b1[ct] = sBcol[(size_t)((m0 + 1) * SS + 4 * ct) * 2];
+        }
 #pragma unroll
-          for (int rg = 0; rg < RG; ++rg) mdmma(acc[rg][ct].x, acc[rg][ct].y, hA[rg].x, b0);
+        for (int ct = 0; ct < CT; ++ct)
 #pragma unroll
-          for (int rg = 0; rg < RG; ++rg) mdmma(acc[rg][ct].x, acc[rg][ct].y, hA[rg].y, b1);
-          if (CPLX) {
-            // (i Hi) sigma: operand (-Im sigma, Re sigma) = the lane's OTHER component, sign by parity
-            const double* other = (r & 1) ? sBcol - 1 : sBcol + 1;
-            const double sg = (r & 1) ? 1.0 : -1.0;
-            const double d0 = sg * other[(size_t)(m0 * SS + 4 * ct) * 2];
-            const double d1 = sg * other[(size_t)((m0 + 1) * SS + 4 * ct) * 2];
+          for (int rg = 0; rg < RG; ++rg) mdmma(acc[rg][ct].x, acc[rg][ct].y, hA[rg].x, b0[ct]);
 #pragma unroll
-            for (int rg = 0; rg < RG; ++rg) mdmma(acc[rg][ct].x, acc[rg][ct].y, gA[rg].x, d0);
+        for (int ct = 0; ct < CT; ++ct)
 #pragma unroll
-            for (int rg = 0; rg < RG; ++rg) mdmma(acc[rg][ct].x, acc[rg][ct].y, gA[rg].y, d1);
+          for (int rg = 0; rg < RG; ++rg) mdmma(acc[rg][ct].x, acc[rg][ct].y, hA[rg].y, b1[ct]);
+        if (CPLX) {
+          // (i Hi) sigma: operand (-Im sigma, Re sigma) = the lane's OTHER component, sign by parity
+          const double* other = (r & 1) ? sBcol - 1 : sBcol + 1;
+          const double sg = (r & 1) ? 1.0 : -1.0;
+#pragma unroll
+          for (int ct = 0; ct < CT; ++ct) {
+            b0[ct] = sg * other[(size_t)(m0 * SS + 4 * ct) * 2];
+            b1[ct] = sg * other[(size_t)((m0 + 1) * SS + 4 * ct) * 2];
           }
+#pragma unroll
+          for (int ct = 0; ct < CT; ++ct)
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) mdmma(acc[rg][ct].x, acc[rg][ct].y, gA[rg].x, b0[ct]);
+#pragma unroll
+          for (int ct = 0; ct < CT; ++ct)
+#pragma unroll
+            for (int rg = 0; rg < RG; ++rg) mdmma(acc[rg][ct].x, acc[rg][ct].y, gA[rg].y, b1[ct]);
         }
       }
 #pragma unroll
@@ -264,7 +319,8 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
     }
 
     // ---- k = -i C - (d_u + T) o sigma (Eq. 13-14), in the fragment layout ---------------------------
-    const double dd = p.damp[node];
+    const unsigned char* lhead = sLinkBase + lbuf * kLinkBuf;
+    const double dd = *reinterpret_cast<const double*>(lhead);
 #pragma unroll
     for (int rg = 0; rg < RG; ++rg) {
       const int row = i0w + 8 * rg + rho;
@@ -285,19 +341,23 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
     if (warp == 0) {
       if (lane == 0) *sNode = next;
       load_sigma(next);
+      publish(nst, lbuf ^ 1);                         // read after the next node's barrier
     }
 
     // ---- couplings to sigma_{u +- e_l} (Eq. 15-17, 23, 25, 35-36, summed over the bath's states) ------
     {
-      const int64_t e0 = P.lptr[node], e1 = P.lptr[node + 1];
-      for (int64_t e = e0; e < e1; ++e) {
-        const int4 ent = P.lent[e];
+      const long long e0 = *reinterpret_cast<const long long*>(lhead + 8);
+      const int cnt = *reinterpret_cast<const int*>(lhead + 16);
+      const int4* staged = reinterpret_cast<const int4*>(lhead + 32);
+#pragma unroll 2
+      for (int q = 0; q < cnt; ++q) {
+        const int4 ent = q < kMmaStaged ? staged[q] : __ldg(P.lent + e0 + q);
         const int l = ent.y, b = l / p.M;
         // element factor = i fx (q_i - q_j) + fo (q_i + q_j)
         double fx, fo;
-        if (ent.z == 0) { fx = sqrt((double)(ent.w + 1)) * P.cP[l]; fo = 0.0; }               // "+"
-        else { const double sn = sqrt((double)ent.w); fx = sn * P.cX[l]; fo = sn * P.cO[l]; }   // "-"
-        // membership bits of the warp's rows (one 32-bit word: the row tile starts at a multiple of 16 and is 16 or
+        if (ent.z == 0) { fx = sSqrt[ent.w + 1] * P.cP[l]; fo = 0.0; }                         // "+"
+        else { const double sn = sSqrt[ent.w]; fx = sn * P.cX[l]; fo = sn * P.cO[l]; }           // "-"
+        // membership bits of the warp's rows (one 32-bit word: the row tile starts at a multiple of 8 and is 8 or
         // 32 rows long) and of its columns (a 64-bit window starting at column j0w)
         const unsigned rbits = sMask[b * 4 + (i0w >> 5)] >> (i0w & 31);
         const unsigned long long cbits =
@@ -316,8 +376,9 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
             const unsigned qj = (qc >> ct) & 1u;
             const int col = j0w + 4 * ct + t;
             if ((qr | qj) && col < N) {
-              const double vx = (double)qr - (double)qj, vo = (double)(qr + qj);
-              const double fr = fo * vo, fi = fx * vx;
+              // i fx (q_i - q_j) + fo (q_i + q_j) with q in {0, 1}
+              const double fi = (qr == qj) ? 0.0 : (qr ? fx : -fx);
+              const double fr = (qr & qj) ? 2.0 * fo : fo;
               const double2 w = __ldg(nb + (size_t)row * N + col);
               acc[rg][ct].x = fma(fr, w.x, fma(-fi, w.y, acc[rg][ct].x));
               acc[rg][ct].y = fma(fr, w.y, fma(fi, w.x, acc[rg][ct].y));
@@ -326,6 +387,8 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
         }
       }
     }
+
+    lbuf ^= 1;
 
     // ---- fused RK4 stage epilogue straight from the fragment layout ------------------------------------
     const size_t nbase = (size_t)node * NN;

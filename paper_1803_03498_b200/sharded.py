@@ -22,25 +22,50 @@ def halo_all_to_all(buf, send, n_owned, send_counts, recv_counts, group=None):
                            input_split_sizes=[int(c) for c in send_counts], group=group)
 
 
+def slice_all_to_all(recv, send, per, send_counts, recv_counts, group=None):
+    """Slice halo: `per` complex128 per (node, state) pair; send / recv are flat float64 buffers of packed pairs
+    grouped by destination / source rank.  One all_to_all_single."""
+    import torch.distributed as dist
+    n_send, n_recv = int(np.sum(send_counts)) * 2 * per, int(np.sum(recv_counts)) * 2 * per
+    dist.all_to_all_single(recv[:n_recv], send[:n_send],
+                           output_split_sizes=[int(c) * 2 * per for c in recv_counts],
+                           input_split_sizes=[int(c) * 2 * per for c in send_counts], group=group)
+
+
 class ShardedHeom:
-    """Rank `rank` of `world`: a partition context + the exchange.  group=None: the default process group."""
+    """Rank `rank` of `world`: a partition context + the exchange.  group=None: the default process group.
+    halo = "slices" (default): only row s -- and column s for states that are not exactly Hermitian -- of every
+    (ghost, state) pair a gather reads crosses the link (heom_pack_halo_slices / heom_unpack_halo_slices around one
+    all_to_all_single); halo = "nodes": whole N x N ghost nodes, received in place (no unpack kernel)."""
 
     def __init__(self, H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, rank, world, device=0, bath_state=None,
-                 group=None, **options):
-        self.rank, self.world, self.group = int(rank), int(world), group
+                 group=None, halo="slices", **options):
+        self.rank, self.world, self.group, self.halo = int(rank), int(world), group, halo
         self.g = Heom(H_cm, lambda_cm, nu_per_fs, T_kelvin, K, D, device=device, bath_state=bath_state,
                       partition=(rank, world), **options)
         self.n_owned = self.g.owned()
         self.global_ids, self.send_counts, self.recv_counts, self.send_idx = self.g.partition_plan()
-        self._send = None
+        self.pair_send_counts, self.pair_recv_counts = self.g.partition_plan_slices()[:2]
+        self._send = self._recv = None
 
     def bind(self, stream=None):
         import torch
         self.g.bind(stream=stream)
-        rows = max(1, int(self.send_counts.sum()))
-        self._send = torch.empty((rows, 2 * self.g.N * self.g.N), dtype=torch.float64,
-                                 device=self.g._workspace.device)
+        dev = self.g._workspace.device
+        if self.halo == "nodes":
+            rows = max(1, int(self.send_counts.sum()))
+            self._send = torch.empty((rows, 2 * self.g.N * self.g.N), dtype=torch.float64, device=dev)
+        else:
+            per = 2 * 2 * self.g.N          # float64 per pair at most (row + column, complex)
+            self._send = torch.empty(max(1, int(self.pair_send_counts.sum())) * per, dtype=torch.float64, device=dev)
+            self._recv = torch.empty(max(1, int(self.pair_recv_counts.sum())) * per, dtype=torch.float64, device=dev)
         return self
+
+    def halo_bytes_per_stage(self):
+        """Bytes this rank sends per stage with the halo in use (plan count, not a measurement)."""
+        if self.halo == "nodes":
+            return int(self.send_counts.sum()) * 16 * self.g.N * self.g.N
+        return int(self.pair_send_counts.sum()) * 16 * self.g.halo_slice_elements()
 
     # -- state ----------------------------------------------------------------------------------
     def set_state(self, sigma0):
@@ -71,10 +96,16 @@ class ShardedHeom:
         import torch
         with torch.cuda.stream(self.g._stream):
             ptr = self.g.stage_output(stage)
-            buf = self.g.buffer_view(ptr)
-            if int(self.send_counts.sum()):
-                self.g.pack_halo(ptr, self._send.data_ptr())
-            halo_all_to_all(buf, self._send, self.n_owned, self.send_counts, self.recv_counts, self.group)
+            if self.halo == "nodes":
+                buf = self.g.buffer_view(ptr)
+                if int(self.send_counts.sum()):
+                    self.g.pack_halo(ptr, self._send.data_ptr())
+                halo_all_to_all(buf, self._send, self.n_owned, self.send_counts, self.recv_counts, self.group)
+            else:
+                per = self.g.halo_slice_elements()
+                self.g.pack_halo_slices(ptr, self._send.data_ptr())
+                slice_all_to_all(self._recv, self._send, per, self.pair_send_counts, self.pair_recv_counts, self.group)
+                self.g.unpack_halo_slices(self._recv.data_ptr(), ptr)
 
     def rk4_steps(self, dt_fs, nsteps):
         import torch
@@ -101,6 +132,27 @@ class ShardedHeom:
         if name == "g":
             raise AttributeError(name)
         return getattr(self.g, name)
+
+
+def slice_plan_check(parts):
+    """Host-side consistency of the slice-halo plans (tests): the (node, state) pairs rank p sends to r are, pair
+    for pair and in order, the pairs r expects from p.  parts[r] = (global_ids, plan_slices tuple)."""
+    world = len(parts)
+    for r in range(world):
+        gid_r, (sc_r, rc_r, sn_r, ss_r, rn_r, rs_r) = parts[r]
+        roff = 0
+        for p in range(world):
+            gid_p, (sc_p, rc_p, sn_p, ss_p, rn_p, rs_p) = parts[p]
+            soff = int(sc_p[:r].sum())
+            n = int(sc_p[r])
+            if n != int(rc_r[p]):
+                return False
+            if not np.array_equal(gid_p[sn_p[soff:soff + n]], gid_r[rn_r[roff:roff + n]]):
+                return False
+            if not np.array_equal(ss_p[soff:soff + n], rs_r[roff:roff + n]):
+                return False
+            roff += n
+    return True
 
 
 def exchange_plan_check(plans):

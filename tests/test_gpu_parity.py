@@ -15,7 +15,7 @@ from oracle.oracle import Oracle
 
 pytestmark = pytest.mark.gpu
 
-HERM_KERNELS = ("rhs_hpipe_kernel",)   # exact-Hermiticity-preserving kernels
+HERM_KERNELS = ("rhs_hpipe_kernel", "rhs_large_herm_kernel")   # exact-Hermiticity-preserving kernels
 RHS_TOL = 1e-13
 STATE_TOL = 1e-10
 

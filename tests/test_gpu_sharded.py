@@ -21,16 +21,40 @@ def rel_err(a, b):
 
 
 class LocalWorld:
-    def __init__(self, w, world, bath_state=None, **opts):
+    def __init__(self, w, world, bath_state=None, halo="nodes", **opts):
         from paper_1803_03498_b200 import Heom
-        self.world = world
+        self.world, self.halo = world, halo
         self.parts = [Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, partition=(r, world),
                            bath_state=bath_state, **opts).bind(poison=True) for r in range(world)]
         self.plans = [g.partition_plan() for g in self.parts]
         self.send = [torch.full((max(1, int(p[1].sum())), 2 * g.N * g.N), float("nan"), dtype=torch.float64, device="cuda")
                      for g, p in zip(self.parts, self.plans)]
+        self.splans = [g.partition_plan_slices() for g in self.parts]
+        self.ssend = [torch.full((max(1, int(p[0].sum())) * 4 * g.N,), float("nan"), dtype=torch.float64, device="cuda")
+                      for g, p in zip(self.parts, self.splans)]
+        self.srecv = [torch.full((max(1, int(p[1].sum())) * 4 * g.N,), float("nan"), dtype=torch.float64, device="cuda")
+                      for g, p in zip(self.parts, self.splans)]
+
+    def exchange_slices(self, ptrs):
+        """What ShardedHeom.exchange does with halo="slices": pack, move exactly the packed pairs, unpack."""
+        for g, s, p in zip(self.parts, self.ssend, ptrs):
+            g.pack_halo_slices(p, s.data_ptr())
+        torch.cuda.synchronize()
+        for r, g in enumerate(self.parts):
+            per = 2 * g.halo_slice_elements()                       # float64 per pair
+            roff = 0
+            for p in range(self.world):
+                n = int(self.splans[r][1][p]) * per
+                soff = int(self.splans[p][0][:r].sum()) * per
+                assert n == int(self.splans[p][0][r]) * per
+                self.srecv[r][roff:roff + n] = self.ssend[p][soff:soff + n]
+                roff += n
+            g.unpack_halo_slices(self.srecv[r].data_ptr(), ptrs[r])
+        torch.cuda.synchronize()
 
     def exchange(self, ptrs):
+        if self.halo == "slices":
+            return self.exchange_slices(ptrs)
         for g, s, p in zip(self.parts, self.send, ptrs):
             if g.partition_plan()[1].sum():
                 g.pack_halo(p, s.data_ptr())
@@ -74,11 +98,11 @@ class LocalWorld:
 @pytest.mark.parametrize("name,D,steps,world", [("cfg2", 4, 100, 2), ("cfg2", 4, 60, 5), ("cfg3", 5, 60, 3),
                                                 ("cfg4", 3, 60, 4), ("cfg5", 1, 20, 2), ("cfg5", 2, 2, 3),
                                                 ("cfg1", 4, 200, 3)])
-@pytest.mark.parametrize("herm,form", [(1, -1), (0, -1), (1, 0)])
-def test_sharded_rk4_parity(name, D, steps, world, herm, form):
+@pytest.mark.parametrize("herm,form,halo", [(1, -1, "slices"), (0, -1, "slices"), (1, 0, "nodes")])
+def test_sharded_rk4_parity(name, D, steps, world, herm, form, halo):
     w = workloads.get(name).with_(D=D)
     o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D)
-    lw = LocalWorld(w, world, hermitian=herm, rk4_form=form)
+    lw = LocalWorld(w, world, halo=halo, hermitian=herm, rk4_form=form)
     assert sum(g.owned() for g in lw.parts) == o.nodes
     # a single right-hand side on a dense random state first (ghost rows of the result are not meaningful)
     st = workloads.random_state(o.nodes, w.N, seed=5)
@@ -91,10 +115,12 @@ def test_sharded_rk4_parity(name, D, steps, world, herm, form):
     assert rel_err(got, ref) < STATE_TOL
     pop, tr = lw.parts[0].populations()                             # rank 0 owns sigma_0
     assert abs(tr - 1.0) < 1e-11 and np.allclose(pop, np.diag(ref[0]).real, atol=1e-11)
-    # ghost copies agree with their owners' rows after the last exchange
+    # ghost copies agree with their owners' rows after the last exchange (whole-node halo; the slice halo
+    # refreshes only the rows and columns the gathers read)
     for g, p in zip(lw.parts, lw.plans):
-        loc = g.get_full_state()
-        assert rel_err(loc, ref[p[0]]) < STATE_TOL
+        if halo == "nodes":
+            loc = g.get_full_state()
+            assert rel_err(loc, ref[p[0]]) < STATE_TOL
         assert g.workspace_guard_intact()                           # nothing wrote past the workspace
 
 

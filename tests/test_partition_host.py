@@ -10,7 +10,7 @@ import torch.multiprocessing as mp
 
 from oracle.oracle import Oracle
 from paper_1803_03498_b200 import Heom, HeomError
-from paper_1803_03498_b200.sharded import exchange_plan_check
+from paper_1803_03498_b200.sharded import exchange_plan_check, slice_plan_check
 
 
 def _parts(N, K, D, world, bath_state=None):
@@ -51,6 +51,35 @@ def test_partition_tables_vs_oracle(N, K, D, world):
     assert sum(1 for g in parts if g.owned() and 0 in g.partition_plan()[0][:g.owned()]) == 1
 
 
+@pytest.mark.parametrize("N,K,D,world,bath_state", [(2, 1, 4, 2, None), (7, 1, 3, 4, None), (3, 2, 5, 8, None),
+                                                    (14, 0, 3, 5, None), (4, 1, 3, 3, [1, 2, 3])])
+def test_slice_halo_plan(N, K, D, world, bath_state):
+    """The slice halo: (ghost, state) pairs are exactly what the owned nodes' links read, each once; sender and
+    receiver lists agree pair for pair; never more rows than whole ghost nodes would carry."""
+    parts = _parts(N, K, D, world, bath_state=bath_state)
+    M = K + 1
+    states = list(range(N)) if bath_state is None else bath_state
+    info = []
+    for r, g in enumerate(parts):
+        gid, sc, rc, idx = g.partition_plan()
+        ps = g.partition_plan_slices()
+        psc, prc, sn, ss, rn, rs = ps
+        n_own = g.owned()
+        lt, lp, lm = g.tables()
+        want = set()
+        for tab in (lp, lm):
+            u, l = np.nonzero(tab[:n_own] >= n_own)                # links of owned nodes into the ghost region
+            want |= set(zip(tab[u, l].tolist(), [states[x // M] for x in l.tolist()]))
+        got = list(zip(rn.tolist(), rs.tolist()))
+        assert len(got) == len(set(got)) and set(got) == want      # every pair once, nothing else
+        assert psc[r] == 0 and prc[r] == 0
+        assert sn.size == psc.sum() and (sn.size == 0 or (sn.min() >= 0 and sn.max() < n_own))
+        assert rn.size == 0 or rn.min() >= n_own
+        assert len(got) <= (g.nodes - n_own) * N                   # at most every row of every ghost
+        info.append((gid, ps))
+    assert slice_plan_check(info)
+
+
 def test_partition_with_site_map_and_validation():
     parts = _parts(4, 1, 3, 2, bath_state=[1, 2, 3])
     o = Oracle(np.zeros((4, 4)), 35.0, 0.02, 300.0, 1, 3, bath_state=[1, 2, 3])
@@ -87,7 +116,18 @@ def _worker(rank, world, port, q):
         send = buf[torch.from_numpy(idx.astype(np.int64))].contiguous() if idx.size else torch.empty((1, 4), dtype=torch.float64)
         halo_all_to_all(buf, send, n_own, sc, rc)
         ok = ok and bool(torch.equal(buf[:, 0], torch.from_numpy(gid.astype(np.float64)) * (rnd + 1)))
-    q.put((rank, ok, int(g.nodes - n_own)))
+    # the slice halo through the same collective: payload = (global id, state) of every pair, twice per element
+    from paper_1803_03498_b200.sharded import slice_all_to_all
+    psc, prc, sn, ss, rn, rs = g.partition_plan_slices()
+    per = 3                                                         # stands for N complex elements
+    send = np.zeros((max(1, sn.size), per, 2))
+    send[:sn.size, :, 0] = gid[sn][:, None]
+    send[:sn.size, :, 1] = ss[:, None]
+    recv = torch.full((max(1, rn.size) * per * 2,), -1.0, dtype=torch.float64)
+    slice_all_to_all(recv, torch.from_numpy(send.reshape(-1)).contiguous(), per, psc, prc)
+    got = recv.numpy().reshape(-1, per, 2)[:rn.size]
+    ok = ok and np.array_equal(got[:, 0, 0], gid[rn].astype(np.float64)) and np.array_equal(got[:, 2, 1], rs.astype(np.float64))
+    q.put((rank, bool(ok), int(g.nodes - n_own)))
     dist.destroy_process_group()
 
 
