@@ -65,7 +65,7 @@ template <int NP, bool CPLX>
 constexpr int mma_ctas_per_sm() {
   constexpr size_t per = mma_smem_bytes<NP, CPLX>() + 1024;            // + the runtime's per-CTA reservation
   constexpr int by_smem = (int)((size_t)227 * 1024 / per);
-  constexpr int by_threads = 1536 / MmaCfg<NP>::THREADS;
+  constexpr int by_threads = 512 / MmaCfg<NP>::THREADS;              // >= 128 registers per thread
   constexpr int m = by_smem < by_threads ? by_smem : by_threads;
   return m < 1 ? 1 : (m > 4 ? 4 : m);
 }
@@ -349,37 +349,45 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
       const long long e0 = *reinterpret_cast<const long long*>(lhead + 8);
       const int cnt = *reinterpret_cast<const int*>(lhead + 16);
       const int4* staged = reinterpret_cast<const int4*>(lhead + 32);
+      // Small tiles (DENSE_LINKS), branch-free per link: every thread loads all RG*CT of its elements (an inactive one
+      // reads element 0 of the neighbour, warp-wide the same address, and gets a zero factor), so that the loads of a
+      // link -- and, with the loop unrolled by two, of two links -- are in flight together.  Membership bits exist only for real states,
+      // so padded rows and columns are inactive by construction.
+      constexpr bool DENSE_LINKS = RG * CT <= 12;
+      const unsigned rsel = ((C::RW == 32) ? 0xffffffffu : ((1u << C::RW) - 1u));
+      const unsigned long long csel = (1ULL << C::CWc) - 1ULL;
 #pragma unroll 2
       for (int q = 0; q < cnt; ++q) {
         const int4 ent = q < kMmaStaged ? staged[q] : __ldg(P.lent + e0 + q);
         const int l = ent.y, b = l / p.M;
-        // element factor = i fx (q_i - q_j) + fo (q_i + q_j)
+        const unsigned rbits = (sMask[b * 4 + (i0w >> 5)] >> (i0w & 31)) & rsel;
+        const unsigned long long cbits =
+            ((((unsigned long long)sMask[b * 4 + (j0w >> 5) + 1] << 32) | sMask[b * 4 + (j0w >> 5)]) >> (j0w & 31)) & csel;
+        if (rbits == 0u && cbits == 0ULL) continue;   // warp-uniform: the link does not touch this warp's tile
+        // element factor = i fx (q_i - q_j) + fo (q_i + q_j), q in {0, 1}
         double fx, fo;
         if (ent.z == 0) { fx = sSqrt[ent.w + 1] * P.cP[l]; fo = 0.0; }                         // "+"
         else { const double sn = sSqrt[ent.w]; fx = sn * P.cX[l]; fo = sn * P.cO[l]; }           // "-"
-        // membership bits of the warp's rows (one 32-bit word: the row tile starts at a multiple of 8 and is 8 or
-        // 32 rows long) and of its columns (a 64-bit window starting at column j0w)
-        const unsigned rbits = sMask[b * 4 + (i0w >> 5)] >> (i0w & 31);
-        const unsigned long long cbits =
-            (((unsigned long long)sMask[b * 4 + (j0w >> 5) + 1] << 32) | sMask[b * 4 + (j0w >> 5)]) >> (j0w & 31);
-        unsigned qc = 0u;                             // membership of this thread's columns, bit ct
-#pragma unroll
-        for (int ct = 0; ct < CT; ++ct) qc |= (unsigned)((cbits >> (4 * ct + t)) & 1ULL) << ct;
         const double2* nb = p.x + (size_t)ent.x * NN;
 #pragma unroll
         for (int rg = 0; rg < RG; ++rg) {
           const int row = i0w + 8 * rg + rho;
-          const unsigned qr = (rbits >> (8 * rg + rho)) & 1u;
-          if (!(qr | qc) || row >= N) continue;
+          const bool qr = (rbits >> (8 * rg + rho)) & 1u;
+          // (re, im) factor of the element for q_j = 0 and for q_j = 1
+          const double a0r = qr ? fo : 0.0, a0i = qr ? fx : 0.0;
+          const double a1r = qr ? 2.0 * fo : fo, a1i = qr ? 0.0 : -fx;
 #pragma unroll
           for (int ct = 0; ct < CT; ++ct) {
-            const unsigned qj = (qc >> ct) & 1u;
             const int col = j0w + 4 * ct + t;
-            if ((qr | qj) && col < N) {
-              // i fx (q_i - q_j) + fo (q_i + q_j) with q in {0, 1}
-              const double fi = (qr == qj) ? 0.0 : (qr ? fx : -fx);
-              const double fr = (qr & qj) ? 2.0 * fo : fo;
-              const double2 w = __ldg(nb + (size_t)row * N + col);
+            const bool qj = (cbits >> (4 * ct + t)) & 1ULL;
+            const double fr = qj ? a1r : a0r, fi = qj ? a1i : a0i;
+            if (DENSE_LINKS) {
+              const int off = (qr | qj) ? row * N + col : 0;
+              const double2 w = __ldg(nb + off);
+              acc[rg][ct].x = fma(fr, w.x, fma(-fi, w.y, acc[rg][ct].x));
+              acc[rg][ct].y = fma(fr, w.y, fma(fi, w.x, acc[rg][ct].y));
+            } else if (qr | qj) {                     // large tiles: few of a thread's elements are touched
+              const double2 w = __ldg(nb + row * N + col);
               acc[rg][ct].x = fma(fr, w.x, fma(-fi, w.y, acc[rg][ct].x));
               acc[rg][ct].y = fma(fr, w.y, fma(fi, w.x, acc[rg][ct].y));
             }
