@@ -32,9 +32,9 @@ import workloads  # noqa: E402
 METRIC = "heom_node_updates_per_s"
 UNIT = "node-updates/s"
 # per_config: steps per chunk of the short runs of the non-headline configs
-SHORT_STEPS = {"cfg1": 1000, "cfg2": 200, "cfg3": 8, "cfg4": 50, "cfg5": 2, "absorb": 200, "twoex": 50}
+SHORT_STEPS = {"cfg1": 1000, "cfg2": 200, "cfg3": 8, "cfg4": 50, "cfg5": 2, "absorb": 200, "twoex": 50, "mid24": 20}
 SEEDS = {"cfg1": None, "cfg2": workloads.SEED_FMO, "cfg3": workloads.SEED_FMO, "cfg4": workloads.SEED_LHCII,
-         "cfg5": workloads.SEED_LARGE, "absorb": workloads.SEED_FMO, "twoex": workloads.SEED_FMO}
+         "cfg5": workloads.SEED_LARGE, "absorb": workloads.SEED_FMO, "twoex": workloads.SEED_FMO, "mid24": workloads.SEED_LHCII + 7}
 
 
 def measured_peaks():
@@ -169,6 +169,7 @@ def run_reference(args, w):
 def config_dict(w, key, n_gpus, shard=False):
     origin = (f"BASELINE.json configs[{list(workloads.CONFIGS).index(key)}]" if key in workloads.CONFIGS
               else "two-exciton space of configs[1]'s H (29 states, P:471-481, Eq. 54; not a BASELINE config)" if key == "twoex"
+              else "mid-size site-map system, configs[3]'s generator at 24 sites (not a BASELINE config)" if key == "mid24"
               else "linear-absorption variant of configs[1] (ground state + 7 sites, sigma_0(0) = mu_z|0><0|; not a BASELINE config)")
     return {"workload": f"{w.name}: {origin} "
                         f"N={w.N} K={w.K} D={w.D} T={w.T_kelvin:g}K nodes={w.nodes} dt={w.dt_fs}fs",
@@ -274,6 +275,20 @@ def run_config(key, args, steps, ctx, with_e2e=True, with_cpu=True, options=None
                "h2d_bytes_per_step": 16 * w.N * w.N / e_steps, "d2h_bytes_per_step": 8 * (w.N + 2),
                "what": "heom_set_state(HOST sigma_0) once, then per step heom_rk4_steps(dt,1) + "
                        "heom_populations -> HOST; host wall clock"}
+    stability = None
+    if key == "cfg3" and not shard:
+        # SURVEY.md 8(c) A7 / BASELINE.md: config 3 as specified (dt = 1 fs: dt * max d_u = 2.96 is outside RK4's
+        # stability region, R8) with max|sigma| per hierarchy level logged, and the stable variant
+        # (dt = 0.9 fs) alongside; same kernel, same launches, same throughput -- only the growth differs
+        stability = {}
+        for dt in (w.dt_fs, 0.9):
+            g.set_state(sigma0)
+            with torch.cuda.stream(stream):
+                g.rk4_steps(dt, w.steps)
+            lm = g.level_max()
+            pop_s, tr_s = g.populations()
+            stability[f"dt={dt}fs"] = {"steps": w.steps, "max_abs_per_level": [float(f"{v:.3e}") for v in lm],
+                                       "trace_minus_1": tr_s.real - 1.0, "rho11": float(pop_s[0])}
     kernel_name = g.kernel_name()
     n_owned = g.n_owned if shard else w.nodes
     g.close()
@@ -348,6 +363,8 @@ def run_config(key, args, steps, ctx, with_e2e=True, with_cpu=True, options=None
              "check": {"trace": [tr.real, tr.imag], "rho11": float(pop[0])}}
     if e2e:
         block["e2e"] = e2e
+    if stability:
+        block["stability"] = stability
     if with_cpu and world == 1:
         block["cpu_baseline"] = oracle_throughput(w, target_seconds=args.cpu_seconds)
     return block

@@ -175,6 +175,11 @@ heom_status heom_sync(heom_ctx* ctx);
 heom_status heom_populations(heom_ctx* ctx, double* pop, double* trace_re,
                              double* trace_im);
 
+/* Growth monitor (Eq. 38: dt << 1/gamma_k; config 3 at dt = 1 fs lies outside RK4's
+ * stability region): max_abs[L] = max over the nodes of hierarchy level L (sum n = L) and their elements of
+ * max(|Re|, |Im|), L = 0..D (HOST [D+1]); +inf if a NaN or Inf is present.  Device reduction; synchronises. */
+heom_status heom_level_max(heom_ctx* ctx, double* max_abs);
+
 /* Tr(A sigma_0) = sum_ij A[i][j] sigma_0[j][i]: the integrand of the dipole correlation function of
  * Eq. 56 with A = mu_p.  A HOST [N][N] complex128 row-major; re, im HOST (may be NULL).
  * Computed by a device reduction kernel; synchronises. */

@@ -24,7 +24,7 @@ SYMBOLS = [
     "heom_set_state", "heom_set_full_state", "heom_get_full_state", "heom_rhs", "heom_rk4_steps",
     "heom_sync", "heom_populations", "heom_launch_count", "heom_kernel_time", "heom_kernel_name",
     "heom_last_error", "heom_probe_peak", "heom_create_general", "heom_set_hamiltonian",
-    "heom_partition_plan_slices", "heom_halo_slice_elements", "heom_pack_halo_slices", "heom_unpack_halo_slices",
+    "heom_level_max", "heom_partition_plan_slices", "heom_halo_slice_elements", "heom_pack_halo_slices", "heom_unpack_halo_slices",
 ]
 
 _lib = None
@@ -59,6 +59,7 @@ def load_library():
     lib.heom_partition_owned.argtypes = [P]
     lib.heom_partition_owned.restype = C.c_int64
     lib.heom_partition_plan.argtypes = [P, P, P, P, P]
+    lib.heom_level_max.argtypes = [P, P]
     lib.heom_partition_plan_slices.argtypes = [P, P, P, P, P, P, P]
     lib.heom_halo_slice_elements.argtypes = [P]
     lib.heom_pack_halo_slices.argtypes = [P, P, P]
@@ -348,6 +349,12 @@ class Heom:
         off = int(dev_ptr) - self._workspace.data_ptr()
         nbytes = self.nodes * self.N * self.N * 16
         return self._workspace[off:off + nbytes].view(torch.float64).view(self.nodes, 2 * self.N * self.N)
+
+    def level_max(self):
+        """heom_level_max: max(|Re|, |Im|) over the nodes of every hierarchy level, L = 0..D."""
+        out = np.zeros(self.D + 1)
+        self._ck(self._lib.heom_level_max(self._h, out.ctypes.data))
+        return out
 
     def expectation(self, A):
         """Tr(A sigma_0) (heom_expectation)."""

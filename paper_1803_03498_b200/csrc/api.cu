@@ -83,6 +83,8 @@ struct heom_ctx {
   bool partitioned = false;
   int part_rank = 0, part_world = 1;
   Partition part;
+  uint8_t* d_level = nullptr;         // hierarchy level of every storage slot (heom_level_max)
+  unsigned long long* d_lmax = nullptr;   // [256] scratch of heom_level_max
   int32_t* d_send = nullptr; // DEVICE copy of part.send_idx
   int32_t *d_spn = nullptr, *d_sps = nullptr, *d_rpn = nullptr, *d_rps = nullptr;   // slice-halo pair lists
   size_t n_links = 0;
@@ -194,7 +196,7 @@ int node_stride(int N) { return N * N; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_linksP, off_Hs, off_delta, off_Him, off_gen, off_A, off_S0, off_send, off_pairs, off_lptr, off_lent, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_linksP, off_Hs, off_delta, off_Him, off_gen, off_A, off_S0, off_level, off_send, off_pairs, off_lptr, off_lent, total;
 };
 
 // Which kernel family the bound configuration will run (fixed by the shape and the "kernel" option), so that the
@@ -241,6 +243,7 @@ Layout layout_of(const heom_ctx* c) {
   L.off_gen = o; o += align_up((N + 1) * 4) + align_up(c->sbl.size() * 4 + 16) + align_up((size_t)c->B * 16 + 16);
   L.off_A = o; o += align_up(N * N * 16);
   L.off_S0 = o; o += align_up(N * N * 16);
+  L.off_level = o; o += align_up(nodes + 16) + align_up(256 * 8);
   L.off_send = o; o += align_up(c->part.send_idx.size() * 4 + 16);
   L.off_pairs = o; o += 2 * align_up(c->part.send_pair_node.size() * 4 + 16) + 2 * align_up(c->part.recv_pair_node.size() * 4 + 16);
   if (kc.large || kc.mma) {
@@ -660,6 +663,17 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   }
   ctx->d_A = (double2*)(base + L.off_A);
   ctx->d_S0 = (double2*)(base + L.off_S0);
+  ctx->d_level = (uint8_t*)(base + L.off_level);
+  ctx->d_lmax = (unsigned long long*)(base + L.off_level + align_up((size_t)ctx->h.nodes + 16));
+  {
+    std::vector<uint8_t> lev((size_t)ctx->h.nodes, 0);
+    for (int64_t u = 0; u < ctx->h.nodes; ++u) {
+      int Ls = 0;
+      for (int l = 0; l < ctx->h.W; ++l) Ls += ctx->h.tuples[(size_t)u * ctx->h.W + l];
+      lev[(size_t)ctx->h.slot_of[(size_t)u]] = (uint8_t)Ls;
+    }
+    CU(cudaMemcpy(ctx->d_level, lev.data(), lev.size(), cudaMemcpyHostToDevice));
+  }
   ctx->d_send = (int32_t*)(base + L.off_send);
   if (!ctx->part.send_idx.empty())
     CU(cudaMemcpy(ctx->d_send, ctx->part.send_idx.data(), ctx->part.send_idx.size() * 4, cudaMemcpyHostToDevice));
@@ -1067,6 +1081,23 @@ heom_status heom_populations(heom_ctx* ctx, double* pop, double* trace_re, doubl
   if (pop) std::memcpy(pop, ctx->h_pinned, (size_t)N * 8);
   if (trace_re) *trace_re = ctx->h_pinned[N];
   if (trace_im) *trace_im = ctx->h_pinned[N + 1];
+  return HEOM_OK;
+}
+
+heom_status heom_level_max(heom_ctx* ctx, double* max_abs) {
+  if (!ctx || !max_abs) return HEOM_EINVAL;
+  if (!ctx->bound || !ctx->have_state) return fail(ctx, HEOM_ESTATE, "no state set");
+  const bool ket = ctx->ket_col >= 0;
+  // a partition reports its owned nodes (ghost rows are copies)
+  const long long n = ctx->partitioned ? (long long)ctx->part.n_owned : (long long)ctx->h.nodes;
+  CU(cudaMemsetAsync(ctx->d_lmax, 0, 256 * 8, ctx->stream));
+  CU(launch_level_max(ket ? ket_buf(ctx, KET_Y) : ctx->y, ctx->d_level, n, ket ? ctx->h.N : ctx->h.N * ctx->h.N,
+                      ctx->d_lmax, ctx->stream));
+  ctx->launches += 1;
+  unsigned long long bits[256];
+  CU(cudaMemcpyAsync(bits, ctx->d_lmax, 256 * 8, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  for (int L = 0; L <= ctx->h.D; ++L) std::memcpy(&max_abs[L], &bits[L], 8);
   return HEOM_OK;
 }
 

@@ -116,6 +116,11 @@ cudaError_t launch_pack_rows(const double2* src, double2* dst, const int32_t* id
 cudaError_t launch_halo_slices(double2* state, double2* packed, const int32_t* node, const int32_t* st, long long pairs,
                                int N, int with_cols, int to_packed, cudaStream_t s);
 
+// out[L] = max over the nodes of level L of max(|re|, |im|) of their elements, as the bit pattern of the double
+// (out must be zeroed; 256 entries); level: DEVICE uint8 per storage slot; per = complex elements per node
+cudaError_t launch_level_max(const double2* state, const uint8_t* level, long long nodes, int per,
+                             unsigned long long* out, cudaStream_t s);
+
 // out[0], out[1] = Tr(A sigma_0) (re, im); A: DEVICE [N][N] complex128
 cudaError_t launch_expectation(const double2* node0, const double2* A, int N, double* out, cudaStream_t s);
 

@@ -257,6 +257,35 @@ cudaError_t launch_halo_slices(double2* state, double2* packed, const int32_t* n
   return cudaGetLastError();
 }
 
+// max |element| over the nodes of every hierarchy level: out[L] (bit pattern of a non-negative double, compared as
+// an integer) for L = 0..D; per is the number of complex elements per node
+__global__ void level_max_kernel(const double2* __restrict__ state, const uint8_t* __restrict__ level, long long nodes,
+                                 int per, unsigned long long* __restrict__ out) {
+  __shared__ unsigned long long smax[256];
+  for (int e = threadIdx.x; e < 256; e += blockDim.x) smax[e] = 0ULL;
+  __syncthreads();
+  const long long total = nodes * per;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
+       t += (long long)gridDim.x * blockDim.x) {
+    const double2 v = state[t];
+    const double a = fmax(fabs(v.x), fabs(v.y));          // max-norm of the element: |re|, |im|
+    const double m = a == a ? a : __longlong_as_double(0x7ff0000000000000LL);   // NaN counts as +inf
+    atomicMax(&smax[level[t / per]], (unsigned long long)__double_as_longlong(m));
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < 256; e += blockDim.x)
+    if (smax[e]) atomicMax(&out[e], smax[e]);
+}
+
+cudaError_t launch_level_max(const double2* state, const uint8_t* level, long long nodes, int per,
+                             unsigned long long* out, cudaStream_t s) {
+  long long blocks = (nodes * per + 255) / 256;
+  if (blocks > 148 * 8) blocks = 148 * 8;
+  if (blocks < 1) blocks = 1;
+  level_max_kernel<<<(int)blocks, 256, 0, s>>>(state, level, nodes, per, out);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_expectation(const double2* node0, const double2* A, int N, double* out, cudaStream_t s) {
   expectation_kernel<<<1, 32, 0, s>>>(node0, A, N, out);
   return cudaGetLastError();

@@ -249,8 +249,11 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   int s = 0, ab = 0;                                  // ring slot and AC buffer of this pass
   unsigned ph = 0, pha = 0;                           // their mbarrier phases
   while (q < npass) {
-    int qnn = 0;                                    // the pass after the next one (consumed at the end of this pass)
-    if (producer) qnn = draw();                     // always: keeps the number of tickets per launch fixed
+    // the pass after the next one: the ticket is drawn now and its value looked at only at the end of this pass,
+    // so that the atomic's round trip (microseconds under contention: 13 % of the stall samples when the value was
+    // consumed at once, profiles/r2_cfg2_hpipe.md) hides behind the pass.  Always drawn: tickets per launch are fixed.
+    unsigned long long traw = 0ULL;
+    if (producer) traw = atomicAdd(P.tickets, 1ULL);
     const int n0 = q * G;
     const int ncnt = min(G, p.nodes - n0);
     unsigned char* slot = ring + s * slot_bytes;
@@ -494,6 +497,11 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     }
     if ((s ^= 1) == 0) ph ^= 1u;
     if ((ab ^= 1) == 0) pha ^= 1u;
+    int qnn = 0;
+    if (producer) {
+      const unsigned long long t = traw - P.ticket_base;
+      qnn = t < (unsigned long long)npass ? (int)t : npass;
+    }
     q = qn;
     qn = __shfl_sync(0xffffffffu, qnn, 0);
   }

@@ -141,10 +141,15 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
     const unsigned long long tk = atomicAdd(P.tickets, 1ULL) - P.ticket_base;
     return tk < (unsigned long long)nodes ? (int)tk : nodes;
   };
+  // Nodes are drawn TWO ahead: the ticket for the node after the next one is requested at the top of an iteration
+  // and its value looked at only at the bottom, so that the atomic's round trip never stalls warp 0 (and, through
+  // the CTA barrier, everyone else).  Every CTA ends with two failing draws.
+  int next = nodes;                                   // the node after the one in flight (warp 0)
   if (warp == 0) {
     int first = 0;
-    if (lane == 0) { first = draw(); *sNode = first; }
+    if (lane == 0) { first = draw(); next = draw(); *sNode = first; }
     first = __shfl_sync(0xffffffffu, first, 0);
+    next = __shfl_sync(0xffffffffu, next, 0);
     load_sigma(first);
   }
 
@@ -154,14 +159,11 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
     ph ^= 1u;
     const int node = *reinterpret_cast<volatile int*>(sNode);
     if (node >= nodes) break;
-    // warp 0 draws the next node now and pulls its sigma into L2 behind this node's arithmetic
-    int next = nodes;
-    if (warp == 0) {
-      if (lane == 0) {
-        next = draw();
-        if (next < nodes) lbulk_prefetch_l2(p.x + (size_t)next * NN, (unsigned)NN * 16);
-      }
-      next = __shfl_sync(0xffffffffu, next, 0);
+    // warp 0 pulls the next node's sigma into L2 behind this node's arithmetic and requests a ticket
+    unsigned long long traw = 0ULL;
+    if (warp == 0 && lane == 0) {
+      if (next < nodes) lbulk_prefetch_l2(p.x + (size_t)next * NN, (unsigned)NN * 16);
+      traw = atomicAdd(P.tickets, 1ULL);
     }
 
     // ---- C = (H/hbar) sigma - sigma (H/hbar) on the FP64 tensor cores (Eq. 12) --------------------
@@ -347,6 +349,10 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
         }
       }
     }
+    if (warp == 0) {                                  // the ticket requested at the top has long arrived
+      const unsigned long long tk = traw - P.ticket_base;
+      next = __shfl_sync(0xffffffffu, tk < (unsigned long long)nodes ? (int)tk : nodes, 0);
+    }
   }
 }
 
@@ -389,7 +395,7 @@ cudaError_t launch_large_t(const RhsParams& p, const int64_t* lptr, const int4* 
   rhs_large_kernel<N, HERM><<<grid, C::THREADS, smem, s>>>(P);
   const cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) {
-    *ticket_base += (unsigned long long)p.nodes + (unsigned long long)grid;   // one failing draw per CTA
+    *ticket_base += (unsigned long long)p.nodes + 2ULL * (unsigned long long)grid;   // two failing draws per CTA
   } else {                                 // nothing ran: keep host base and device counter in step
     cudaMemsetAsync(tickets, 0, sizeof(unsigned long long), s);
     *ticket_base = 0;

@@ -51,6 +51,9 @@ struct MmaCfg {
   static constexpr int CG = CWc / 8;                  // 8-complex-column groups per warp (P2 n-tiles)
   static constexpr int HS = NP + 2;                   // H row stride in doubles  (row bytes == 16 mod 128)
   static constexpr int SS = NP + 1;                   // sigma row stride in double2 (row bytes == 16 mod 128)
+  // small problems leave shared memory free: a second sigma tile lets the next node's TMA load run behind this
+  // node's contraction instead of behind its gathers and epilogue only
+  static constexpr bool DB = NP <= 48;
   static_assert(NP % 16 == 0 && RW % 8 == 0 && CWc % 8 == 0, "unsupported NP");
   static_assert((HS * 8) % 128 == 16 && (SS * 16) % 128 == 16, "row padding");
 };
@@ -58,8 +61,8 @@ struct MmaCfg {
 template <int NP, bool CPLX>
 constexpr size_t mma_smem_bytes() {
   using C = MmaCfg<NP>;
-  return (size_t)NP * C::HS * 8 * (CPLX ? 2 : 1) + (size_t)NP * C::SS * 16 + (size_t)kMmaMaxBaths * 16 +
-         2 * ((size_t)kMmaStaged * 16 + 32) + 8 + 16 + 258 * 8;
+  return (size_t)NP * C::HS * 8 * (CPLX ? 2 : 1) + (size_t)NP * C::SS * 16 * (C::DB ? 2 : 1) + (size_t)kMmaMaxBaths * 16 +
+         2 * ((size_t)kMmaStaged * 16 + 32) + 16 + 16 + 258 * 8;
 }
 template <int NP, bool CPLX>
 constexpr int mma_ctas_per_sm() {
@@ -121,13 +124,14 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
   const int N = p.N, NN = N * N;
   double* sH = reinterpret_cast<double*>(smem_raw);                           // [NP][HS]  Re H / hbar
   double* sHi = sH + (CPLX ? NP * HS : 0);                                    // [NP][HS]  Im H / hbar (CPLX)
-  double2* sS = reinterpret_cast<double2*>(sHi + NP * HS);                    // [NP][SS]  sigma of the node
-  unsigned* sMask = reinterpret_cast<unsigned*>(sS + NP * SS);                // [kMmaMaxBaths][4] membership bits
+  constexpr bool DB = C::DB;
+  double2* sS0 = reinterpret_cast<double2*>(sHi + NP * HS);                   // [DB ? 2 : 1][NP][SS]  sigma tile(s)
+  unsigned* sMask = reinterpret_cast<unsigned*>(sS0 + (DB ? 2 : 1) * NP * SS);   // [kMmaMaxBaths][4] membership bits
   // per node parity: {damping rate d_u, first entry e0, entry count} and the first kMmaStaged link entries
   unsigned char* sLinkBase = reinterpret_cast<unsigned char*>(sMask + 4 * kMmaMaxBaths);
   constexpr int kLinkBuf = kMmaStaged * 16 + 32;
-  unsigned long long* bar = reinterpret_cast<unsigned long long*>(sLinkBase + 2 * kLinkBuf);
-  int* sNode = reinterpret_cast<int*>(bar + 1);
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(sLinkBase + 2 * kLinkBuf);   // [2]
+  int* sNode = reinterpret_cast<int*>(bar + 2);                                                  // [2] (+ padding)
   double* sSqrt = reinterpret_cast<double*>(sNode + 4);                       // [258] sqrt(n), n = 0..D+1 <= 256
   for (int e = threadIdx.x; e < 258; e += C::THREADS) sSqrt[e] = sqrt((double)e);
 
@@ -137,10 +141,11 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
     sH[e] = in ? p.H[i * N + j] * p.inv_hbar : 0.0;
     if (CPLX) sHi[e] = (in && p.Him) ? p.Him[i * N + j] * p.inv_hbar : 0.0;
   }
-  for (int e = threadIdx.x; e < NP * SS; e += C::THREADS) sS[e] = make_double2(0.0, 0.0);   // padding stays zero
+  for (int e = threadIdx.x; e < (DB ? 2 : 1) * NP * SS; e += C::THREADS) sS0[e] = make_double2(0.0, 0.0);   // padding stays zero
   for (int e = threadIdx.x; e < 4 * kMmaMaxBaths; e += C::THREADS) sMask[e] = e < 4 * p.B ? p.bmask[e] : 0u;
   if (threadIdx.x == 0) {
     mmbar_init(bar, 1);
+    mmbar_init(bar + 1, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the zero fill precedes the bulk copies
@@ -152,12 +157,12 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
   const int i0w = (warp / C::WC) * C::RW, j0w = (warp % C::WC) * C::CWc;
   const int nodes = p.nodes;
 
-  auto load_sigma = [&](int node) {
-    if (lane == 0) mmbar_expect_tx(bar, node < nodes ? (unsigned)NN * 16 : 0u);
+  auto load_sigma = [&](int node, int buf) {
+    if (lane == 0) mmbar_expect_tx(bar + buf, node < nodes ? (unsigned)NN * 16 : 0u);
     __syncwarp();
     if (node < nodes)
       for (int row = lane; row < N; row += 32)
-        mbulk_g2s(sS + row * SS, p.x + (size_t)node * NN + (size_t)row * N, (unsigned)N * 16, bar);
+        mbulk_g2s(sS0 + buf * NP * SS + row * SS, p.x + (size_t)node * NN + (size_t)row * N, (unsigned)N * 16, bar + buf);
   };
   auto draw = [&]() -> int {
     const unsigned long long tk = atomicAdd(P.tickets, 1ULL) - P.ticket_base;
@@ -189,11 +194,15 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
     ents[lane] = st.ent[0];
     ents[lane + 32] = st.ent[1];
   };
+  // Nodes are drawn TWO ahead (as in kernels_large.cu): the ticket requested at the top of an iteration is looked at
+  // at its bottom, so the atomic's round trip never stalls warp 0.  Every CTA ends with two failing draws.
+  int next = nodes;                                   // the node after the one in flight (warp 0)
   if (warp == 0) {
     int first = 0;
-    if (lane == 0) { first = draw(); *sNode = first; }
+    if (lane == 0) { first = draw(); next = draw(); sNode[0] = first; }
     first = __shfl_sync(0xffffffffu, first, 0);
-    load_sigma(first);
+    next = __shfl_sync(0xffffffffu, next, 0);
+    load_sigma(first, 0);
     publish(fetch(first), 0);
   }
   __syncthreads();
@@ -211,24 +220,31 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
       }
   }
 
-  unsigned ph = 0;
+  unsigned ph = 0;                                    // bit b: phase of bar[b]
   int lbuf = 0;                                       // link-staging buffer of the node in flight
+  int cur = 0;                                        // sigma tile / mbarrier / sNode slot of the node in flight
   for (;;) {
-    mmbar_wait(bar, ph);                              // sigma of the node has landed (or there is no node)
-    ph ^= 1u;
-    const int node = *reinterpret_cast<volatile int*>(sNode);
+    mmbar_wait(bar + cur, (ph >> cur) & 1u);          // sigma of the node has landed (or there is no node)
+    ph ^= 1u << cur;
+    const int node = *reinterpret_cast<volatile int*>(sNode + cur);
     if (node >= nodes) break;
-    int next = nodes;
+    const double2* sS = sS0 + cur * NP * SS;
     Staged nst;
+    unsigned long long traw = 0ULL;
     if (warp == 0) {
+      if (DB) {
+        // the other tile was last read before the previous node's CTA barrier: the next node's sigma streams into
+        // it behind this node's contraction
+        if (lane == 0) sNode[cur ^ 1] = next;
+        load_sigma(next, cur ^ 1);
+      }
       if (lane == 0) {
-        next = draw();
         if (next < nodes) {
           mbulk_prefetch_l2(p.x + (size_t)next * NN, (unsigned)NN * 16);
           if (p.horner && p.y != p.x) mbulk_prefetch_l2(p.y + (size_t)next * NN, (unsigned)NN * 16);
         }
+        traw = atomicAdd(P.tickets, 1ULL);
       }
-      next = __shfl_sync(0xffffffffu, next, 0);
       nst = fetch(next);                              // in flight behind this node's contraction
     }
 
@@ -339,8 +355,10 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
 
     // ---- next node: start its TMA load behind the rest of this node's work ---------------------------
     if (warp == 0) {
-      if (lane == 0) *sNode = next;
-      load_sigma(next);
+      if (!DB) {
+        if (lane == 0) sNode[0] = next;
+        load_sigma(next, 0);
+      }
       publish(nst, lbuf ^ 1);                         // read after the next node's barrier
     }
 
@@ -397,6 +415,7 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
     }
 
     lbuf ^= 1;
+    if (DB) cur ^= 1;
 
     // ---- fused RK4 stage epilogue straight from the fragment layout ------------------------------------
     const size_t nbase = (size_t)node * NN;
@@ -444,6 +463,10 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
         }
       }
     }
+    if (warp == 0) {                                  // the ticket requested at the top has long arrived
+      const unsigned long long tk = traw - P.ticket_base;
+      next = __shfl_sync(0xffffffffu, tk < (unsigned long long)nodes ? (int)tk : nodes, 0);
+    }
   }
 }
 
@@ -480,7 +503,7 @@ cudaError_t launch_mma_t(const RhsParams& p, const int64_t* lptr, const int4* le
   rhs_mma_kernel<NP, CPLX><<<grid, C::THREADS, smem, s>>>(P);
   const cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) {
-    *ticket_base += (unsigned long long)p.nodes + (unsigned long long)grid;   // one failing draw per CTA
+    *ticket_base += (unsigned long long)p.nodes + 2ULL * (unsigned long long)grid;   // two failing draws per CTA
   } else {
     cudaMemsetAsync(tickets, 0, sizeof(unsigned long long), s);
     *ticket_base = 0;

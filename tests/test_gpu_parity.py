@@ -158,6 +158,19 @@ def test_pade_coefficients_parity(name, D, K, T):
     assert abs(tr - 1.0) < 1e-11
 
 
+def test_level_max_monitor():
+    """heom_level_max (the growth monitor of SURVEY.md 8(c) A7): max(|Re|, |Im|) per hierarchy level against numpy on the
+    state read back, on the matrix, the column and the tensor-core paths."""
+    from paper_1803_03498_b200 import Heom
+    for w, steps in ((workloads.fmo_like().with_(D=3), 30), (workloads.get("cfg5").with_(D=1), 5)):
+        g = Heom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D).bind()
+        g.set_state(w.sigma0()); g.rk4_steps(w.dt_fs, steps)
+        st = g.get_full_state()
+        t = g.tables()[0].sum(axis=1)
+        want = [np.maximum(np.abs(st[t == L].real), np.abs(st[t == L].imag)).max() for L in range(w.D + 1)]
+        assert np.array_equal(g.level_max(), np.array(want))
+
+
 def test_nonhermitian_initial_state_propagation():
     """Linear-absorption-like input: sigma_0(0) = mu rho is not Hermitian."""
     w = _small(4, 1, 4, seed=3)

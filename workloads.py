@@ -151,10 +151,22 @@ def two_exciton_fmo(D=5, K=1, T=77.0):
     return Workload("twoex_fmo29", H, 35.0, 50.0, T, K, D, 0.2, 200, None, s0, tuple(tuple(x) for x in S))
 
 
+def mid_size(N=24, D=5):
+    """Not a BASELINE config: a mid-size site-map system (N between the small-N and the N = 32/64/96 kernels; the
+    paper's "larger state spaces") with cfg4's generator (LHCII-like couplings), K = 0, one bath per
+    site.  Defaults: 24 sites, D = 5: 118 755 nodes of 24 x 24 (1.09 GB per state buffer)."""
+    rng = np.random.default_rng(SEED_LHCII + 7)
+    eps = rng.uniform(0.0, 600.0, size=N)
+    sign = rng.choice([-1.0, 1.0], size=N * (N - 1) // 2)
+    iu = np.triu_indices(N, k=1)
+    J = 80.0 * np.exp(-np.abs(iu[0] - iu[1]) / 3.0) * sign
+    return Workload(f"mid_sites{N}", _symmetric_from_upper(N, eps, J), 37.0, 40.0, 300.0, 0, D, 0.5, 200)
+
+
 CONFIGS = {
     "cfg1": dimer, "cfg2": fmo_like, "cfg3": deep, "cfg4": lhcii_like, "cfg5": large,
 }
-EXTRA = {"absorb": absorption_fmo, "twoex": two_exciton_fmo}
+EXTRA = {"absorb": absorption_fmo, "twoex": two_exciton_fmo, "mid24": mid_size}
 
 
 def get(name):
