@@ -300,7 +300,7 @@ def run_config(key, args, steps, ctx, with_e2e=True, with_cpu=True, options=None
     peaks, which = measured_peaks()
     value = 4.0 * w.nodes * steps * job / (ms * 1e-3)
     horner = kernel_name in ("rhs_hpipe_kernel", "rhs_hpipe_general_kernel", "rhs_large_kernel", "rhs_ket_kernel",
-                             "rhs_mma_kernel", "rhs_large_herm_kernel") \
+                             "rhs_mma_kernel", "rhs_large_herm_kernel", "rhs_mma_herm_kernel") \
         and opts.get("rk4_form", -1) != 0
     # fused classical RK4 moves 16 state sizes per step = 64 N^2 bytes per node-update; the Horner form
     # the kernels run by default (R6) moves 2 + 3 + 3 + 3 = 11 state sizes = 44 N^2 bytes per node-update
@@ -333,7 +333,7 @@ def run_config(key, args, steps, ctx, with_e2e=True, with_cpu=True, options=None
         fp = ctx["fp64"]
         tf = alg_flops_per_launch / avg_launch_s / 1e12
         # Hermitian states: the kernel forms H sigma only and takes k = Z + Z^dagger (4 N^3 executed flops)
-        exe_flops = alg_flops_per_launch * (0.5 if kernel_name == "rhs_large_herm_kernel" else 1.0)
+        exe_flops = alg_flops_per_launch * (0.5 if kernel_name in ("rhs_large_herm_kernel", "rhs_mma_herm_kernel") else 1.0)
         roof = {"bound": "alu", "achieved": tf, "peak": fp["dmma_tflops"], "unit": "TFLOP/s",
                 "frac": tf / fp["dmma_tflops"], "peak_source": "measured: " + fp["how"],
                 "dfma_peak_tflops": fp["dfma_tflops"],

@@ -209,7 +209,7 @@ KernelChoice kernel_choice(const heom_ctx* c) {
   k.large = c->kernel >= 1 && !c->general && large_supported(N, Wd);
   k.hpipe = c->kernel >= 1 && !c->general && hpipe_supported(N, Wd, D, nodes);
   k.tiny = c->kernel == 1 && !c->general && !c->partitioned && tiny_supported(N, Wd, D, nodes);
-  k.mma = c->kernel >= 1 && c->general && mma_supported(N, Wd, c->B, !c->Him.empty());
+  k.mma = c->kernel >= 1 && c->general && mma_supported(N, Wd, c->B, (int)c->sbl.size(), !c->Him.empty());
   k.plain_tables = k.tiny || !(k.large || k.hpipe || k.mma);   // plus/minus/tuples [nodes][W]: generic and tiny kernels
   return k;
 }
@@ -246,7 +246,8 @@ Layout layout_of(const heom_ctx* c) {
   L.off_level = o; o += align_up(nodes + 16) + align_up(256 * 8);
   L.off_send = o; o += align_up(c->part.send_idx.size() * 4 + 16);
   L.off_pairs = o; o += 2 * align_up(c->part.send_pair_node.size() * 4 + 16) + 2 * align_up(c->part.recv_pair_node.size() * 4 + 16);
-  if (kc.large || kc.mma) {
+  if (kc.mma) { L.off_lptr = o; L.off_lent = o; o += align_up(nodes * (size_t)mma_link_row((int)W) * 4); }
+  if (kc.large) {
     // CSR link list: one 16-byte entry per valid "+" and per valid "-" link (a partition's table has links for its
     // owned rows only, so the two counts differ there)
     size_t links = 0;
@@ -294,8 +295,9 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
     CU(launch_rhs_ket(p, ctx->d_linksP, ctx->lrowP, ctx->ket_col, ctx->cd.a_plus.data(), ctx->cd.a_minus_x.data(),
                       ctx->cd.a_minus_o.data(), ctx->H.data(), ctx->cd.delta.data(), ctx->sms, ctx->stream));
   else if (ctx->use_mma)
-    CU(launch_rhs_mma(p, ctx->d_lptr, ctx->d_lent, ctx->cd.a_plus.data(), ctx->cd.a_minus_x.data(),
-                      ctx->cd.a_minus_o.data(), ctx->sms, ctx->d_tickets, &ctx->ticket_base, ctx->stream));
+    CU(launch_rhs_mma(p, (const int32_t*)ctx->d_lent, mma_link_row(p.W), ctx->cd.a_plus.data(), ctx->cd.a_minus_x.data(),
+                      ctx->cd.a_minus_o.data(), ctx->herm_opt && ctx->state_hermitian, ctx->sms, ctx->d_tickets,
+                      &ctx->ticket_base, ctx->stream));
   else if (ctx->use_large)
     CU(launch_rhs_large(p, ctx->d_lptr, ctx->d_lent, ctx->d_Hs, ctx->d_delta, ctx->cd.a_plus.data(),
                         ctx->cd.a_minus_x.data(), ctx->cd.a_minus_o.data(), ctx->herm_opt && ctx->state_hermitian,
@@ -735,7 +737,15 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
     }
     CU(cudaMemset(ctx->d_damp + nodes, 0, 8));
     CU(cudaMemcpy(ctx->d_damp, damp.data(), nodes * 8, cudaMemcpyHostToDevice));
-    if (ctx->use_large || ctx->use_mma) {
+    if (ctx->use_mma) {
+      const size_t mrow = (size_t)mma_link_row((int)W);
+      std::vector<int32_t> rows(nodes * mrow, 0);
+#pragma omp parallel for schedule(static)
+      for (int64_t s = 0; s < (int64_t)nodes; ++s)
+        mma_pack_row((int)W, &tp[(size_t)s * W], &tm[(size_t)s * W], &tt[(size_t)s * W], damp[(size_t)s], &rows[(size_t)s * mrow]);
+      CU(cudaMemcpy(ctx->d_lent, rows.data(), nodes * mrow * 4, cudaMemcpyHostToDevice));
+    }
+    if (ctx->use_large) {
       // CSR link list in storage-slot order: "+" links first, then "-" links, of every node
       std::vector<int64_t> lptr(nodes + 1, 0);
       for (size_t s = 0; s < nodes; ++s) {
@@ -998,7 +1008,7 @@ heom_status heom_partition_plan_slices(const heom_ctx* c, int64_t* send_counts, 
 int heom_halo_slice_elements(const heom_ctx* c) {
   if (!c) return -1;
   /* rows only while the state is exactly Hermitian and the row-gather kernels run, rows + columns otherwise */
-  return (c->herm_opt && c->state_hermitian && (c->use_hpipe || c->use_large)) ? c->h.N : 2 * c->h.N;
+  return (c->herm_opt && c->state_hermitian && (c->use_hpipe || c->use_large)) ? c->h.N : 2 * c->h.N;   // (mma: single GPU)
 }
 
 heom_status heom_pack_halo_slices(heom_ctx* ctx, const void* src_dev, void* dst_dev) {
@@ -1143,7 +1153,7 @@ heom_status heom_kernel_time(heom_ctx* ctx, double* total_ms, int64_t* launches)
 const char* heom_kernel_name(const heom_ctx* c) {
   if (!c) return "none";
   if (c->ket_col >= 0) return "rhs_ket_kernel";
-  if (c->use_mma) return "rhs_mma_kernel";
+  if (c->use_mma) return (c->herm_opt && c->state_hermitian) ? "rhs_mma_herm_kernel" : "rhs_mma_kernel";
   if (c->use_large) return (c->herm_opt && c->state_hermitian) ? "rhs_large_herm_kernel" : "rhs_large_kernel";
   if (c->use_hpipe) return (c->herm_opt && c->state_hermitian) ? "rhs_hpipe_kernel" : "rhs_hpipe_general_kernel";
   return "rhs_generic_kernel";

@@ -78,12 +78,16 @@ cudaError_t launch_rhs_large(const RhsParams& p, const int64_t* lptr, const void
                              unsigned long long* ticket_base, cudaStream_t s);
 
 // Tensor-core kernel for 17 <= N <= 96 and general system-bath operators (kernels_mma.cu): p.gen = 1 with the bath
-// membership bits, p.Him != null selects the complex-H instantiation; CSR link list as for the large kernel with
-// mode indices l = b*M + k; a_*: HOST [W][D+1]; tickets as for hpipe.
-bool mma_supported(int N, int W, int B, bool cplx);
-cudaError_t launch_rhs_mma(const RhsParams& p, const int64_t* lptr, const void* lent, const double* a_plus,
-                           const double* a_minus_x, const double* a_minus_o, int sms, unsigned long long* tickets,
-                           unsigned long long* ticket_base, cudaStream_t s);
+// membership bits and the state -> baths lists, p.Him != null selects the complex-H instantiation.  mrows: DEVICE
+// [nodes][mrow] dense link rows written by mma_pack_row (plus[W], minus[W], n[W] as int32 with mode indices
+// l = b*M + k, then d_u); a_*: HOST [W][D+1]; tickets as for hpipe.  hermitian = 1: the state is exactly Hermitian
+// (one product H sigma, row-only gathers, k = Z + Z^dagger; exact Hermiticity preserved).
+bool mma_supported(int N, int W, int B, int memberships, bool cplx);
+int mma_link_row(int W);   // int32 entries per row (multiple of 4)
+void mma_pack_row(int W, const int32_t* plus, const int32_t* minus, const uint8_t* tuple, double damp, int32_t* row);
+cudaError_t launch_rhs_mma(const RhsParams& p, const int32_t* mrows, int mrow, const double* a_plus,
+                           const double* a_minus_x, const double* a_minus_o, int hermitian, int sms,
+                           unsigned long long* tickets, unsigned long long* ticket_base, cudaStream_t s);
 
 // Whole-propagation kernel for tiny hierarchies (kernels_tiny.cu): nsteps classical RK4 steps of the state p.x
 // (DEVICE, storage-slot order, updated in place) inside ONE launch of one CTA; tables as for the generic kernel.

@@ -19,21 +19,25 @@
 //     with Im H: (i Hi) sigma uses the operand (-Im sigma, Re sigma), sigma (i Hi) the operand swap with
 //     -Hi^T = Hi (antisymmetric).
 //   * k = -i C - (d_u + T) o sigma with the Eq. 14 table T read through the read-only cache; the couplings
-//     to sigma_{u +- e_l} walk the node's CSR link list: a link of bath b touches the elements (i,j) with
-//     i or j in the bath's state set (membership bits in shared memory), factor
-//     i a (q_i - q_j) + a_o (q_i + q_j)  (Eq. 23, 25 summed over the bath's states);
+//     to sigma_{u +- e_l} are gathered ELEMENT-wise: element (i,j) is touched by the links of the baths whose
+//     state set contains i or j (state -> baths lists and membership bits in shared memory), factor
+//     i a (q_i - q_j) + a_o (q_i + q_j)  (Eq. 23, 25 summed over the bath's states).  A thread therefore
+//     looks its rows' and columns' baths up in the node's dense link row {plus[W], minus[W], n[W], d_u}
+//     (staged in shared memory two nodes ahead with cp.async) and issues all its gathers independently of
+//     one another -- walking the node's links one after the other cost one L2 round trip per link;
 //   * fused epilogue straight from the fragment layout: Horner form w' = y + ax k (R6), the
 //     classical form with a running sum, or the bare right-hand side.
 #include "kernels.cuh"
 
 #include <cmath>
+#include <cstring>
 
 namespace heom {
 namespace {
 
 constexpr int kMmaMaxModes = 288;   // W of the constant-bank coupling tables
 constexpr int kMmaMaxBaths = 96;
-constexpr int kMmaStaged = 64;      // link entries of a node staged in shared memory (the rest is read from global)
+constexpr int kMmaMaxMember = 256;  // total (state, bath) memberships in the state -> baths lists
 
 template <int NP>
 struct MmaCfg {
@@ -61,12 +65,13 @@ struct MmaCfg {
 template <int NP, bool CPLX>
 constexpr size_t mma_smem_bytes() {
   using C = MmaCfg<NP>;
+  // without the three staged link rows (3 * mrow * 4 bytes, added at launch)
   return (size_t)NP * C::HS * 8 * (CPLX ? 2 : 1) + (size_t)NP * C::SS * 16 * (C::DB ? 2 : 1) + (size_t)kMmaMaxBaths * 16 +
-         2 * ((size_t)kMmaStaged * 16 + 32) + 16 + 16 + 258 * 8;
+         (size_t)(NP + 4 + kMmaMaxMember) * 4 + 16 + 16 + 258 * 8;
 }
 template <int NP, bool CPLX>
 constexpr int mma_ctas_per_sm() {
-  constexpr size_t per = mma_smem_bytes<NP, CPLX>() + 1024;            // + the runtime's per-CTA reservation
+  constexpr size_t per = mma_smem_bytes<NP, CPLX>() + 1024 + 1024;     // + link rows, the runtime's per-CTA reservation
   constexpr int by_smem = (int)((size_t)227 * 1024 / per);
   constexpr int by_threads = 512 / MmaCfg<NP>::THREADS;              // >= 128 registers per thread
   constexpr int m = by_smem < by_threads ? by_smem : by_threads;
@@ -75,8 +80,8 @@ constexpr int mma_ctas_per_sm() {
 
 struct MmaParams {
   RhsParams p;
-  const int64_t* lptr;     // [nodes+1] CSR offsets into lent
-  const int4* lent;        // link entries: x = neighbour slot, y = mode l, z = 0 ("+") or 1 ("-"), w = n_l
+  const int32_t* mrows;    // [nodes][mrow] dense link rows: plus[W], minus[W], n[W] (int32), d_u (double), padding
+  int mrow;                // ints per row (multiple of 4)
   unsigned long long* tickets;
   unsigned long long ticket_base;
   double cP[kMmaMaxModes], cX[kMmaMaxModes], cO[kMmaMaxModes];   // as in kernels_hpipe.cu
@@ -114,7 +119,7 @@ __device__ __forceinline__ void mdmma(double& c0, double& c1, double a, double b
       : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-template <int NP, bool CPLX>
+template <int NP, bool CPLX, bool HERM>
 __global__ void __launch_bounds__(MmaCfg<NP>::THREADS, mma_ctas_per_sm<NP, CPLX>())
 rhs_mma_kernel(const __grid_constant__ MmaParams P) {
   using C = MmaCfg<NP>;
@@ -127,13 +132,16 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
   constexpr bool DB = C::DB;
   double2* sS0 = reinterpret_cast<double2*>(sHi + NP * HS);                   // [DB ? 2 : 1][NP][SS]  sigma tile(s)
   unsigned* sMask = reinterpret_cast<unsigned*>(sS0 + (DB ? 2 : 1) * NP * SS);   // [kMmaMaxBaths][4] membership bits
-  // per node parity: {damping rate d_u, first entry e0, entry count} and the first kMmaStaged link entries
-  unsigned char* sLinkBase = reinterpret_cast<unsigned char*>(sMask + 4 * kMmaMaxBaths);
-  constexpr int kLinkBuf = kMmaStaged * 16 + 32;
-  unsigned long long* bar = reinterpret_cast<unsigned long long*>(sLinkBase + 2 * kLinkBuf);   // [2]
+  int* sSptr = reinterpret_cast<int*>(sMask + 4 * kMmaMaxBaths);               // [NP + 4] state -> baths CSR offsets
+  int* sSbl = sSptr + NP + 4;                                                  // [kMmaMaxMember] bath indices
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(sSbl + kMmaMaxMember);   // [2]
   int* sNode = reinterpret_cast<int*>(bar + 2);                                                  // [2] (+ padding)
   double* sSqrt = reinterpret_cast<double*>(sNode + 4);                       // [258] sqrt(n), n = 0..D+1 <= 256
+  int32_t* sRows = reinterpret_cast<int32_t*>(sSqrt + 258);                   // [3][mrow] staged link rows
+  const int mrow = P.mrow, W = p.W;
   for (int e = threadIdx.x; e < 258; e += C::THREADS) sSqrt[e] = sqrt((double)e);
+  for (int e = threadIdx.x; e < NP + 4; e += C::THREADS) sSptr[e] = p.sptr[e < N ? e : N];
+  for (int e = threadIdx.x; e < kMmaMaxMember; e += C::THREADS) sSbl[e] = e < p.sptr[N] ? p.sbl[e] : 0;
 
   for (int e = threadIdx.x; e < NP * HS; e += C::THREADS) {
     const int i = e / HS, j = e % HS;
@@ -168,31 +176,17 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
     const unsigned long long tk = atomicAdd(P.tickets, 1ULL) - P.ticket_base;
     return tk < (unsigned long long)nodes ? (int)tk : nodes;
   };
-  // warp 0 stages a node's header and link entries: fetch() early (registers), publish() behind a CTA barrier
-  struct Staged { double dd; long long e0; int cnt; int4 ent[2]; };
-  auto fetch = [&](int node) {
-    Staged st;
-    st.dd = 0.0; st.e0 = 0; st.cnt = 0;
-    st.ent[0] = make_int4(0, 0, 0, 0); st.ent[1] = make_int4(0, 0, 0, 0);
+  // warp 0 stages a node's link row with 16-byte cp.async copies into one of THREE buffers: the next node's row is
+  // requested at the top of an iteration (its buffer was last read two iterations ago, which every warp had left
+  // before the barrier warp 0 has passed since) and waited for before this iteration's barrier
+  auto stage_row = [&](int node, int buf) {
     if (node < nodes) {
-      st.e0 = P.lptr[node];
-      st.cnt = (int)(P.lptr[node + 1] - st.e0);
-      st.dd = p.damp[node];
-      if (lane < st.cnt && lane < kMmaStaged) st.ent[0] = __ldg(P.lent + st.e0 + lane);
-      if (lane + 32 < st.cnt && lane + 32 < kMmaStaged) st.ent[1] = __ldg(P.lent + st.e0 + lane + 32);
+      const int32_t* src = P.mrows + (size_t)node * mrow;
+      const unsigned dst = msmem_u32(sRows + buf * mrow);
+      for (int c = lane; c < mrow / 4; c += 32)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * c), "l"(src + 4 * c) : "memory");
     }
-    return st;
-  };
-  auto publish = [&](const Staged& st, int buf) {
-    unsigned char* base = sLinkBase + buf * kLinkBuf;
-    if (lane == 0) {
-      *reinterpret_cast<double*>(base) = st.dd;
-      *reinterpret_cast<long long*>(base + 8) = st.e0;
-      *reinterpret_cast<int*>(base + 16) = st.cnt;
-    }
-    int4* ents = reinterpret_cast<int4*>(base + 32);
-    ents[lane] = st.ent[0];
-    ents[lane + 32] = st.ent[1];
+    asm volatile("cp.async.commit_group;" ::: "memory");
   };
   // Nodes are drawn TWO ahead (as in kernels_large.cu): the ticket requested at the top of an iteration is looked at
   // at its bottom, so the atomic's round trip never stalls warp 0.  Every CTA ends with two failing draws.
@@ -203,7 +197,8 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
     first = __shfl_sync(0xffffffffu, first, 0);
     next = __shfl_sync(0xffffffffu, next, 0);
     load_sigma(first, 0);
-    publish(fetch(first), 0);
+    stage_row(first, 0);
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
   }
   __syncthreads();
 
@@ -221,7 +216,7 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
   }
 
   unsigned ph = 0;                                    // bit b: phase of bar[b]
-  int lbuf = 0;                                       // link-staging buffer of the node in flight
+  int lbuf = 0;                                       // link-row buffer (of three) of the node in flight
   int cur = 0;                                        // sigma tile / mbarrier / sNode slot of the node in flight
   for (;;) {
     mmbar_wait(bar + cur, (ph >> cur) & 1u);          // sigma of the node has landed (or there is no node)
@@ -229,7 +224,6 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
     const int node = *reinterpret_cast<volatile int*>(sNode + cur);
     if (node >= nodes) break;
     const double2* sS = sS0 + cur * NP * SS;
-    Staged nst;
     unsigned long long traw = 0ULL;
     if (warp == 0) {
       if (DB) {
@@ -245,7 +239,7 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
         }
         traw = atomicAdd(P.tickets, 1ULL);
       }
-      nst = fetch(next);                              // in flight behind this node's contraction
+      stage_row(next, lbuf == 2 ? 0 : lbuf + 1);      // in flight behind this node's contraction
     }
 
     // ---- C = (H/hbar) sigma - sigma (H/hbar) on the FP64 tensor cores (Eq. 12) --------------------
@@ -303,6 +297,7 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
             for (int rg = 0; rg < RG; ++rg) mdmma(acc[rg][ct].x, acc[rg][ct].y, gA[rg].y, b1[ct]);
         }
       }
+      if (!HERM)
 #pragma unroll
       for (int h = 0; h < 2; ++h) {  // P2: natural k, two sub-steps of 4
         const int mm = m0 + 4 * h;
@@ -335,8 +330,8 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
     }
 
     // ---- k = -i C - (d_u + T) o sigma (Eq. 13-14), in the fragment layout ---------------------------
-    const unsigned char* lhead = sLinkBase + lbuf * kLinkBuf;
-    const double dd = *reinterpret_cast<const double*>(lhead);
+    const int32_t* srow = sRows + lbuf * mrow;       // this node's plus[W], minus[W], n[W], d_u
+    const double dd = *reinterpret_cast<const double*>(srow + 3 * W + (W & 1));
 #pragma unroll
     for (int rg = 0; rg < RG; ++rg) {
       const int row = i0w + 8 * rg + rho;
@@ -345,76 +340,120 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
         const int col = j0w + 4 * ct + t;
         const double2 sv = sS[row * SS + col];
         const double tv = T_IN_REGS ? tt[rg * CT + ct] : ((row < N && col < N) ? __ldg(p.Tterm + row * N + col) : 0.0);
-        const double dt = dd + tv;
+        const double dt = HERM ? 0.5 * (dd + tv) : dd + tv;   // HERM: Z = -i P1 - (d_u + T)/2 o sigma
         const double2 c = acc[rg][ct];
         acc[rg][ct] = make_double2(fma(-dt, sv.x, c.y), fma(-dt, sv.y, -c.x));
       }
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncthreads();                                  // every warp is done with the node's sigma
-
-    // ---- next node: start its TMA load behind the rest of this node's work ---------------------------
-    if (warp == 0) {
-      if (!DB) {
+    if (warp == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");   // the next node's link row has landed
+    if (!HERM) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      __syncthreads();                                // every warp is done with the node's sigma
+      // ---- next node: start its TMA load behind the rest of this node's work -------------------------
+      if (!DB && warp == 0) {
         if (lane == 0) sNode[0] = next;
         load_sigma(next, 0);
       }
-      publish(nst, lbuf ^ 1);                         // read after the next node's barrier
     }
 
     // ---- couplings to sigma_{u +- e_l} (Eq. 15-17, 23, 25, 35-36, summed over the bath's states) ------
+    // Element (i,j) takes, from every link of a bath b, the factor i fx (q_i - q_j) + fo (q_i + q_j), q = membership
+    // of b's state set.  Row part: the baths that contain the thread's row i act on all its columns (q_i = 1);
+    // column part: the baths that contain its column j and not the row (q_i = 0, q_j = 1).  HERM: the row part with
+    // (fo + i fx) only -- Z^dagger supplies the rest.  Every gather depends on the staged link row alone.
     {
-      const long long e0 = *reinterpret_cast<const long long*>(lhead + 8);
-      const int cnt = *reinterpret_cast<const int*>(lhead + 16);
-      const int4* staged = reinterpret_cast<const int4*>(lhead + 32);
-      // Small tiles (DENSE_LINKS), branch-free per link: every thread loads all RG*CT of its elements (an inactive one
-      // reads element 0 of the neighbour, warp-wide the same address, and gets a zero factor), so that the loads of a
-      // link -- and, with the loop unrolled by two, of two links -- are in flight together.  Membership bits exist only for real states,
-      // so padded rows and columns are inactive by construction.
-      constexpr bool DENSE_LINKS = RG * CT <= 12;
-      const unsigned rsel = ((C::RW == 32) ? 0xffffffffu : ((1u << C::RW) - 1u));
-      const unsigned long long csel = (1ULL << C::CWc) - 1ULL;
-#pragma unroll 2
-      for (int q = 0; q < cnt; ++q) {
-        const int4 ent = q < kMmaStaged ? staged[q] : __ldg(P.lent + e0 + q);
-        const int l = ent.y, b = l / p.M;
-        const unsigned rbits = (sMask[b * 4 + (i0w >> 5)] >> (i0w & 31)) & rsel;
-        const unsigned long long cbits =
-            ((((unsigned long long)sMask[b * 4 + (j0w >> 5) + 1] << 32) | sMask[b * 4 + (j0w >> 5)]) >> (j0w & 31)) & csel;
-        if (rbits == 0u && cbits == 0ULL) continue;   // warp-uniform: the link does not touch this warp's tile
-        // element factor = i fx (q_i - q_j) + fo (q_i + q_j), q in {0, 1}
-        double fx, fo;
-        if (ent.z == 0) { fx = sSqrt[ent.w + 1] * P.cP[l]; fo = 0.0; }                         // "+"
-        else { const double sn = sSqrt[ent.w]; fx = sn * P.cX[l]; fo = sn * P.cO[l]; }           // "-"
-        const double2* nb = p.x + (size_t)ent.x * NN;
+      const int32_t* spl = srow;
+      const int32_t* smi = srow + W;
+      const int32_t* snn = srow + 2 * W;
+      const int M = p.M;
 #pragma unroll
-        for (int rg = 0; rg < RG; ++rg) {
-          const int row = i0w + 8 * rg + rho;
-          const bool qr = (rbits >> (8 * rg + rho)) & 1u;
-          // (re, im) factor of the element for q_j = 0 and for q_j = 1
-          const double a0r = qr ? fo : 0.0, a0i = qr ? fx : 0.0;
-          const double a1r = qr ? 2.0 * fo : fo, a1i = qr ? 0.0 : -fx;
+      for (int rg = 0; rg < RG; ++rg) {
+        const int row = i0w + 8 * rg + rho;
+        if (row >= N) continue;
+        for (int e = sSptr[row]; e < sSptr[row + 1]; ++e) {
+          const int b = sSbl[e];
+          const unsigned long long cbits =
+              (((unsigned long long)sMask[b * 4 + (j0w >> 5) + 1] << 32) | sMask[b * 4 + (j0w >> 5)]) >> (j0w & 31);
+          for (int k2 = 0; k2 < 2 * M; ++k2) {       // the bath's modes, "+" then "-" link of each
+            const int l = b * M + (k2 >> 1);
+            const int slot = (k2 & 1) ? smi[l] : spl[l];
+            if (slot < 0) continue;
+            const int n = snn[l];
+            double fx, fo;
+            if (k2 & 1) { const double sn = sSqrt[n]; fx = sn * P.cX[l]; fo = sn * P.cO[l]; }   // "-"
+            else { fx = sSqrt[n + 1] * P.cP[l]; fo = 0.0; }                                     // "+"
+            const double2* nbrow = p.x + (size_t)slot * NN + (size_t)row * N;
 #pragma unroll
-          for (int ct = 0; ct < CT; ++ct) {
-            const int col = j0w + 4 * ct + t;
-            const bool qj = (cbits >> (4 * ct + t)) & 1ULL;
-            const double fr = qj ? a1r : a0r, fi = qj ? a1i : a0i;
-            if (DENSE_LINKS) {
-              const int off = (qr | qj) ? row * N + col : 0;
-              const double2 w = __ldg(nb + off);
-              acc[rg][ct].x = fma(fr, w.x, fma(-fi, w.y, acc[rg][ct].x));
-              acc[rg][ct].y = fma(fr, w.y, fma(fi, w.x, acc[rg][ct].y));
-            } else if (qr | qj) {                     // large tiles: few of a thread's elements are touched
-              const double2 w = __ldg(nb + row * N + col);
-              acc[rg][ct].x = fma(fr, w.x, fma(-fi, w.y, acc[rg][ct].x));
-              acc[rg][ct].y = fma(fr, w.y, fma(fi, w.x, acc[rg][ct].y));
+            for (int ct = 0; ct < CT; ++ct) {
+              const int col = j0w + 4 * ct + t;
+              if (col < N) {
+                const bool qj = !HERM && ((cbits >> (4 * ct + t)) & 1ULL);
+                const double fr = qj ? 2.0 * fo : fo, fi = qj ? 0.0 : fx;
+                const double2 w = __ldg(nbrow + col);
+                acc[rg][ct].x = fma(fr, w.x, fma(-fi, w.y, acc[rg][ct].x));
+                acc[rg][ct].y = fma(fr, w.y, fma(fi, w.x, acc[rg][ct].y));
+              }
+            }
+          }
+        }
+      }
+      if (!HERM) {
+#pragma unroll
+        for (int ct = 0; ct < CT; ++ct) {
+          const int col = j0w + 4 * ct + t;
+          if (col >= N) continue;
+          for (int e = sSptr[col]; e < sSptr[col + 1]; ++e) {
+            const int b = sSbl[e];
+            const unsigned rbits = sMask[b * 4 + (i0w >> 5)] >> (i0w & 31);
+            for (int k2 = 0; k2 < 2 * M; ++k2) {
+              const int l = b * M + (k2 >> 1);
+              const int slot = (k2 & 1) ? smi[l] : spl[l];
+              if (slot < 0) continue;
+              const int n = snn[l];
+              double fx, fo;
+              if (k2 & 1) { const double sn = sSqrt[n]; fx = sn * P.cX[l]; fo = sn * P.cO[l]; }
+              else { fx = sSqrt[n + 1] * P.cP[l]; fo = 0.0; }
+              const double2* nbcol = p.x + (size_t)slot * NN + col;
+#pragma unroll
+              for (int rg = 0; rg < RG; ++rg) {
+                const int row = i0w + 8 * rg + rho;
+                if (row < N && !((rbits >> (8 * rg + rho)) & 1u)) {   // rows inside the set were done above
+                  const double2 w = __ldg(nbcol + (size_t)row * N);
+                  acc[rg][ct].x = fma(fo, w.x, fma(fx, w.y, acc[rg][ct].x));      // (fo - i fx) w
+                  acc[rg][ct].y = fma(fo, w.y, fma(-fx, w.x, acc[rg][ct].y));
+                }
+              }
             }
           }
         }
       }
     }
 
-    lbuf ^= 1;
+    if (HERM) {
+      // ---- k = Z + Z^dagger through the sigma tile (every warp is done with it after the first barrier) ----
+      double2* sZ = sS0 + cur * NP * SS;
+      __syncthreads();
+#pragma unroll
+      for (int rg = 0; rg < RG; ++rg)
+#pragma unroll
+        for (int ct = 0; ct < CT; ++ct) sZ[(i0w + 8 * rg + rho) * SS + j0w + 4 * ct + t] = acc[rg][ct];
+      __syncthreads();
+#pragma unroll
+      for (int rg = 0; rg < RG; ++rg)
+#pragma unroll
+        for (int ct = 0; ct < CT; ++ct) {
+          const double2 zt = sZ[(j0w + 4 * ct + t) * SS + i0w + 8 * rg + rho];     // Z[col][row]
+          acc[rg][ct].x += zt.x;
+          acc[rg][ct].y -= zt.y;
+        }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      __syncthreads();                                // the tile may be overwritten by a TMA load
+      if (!DB && warp == 0) {
+        if (lane == 0) sNode[0] = next;
+        load_sigma(next, 0);
+      }
+    }
+    lbuf = lbuf == 2 ? 0 : lbuf + 1;
     if (DB) cur ^= 1;
 
     // ---- fused RK4 stage epilogue straight from the fragment layout ------------------------------------
@@ -470,14 +509,14 @@ rhs_mma_kernel(const __grid_constant__ MmaParams P) {
   }
 }
 
-template <int NP, bool CPLX>
-cudaError_t launch_mma_t(const RhsParams& p, const int64_t* lptr, const int4* lent, const double* a_plus,
+template <int NP, bool CPLX, bool HERM>
+cudaError_t launch_mma_t(const RhsParams& p, const int32_t* mrows, int mrow, const double* a_plus,
                          const double* a_minus_x, const double* a_minus_o, int sms, unsigned long long* tickets,
                          unsigned long long* ticket_base, cudaStream_t s) {
   using C = MmaCfg<NP>;
   if (p.W > kMmaMaxModes || p.B > kMmaMaxBaths) return cudaErrorInvalidValue;
   MmaParams P;
-  P.p = p; P.lptr = lptr; P.lent = lent;
+  P.p = p; P.mrows = mrows; P.mrow = mrow;
   const int D1 = p.D + 1;
   for (int l = 0; l < kMmaMaxModes; ++l) {
     const bool on = l < p.W && p.D >= 1;
@@ -485,22 +524,22 @@ cudaError_t launch_mma_t(const RhsParams& p, const int64_t* lptr, const int4* le
     P.cX[l] = on ? a_minus_x[(size_t)l * D1 + 1] : 0.0;
     P.cO[l] = on ? a_minus_o[(size_t)l * D1 + 1] : 0.0;
   }
-  constexpr size_t smem = mma_smem_bytes<NP, CPLX>();
-  static bool configured_on[64] = {};
+  const size_t smem = mma_smem_bytes<NP, CPLX>() + 3 * (size_t)mrow * 4;
+  static size_t configured_on[64] = {};
   int dev_ = 0;
   cudaGetDevice(&dev_);
-  bool& configured = configured_on[dev_ & 63];
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(rhs_mma_kernel<NP, CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  size_t& configured = configured_on[dev_ & 63];
+  if (smem > configured) {
+    cudaError_t e = cudaFuncSetAttribute(rhs_mma_kernel<NP, CPLX, HERM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = true;
+    configured = smem;
   }
   int grid = sms * mma_ctas_per_sm<NP, CPLX>();
   if (grid > p.nodes) grid = p.nodes;
   if (grid < 1) grid = 1;
   P.tickets = tickets;
   P.ticket_base = *ticket_base;
-  rhs_mma_kernel<NP, CPLX><<<grid, C::THREADS, smem, s>>>(P);
+  rhs_mma_kernel<NP, CPLX, HERM><<<grid, C::THREADS, smem, s>>>(P);
   const cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) {
     *ticket_base += (unsigned long long)p.nodes + 2ULL * (unsigned long long)grid;   // two failing draws per CTA
@@ -515,28 +554,42 @@ int mma_padded(int N) { return N <= 32 ? 32 : (N + 15) / 16 * 16; }
 
 }  // namespace
 
-bool mma_supported(int N, int W, int B, bool cplx) {
-  if (N < 17 || N > 96 || W > kMmaMaxModes || B > kMmaMaxBaths) return false;
+int mma_link_row(int W) { return (3 * W + (W & 1) + 2 + 3) / 4 * 4; }   // ints: plus, minus, n, (pad), d_u; 16-byte multiple
+
+void mma_pack_row(int W, const int32_t* plus, const int32_t* minus, const uint8_t* tuple, double damp, int32_t* row) {
+  for (int l = 0; l < W; ++l) { row[l] = plus[l]; row[W + l] = minus[l]; row[2 * W + l] = tuple[l]; }
+  const int off = 3 * W + (W & 1);                    // 8-byte aligned
+  double d = damp;
+  std::memcpy(row + off, &d, 8);
+  for (int e = off + 2; e < mma_link_row(W); ++e) row[e] = 0;
+  if (W & 1) row[3 * W] = 0;
+}
+
+bool mma_supported(int N, int W, int B, int memberships, bool cplx) {
+  if (N < 17 || N > 96 || W > kMmaMaxModes || B > kMmaMaxBaths || memberships > kMmaMaxMember) return false;
+  if (mma_padded(N) == 96 && mma_smem_bytes<96, false>() + 3 * (size_t)mma_link_row(W) * 4 > (size_t)227 * 1024)
+    return false;                                     // H, sigma and the staged link rows must fit one SM
   return !(cplx && mma_padded(N) == 96);              // Re H, Im H and sigma do not fit one SM's shared memory
 }
 
-cudaError_t launch_rhs_mma(const RhsParams& p, const int64_t* lptr, const void* lent, const double* a_plus,
-                           const double* a_minus_x, const double* a_minus_o, int sms, unsigned long long* tickets,
-                           unsigned long long* ticket_base, cudaStream_t s) {
-  const int4* le = reinterpret_cast<const int4*>(lent);
+cudaError_t launch_rhs_mma(const RhsParams& p, const int32_t* mrows, int mrow, const double* a_plus,
+                           const double* a_minus_x, const double* a_minus_o, int hermitian, int sms,
+                           unsigned long long* tickets, unsigned long long* ticket_base, cudaStream_t s) {
   const bool cplx = p.Him != nullptr;
-#define HEOM_MMA_CASE(np)                                                                                          \
-  case np:                                                                                                         \
-    return cplx ? launch_mma_t<np, true>(p, lptr, le, a_plus, a_minus_x, a_minus_o, sms, tickets, ticket_base, s)  \
-                : launch_mma_t<np, false>(p, lptr, le, a_plus, a_minus_x, a_minus_o, sms, tickets, ticket_base, s);
+#define HEOM_MMA_ARGS p, mrows, mrow, a_plus, a_minus_x, a_minus_o, sms, tickets, ticket_base, s
+#define HEOM_MMA_CASE(np)                                                                              \
+  case np:                                                                                             \
+    if (cplx) return hermitian ? launch_mma_t<np, true, true>(HEOM_MMA_ARGS) : launch_mma_t<np, true, false>(HEOM_MMA_ARGS);   \
+    return hermitian ? launch_mma_t<np, false, true>(HEOM_MMA_ARGS) : launch_mma_t<np, false, false>(HEOM_MMA_ARGS);
   switch (mma_padded(p.N)) {
     HEOM_MMA_CASE(32) HEOM_MMA_CASE(48) HEOM_MMA_CASE(64) HEOM_MMA_CASE(80)
     case 96:
       if (cplx) return cudaErrorInvalidValue;
-      return launch_mma_t<96, false>(p, lptr, le, a_plus, a_minus_x, a_minus_o, sms, tickets, ticket_base, s);
+      return hermitian ? launch_mma_t<96, false, true>(HEOM_MMA_ARGS) : launch_mma_t<96, false, false>(HEOM_MMA_ARGS);
     default: return cudaErrorInvalidValue;
   }
 #undef HEOM_MMA_CASE
+#undef HEOM_MMA_ARGS
 }
 
 }  // namespace heom
