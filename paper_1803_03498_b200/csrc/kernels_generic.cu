@@ -269,7 +269,8 @@ __global__ void level_max_kernel(const double2* __restrict__ state, const uint8_
        t += (long long)gridDim.x * blockDim.x) {
     const double2 v = state[t];
     const double a = fmax(fabs(v.x), fabs(v.y));          // max-norm of the element: |re|, |im|
-    const double m = a == a ? a : __longlong_as_double(0x7ff0000000000000LL);   // NaN counts as +inf
+    // NaN counts as +inf (fmax drops a NaN operand: test the parts themselves)
+    const double m = (v.x == v.x && v.y == v.y) ? a : __longlong_as_double(0x7ff0000000000000LL);
     atomicMax(&smax[level[t / per]], (unsigned long long)__double_as_longlong(m));
   }
   __syncthreads();
