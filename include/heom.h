@@ -246,6 +246,27 @@ const char* heom_kernel_name(const heom_ctx* ctx);
  * (mma.sync.m8n8k4.f64, SASS DMMA.8x8x4) -- *value in TFLOP/s; 2 = HBM copy bandwidth (read + write bytes of a
  * 1 GiB device-to-device copy kernel) -- *value in GB/s.  Best of 5 timed repetitions after one warm-up. */
 heom_status heom_probe_peak(int device, int kind, double* value);
+/* The growth monitor of heom_level_max for callers that may not allocate device memory (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): no context, no workspace, nothing allocated or
+ * freed.  Its scratch (the per-level running maxima and a finished-blocks counter, 768 bytes) is a file-scope
+ * __device__ array that every GPU loading the library holds until the process exits, hence the limit
+ * depth <= HEOM_STATIC_MAX_DEPTH; a larger depth is rejected with HEOM_EINVAL (use heom_level_max).
+ *   device          CUDA ordinal the pointers belong to (made current for the call, then restored)
+ *   state_dev       DEVICE complex128 [nodes][elems_per_node], any node order (e.g. heom_stage_output's buffer)
+ *   level_dev       DEVICE uint8 [nodes]: hierarchy level sum(n) of every node, same order; levels > depth are ignored
+ *   max_abs_dev     DEVICE double [depth+1]: max over the nodes of level L and their elements of max(|Re|, |Im|);
+ *                   +inf if a NaN or Inf is present; 0 for a level without nodes
+ *   cuda_stream     cudaStream_t; the call enqueues a clear of the scratch and one kernel on it and returns
+ *                   (no synchronisation: max_abs_dev is valid once the stream reaches that point)
+ * All calls on a device share the scratch: each clears it first, so nothing of an earlier call survives, but calls
+ * that overlap on the GPU (different streams without an ordering between them) race and give wrong maxima.
+ * The first call on a device looks the scratch address up (cudaGetSymbolAddress); make it outside a graph capture. */
+#define HEOM_STATIC_MAX_DEPTH 63
+heom_status heom_level_max_static(int device, const void* state_dev, const uint8_t* level_dev, int64_t nodes,
+                                  int elems_per_node, int depth, double* max_abs_dev, void* cuda_stream);
+/* Text of the last error heom_level_max_static returned on the calling thread (static storage, "" if none). */
+const char* heom_static_last_error(void);
+
 /* Human-readable text of the last error on this context (ctx-owned). */
 const char* heom_last_error(const heom_ctx* ctx);
 

@@ -25,6 +25,7 @@ SYMBOLS = [
     "heom_sync", "heom_populations", "heom_launch_count", "heom_kernel_time", "heom_kernel_name",
     "heom_last_error", "heom_probe_peak", "heom_create_general", "heom_set_hamiltonian",
     "heom_level_max", "heom_partition_plan_slices", "heom_halo_slice_elements", "heom_pack_halo_slices", "heom_unpack_halo_slices",
+    "heom_level_max_static", "heom_static_last_error",
 ]
 
 _lib = None
@@ -95,6 +96,9 @@ def load_library():
     lib.heom_last_error.argtypes = [P]
     lib.heom_last_error.restype = C.c_char_p
     lib.heom_probe_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double)]
+    lib.heom_level_max_static.argtypes = [C.c_int, P, P, C.c_int64, C.c_int, C.c_int, P, P]
+    lib.heom_static_last_error.argtypes = []
+    lib.heom_static_last_error.restype = C.c_char_p
     _lib = lib
     return lib
 
@@ -112,6 +116,19 @@ def probe_peak(kind, device=0):
     if rc != 0:
         raise HeomError(rc, "heom_probe_peak failed (no CUDA device?)")
     return v.value
+
+
+STATIC_MAX_DEPTH = 63   # HEOM_STATIC_MAX_DEPTH
+
+
+def level_max_static(state_ptr, level_ptr, nodes, elems_per_node, depth, out_ptr, device=0, cuda_stream=0):
+    """heom_level_max_static: the per-level growth monitor without any allocation (scratch in a static device
+    array, depth <= STATIC_MAX_DEPTH).  All pointers are DEVICE addresses; stream-ordered, does not synchronise."""
+    lib = load_library()
+    rc = lib.heom_level_max_static(int(device), int(state_ptr), int(level_ptr), int(nodes), int(elems_per_node),
+                                   int(depth), int(out_ptr), int(cuda_stream))
+    if rc != 0:
+        raise HeomError(rc, lib.heom_static_last_error().decode())
 
 
 class Heom:
