@@ -45,14 +45,15 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0}, "fallback"
 
 
-def ncu_traffic(name):
+def ncu_traffic(name, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch (average over the four stage launches of one RK4
-    step) from the committed `ncu --set full` captures, listed with their sources in profiles/traffic.json."""
+    step) from the committed `ncu --set full` captures, listed with their sources in profiles/traffic.json;
+    None if the capture is of another kernel than the one this run used."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     try:
         with open(p) as f:
             ent = json.load(f).get(name)
-        return (ent["bytes_per_launch"], ent["source"]) if ent else (None, None)
+        return (ent["bytes_per_launch"], ent["source"]) if ent and ent.get("kernel") == kernel else (None, None)
     except (OSError, ValueError, KeyError):
         return None, None
 
@@ -321,7 +322,7 @@ def run_config(key, args, steps, ctx, with_e2e=True, with_cpu=True, options=None
     if tiny:
         kernel_name = "rk4_tiny_kernel (all steps in one launch; time per RK4 stage)"
     achieved = alg_bytes_per_launch / avg_launch_s / 1e9
-    traffic, traffic_src = ncu_traffic(w.name)
+    traffic, traffic_src = ncu_traffic(w.name, kernel_name if opts.get("rk4_form", -1) != 0 else None)
     common = {"kernel": kernel_name, "avg_launch_ms": avg_launch_s * 1e3,
               "kernel_only_launch_ms": kernel_only_s * 1e3 if kernel_only_s else None,
               "launches_timed": stage_launches * len(chunk_ms), "traffic": traffic, "traffic_source": traffic_src,
