@@ -56,7 +56,10 @@ struct PipeCfg {
   static constexpr int LP = (N <= 2) ? 2 : (N <= 4) ? 4 : (N <= 8) ? 8 : 16;   // lanes per node
   static constexpr int G = 32 / LP;                   // nodes per warp pass
   static constexpr int S = 2;                         // ring slots per warp
-  static constexpr int MAXW = (N <= 8) ? 12 : 6;      // warps per CTA (fewer if shared memory is short)
+  // warps per CTA (fewer if shared memory is short).  N > 8: 8 warps of 254 registers -- measured on config 4
+  // (N = 14): 6 warps 2.556, 7 warps 2.425, 8 warps 2.338 ms per step; 10 warps (168 registers, spills) 3.07.
+  // N <= 8: 12 warps of 168 registers; 16 warps of 128 registers with one mode index per gather batch: the same time.
+  static constexpr int MAXW = (N <= 8) ? 12 : 8;
   static constexpr int MAXW_GENERAL = (N <= 8) ? 8 : 6;   // general states need more registers per thread
   static constexpr int SMEM_BUDGET = 224 * 1024;
   static constexpr int KB = (16 / N) > 0 ? (16 / N) : 1;   // mode indices kk per gather batch (<= 32 loads)
@@ -149,6 +152,15 @@ __device__ __forceinline__ void ldg_link(double2& r, const double2* base, int of
       "}\n" : "+d"(r.x), "+d"(r.y) : "l"(base), "r"(off), "l"(pol));
 }
 
+// One ticket.  Inline PTX on purpose: for a plain atomicAdd under `if (lane == 0)` the compiler emits its
+// warp-aggregation sequence (vote, leader atomic, SHFL of the result), and that SHFL waits for the atomic's round
+// trip on the spot (7.5 % of the stall samples on config 2) although the value is only needed a pass later.
+__device__ __forceinline__ unsigned long long ticket_add(unsigned long long* ctr) {
+  unsigned long long old;
+  asm volatile("atom.global.add.u64 %0, [%1], 1;" : "=l"(old) : "l"(ctr) : "memory");
+  return old;
+}
+
 template <int N, bool HERM>
 __global__ void __launch_bounds__((HERM ? PipeCfg<N>::MAXW : PipeCfg<N>::MAXW_GENERAL) * 32, 1)
 rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
@@ -160,8 +172,10 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   const int M = p.M, lrow = P.lrow, CW = P.nwarps;
   // shared memory per warp: S slots of {XA [G][PS] double2, ML [G][lrow] int32} and 2 AC buffers; then a
   // null meta row, the sqrt table [n][up] = (sqrt(n), up ? sqrt(n+1) : 0) and the mbarriers
+  // (Horner stages keep no running sum: one AC buffer, the transposition scratch, is enough -- more warps fit)
   const int slot_bytes = XB + G * lrow * 4;
-  const int warp_bytes = S * slot_bytes + 2 * AB;
+  const int nab = (p.horner != 0 && p.rhs_only == 0) ? 1 : 2;
+  const int warp_bytes = S * slot_bytes + nab * AB;
   int32_t* sNull = reinterpret_cast<int32_t*>(smem_raw + CW * warp_bytes);    // [lrow]
   double2* sSQ = reinterpret_cast<double2*>(sNull + lrow);                    // [kMaxSqrt][2]
   double* sCoef = reinterpret_cast<double*>(sSQ + 2 * kMaxSqrt);              // [3][kMaxModes]: cP, cX, cO (lane-indexed)
@@ -219,7 +233,7 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
   // Groups of this warp: one ticket per pass, drawn by lane 0 TWO passes ahead (the atomic's round trip under
   // contention is microseconds; values >= npass: no more work).  Every warp ends with exactly two such tickets.
   auto draw = [&]() -> int {
-    const unsigned long long t = atomicAdd(P.tickets, 1ULL) - P.ticket_base;
+    const unsigned long long t = ticket_add(P.tickets) - P.ticket_base;
     return t < (unsigned long long)npass ? (int)t : npass;
   };
   int q = 0, qn = 0;                                  // this pass, the pass after it
@@ -253,13 +267,13 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
     // so that the atomic's round trip (microseconds under contention: 13 % of the stall samples when the value was
     // consumed at once, profiles/r2_cfg2_hpipe.md) hides behind the pass.  Always drawn: tickets per launch are fixed.
     unsigned long long traw = 0ULL;
-    if (producer) traw = atomicAdd(P.tickets, 1ULL);
+    if (producer) traw = ticket_add(P.tickets);
     const int n0 = q * G;
     const int ncnt = min(G, p.nodes - n0);
     unsigned char* slot = ring + s * slot_bytes;
     double2* sXA = reinterpret_cast<double2*>(slot);
-    double2* sAC = reinterpret_cast<double2*>(acbuf + ab * AB);
-    double2* scr = reinterpret_cast<double2*>(acbuf + (ab ^ 1) * AB);
+    double2* sAC = reinterpret_cast<double2*>(acbuf + (nab == 2 ? ab * AB : 0));   // unused when nab == 1
+    double2* scr = reinterpret_cast<double2*>(acbuf + (nab == 2 ? (ab ^ 1) * AB : 0));
     const int32_t* sL = reinterpret_cast<const int32_t*>(slot + XB);
     mbar_wait(barX + s, ph);
 
@@ -509,17 +523,17 @@ rhs_hpipe_kernel(const __grid_constant__ PipeParams<N> P) {
 }
 
 template <int N>
-size_t hpipe_smem(int lrow, int warps) {
+size_t hpipe_smem(int lrow, int warps, int nab = 2) {
   using C = PipeCfg<N>;
-  return (size_t)warps * (C::S * ((size_t)C::XB + (size_t)C::G * lrow * 4) + 2 * (size_t)C::AB) +
+  return (size_t)warps * (C::S * ((size_t)C::XB + (size_t)C::G * lrow * 4) + nab * (size_t)C::AB) +
          (size_t)lrow * 4 + 2 * kMaxSqrt * 16 + 3 * kMaxModes * 8 + (size_t)warps * (2 * C::S + 2) * 8;
 }
 // warps per CTA: as many as fit into the shared-memory budget (0 if not even one fits)
 template <int N>
-int hpipe_warps(int lrow, bool herm = true) {
+int hpipe_warps(int lrow, bool herm = true, int nab = 2) {
   using C = PipeCfg<N>;
   int w = herm ? C::MAXW : C::MAXW_GENERAL;
-  while (w >= 1 && hpipe_smem<N>(lrow, w) > (size_t)C::SMEM_BUDGET) --w;
+  while (w >= 1 && hpipe_smem<N>(lrow, w, nab) > (size_t)C::SMEM_BUDGET) --w;
   return w;
 }
 
@@ -532,7 +546,8 @@ cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, c
   PipeParams<N> P;
   P.p = p; P.links = links; P.lrow = lrow;
   P.npass = (p.nodes + C::G - 1) / C::G;
-  const int wmax = hpipe_warps<N>(lrow, HERM);
+  const int nab = (p.horner != 0 && p.rhs_only == 0) ? 1 : 2;
+  const int wmax = hpipe_warps<N>(lrow, HERM, nab);
   if (wmax < 1) return cudaErrorInvalidValue;
   P.nwarps = (warps > 0 && warps < wmax) ? warps : wmax;
   for (int e = 0; e < N * N; ++e) P.H[e] = H_host[e] * p.inv_hbar;
@@ -544,7 +559,7 @@ cudaError_t launch_hpipe_t(const RhsParams& p, const int32_t* links, int lrow, c
     P.cX[l] = on ? a_minus_x[(size_t)l * D1 + 1] : 0.0;     // sgn sqrt(1 * s_l)
     P.cO[l] = on ? a_minus_o[(size_t)l * D1 + 1] : 0.0;     // sqrt(1 / s_l) lambda nu / hbar
   }
-  const size_t smem = hpipe_smem<N>(lrow, P.nwarps);
+  const size_t smem = hpipe_smem<N>(lrow, P.nwarps, nab);
   static size_t configured_on[64] = {};   // per device: the attribute belongs to the device's context
   int dev_ = 0;
   cudaGetDevice(&dev_);
