@@ -70,6 +70,7 @@ struct heom_ctx {
   bool use_large = false;
   int64_t* d_lptr = nullptr;
   void* d_lent = nullptr;
+  int32_t* d_mrows = nullptr;        // large kernel: dense link rows (mma_pack_row format)
   double *d_Hs = nullptr, *d_delta = nullptr;
   double* d_Him = nullptr;          // general contexts: imaginary part of H (cm^-1)
   int32_t *d_sptr = nullptr, *d_sbl = nullptr;
@@ -196,7 +197,7 @@ int node_stride(int N) { return N * N; }
 
 struct Layout {
   size_t state, off_y, off_acc, off_xa, off_xb, off_plus, off_minus, off_slot, off_tuples, off_damp,
-      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_linksP, off_Hs, off_delta, off_Him, off_gen, off_A, off_S0, off_level, off_send, off_pairs, off_lptr, off_lent, total;
+      off_H, off_T, off_ap, off_amx, off_amo, off_scratch, off_linksP, off_Hs, off_delta, off_Him, off_gen, off_A, off_S0, off_level, off_send, off_pairs, off_lptr, off_lent, off_mrows, total;
 };
 
 // Which kernel family the bound configuration will run (fixed by the shape and the "kernel" option), so that the
@@ -254,6 +255,8 @@ Layout layout_of(const heom_ctx* c) {
     for (size_t q = 0; q < c->h.minus.size(); ++q) links += (c->h.minus[q] >= 0) + (c->h.plus[q] >= 0);
     L.off_lptr = o; o += align_up((nodes + 1) * 8);
     L.off_lent = o; o += align_up(links * 16 + 16);
+    // dense link rows for the Hermitian variant's row-wise gathers
+    L.off_mrows = o; o += align_up(nodes * (size_t)mma_link_row((int)W) * 4);
   }
   L.total = o;
   return L;
@@ -299,7 +302,7 @@ heom_status launch_rhs(heom_ctx* ctx, const RhsParams& p) {
                       ctx->cd.a_minus_o.data(), ctx->herm_opt && ctx->state_hermitian, ctx->sms, ctx->d_tickets,
                       &ctx->ticket_base, ctx->stream));
   else if (ctx->use_large)
-    CU(launch_rhs_large(p, ctx->d_lptr, ctx->d_lent, ctx->d_Hs, ctx->d_delta, ctx->cd.a_plus.data(),
+    CU(launch_rhs_large(p, ctx->d_lptr, ctx->d_lent, ctx->d_mrows, mma_link_row(p.W), ctx->d_Hs, ctx->d_delta, ctx->cd.a_plus.data(),
                         ctx->cd.a_minus_x.data(), ctx->cd.a_minus_o.data(), ctx->herm_opt && ctx->state_hermitian,
                         ctx->sms, ctx->d_tickets, &ctx->ticket_base, ctx->stream));
   else if (ctx->use_hpipe)
@@ -696,6 +699,7 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
   ctx->ket_col = -1;
   ctx->d_lptr = (int64_t*)(base + L.off_lptr);
   ctx->d_lent = (void*)(base + L.off_lent);
+  ctx->d_mrows = (int32_t*)(base + L.off_mrows);
   ctx->d_linksP = (int32_t*)(base + L.off_linksP);
   ctx->lrowP = hpipe_links_row(ctx->h.N, ctx->h.M);
   ctx->use_hpipe = kc.hpipe && !kc.large;
@@ -763,6 +767,14 @@ heom_status heom_bind_workspace(heom_ctx* ctx, void* dev_ptr, size_t bytes, void
           if (tm[(size_t)s * W + l] >= 0) { e[0] = tm[(size_t)s * W + l]; e[1] = (int32_t)l; e[2] = 1; e[3] = tt[(size_t)s * W + l]; e += 4; }
       }
       ctx->n_links = (size_t)lptr[nodes];
+      {
+        const size_t mrow = (size_t)mma_link_row((int)W);
+        std::vector<int32_t> rows(nodes * mrow, 0);
+#pragma omp parallel for schedule(static)
+        for (int64_t s = 0; s < (int64_t)nodes; ++s)
+          mma_pack_row((int)W, &tp[(size_t)s * W], &tm[(size_t)s * W], &tt[(size_t)s * W], damp[(size_t)s], &rows[(size_t)s * mrow]);
+        CU(cudaMemcpy(ctx->d_mrows, rows.data(), nodes * mrow * 4, cudaMemcpyHostToDevice));
+      }
       CU(cudaMemcpy(ctx->d_lptr, lptr.data(), (nodes + 1) * 8, cudaMemcpyHostToDevice));
       CU(cudaMemcpy(ctx->d_lent, lent.data(), (size_t)lptr[nodes] * 16 + 16, cudaMemcpyHostToDevice));
       std::vector<double> Hs(ctx->H);

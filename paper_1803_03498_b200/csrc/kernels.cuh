@@ -72,8 +72,9 @@ cudaError_t launch_rhs_hpipe(const RhsParams& p, const int32_t* links, int lrow,
 // offsets; lent: DEVICE int4 link entries {neighbour slot, mode l, 0 "+" | 1 "-", n_l}; Hs_dev: DEVICE
 // [N][N] = H/hbar; delta_dev: DEVICE [N]; a_*: HOST coupling tables [W][D+1]; tickets as for hpipe.
 bool large_supported(int N, int W);
-cudaError_t launch_rhs_large(const RhsParams& p, const int64_t* lptr, const void* lent, const double* Hs_dev,
-                             const double* delta_dev, const double* a_plus, const double* a_minus_x,
+// mrows: dense link rows [nodes][mrow] in the format of mma_link_row / mma_pack_row (read by the Hermitian variant)
+cudaError_t launch_rhs_large(const RhsParams& p, const int64_t* lptr, const void* lent, const int32_t* mrows, int mrow,
+                             const double* Hs_dev, const double* delta_dev, const double* a_plus, const double* a_minus_x,
                              const double* a_minus_o, int hermitian, int sms, unsigned long long* tickets,
                              unsigned long long* ticket_base, cudaStream_t s);
 

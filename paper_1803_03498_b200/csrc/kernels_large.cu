@@ -56,6 +56,8 @@ struct LargeParams {
   RhsParams p;
   const int64_t* lptr;     // [nodes+1] CSR offsets into lent
   const int4* lent;        // link entries: x = neighbour slot, y = mode l, z = 0 ("+") or 1 ("-"), w = n_l
+  const int32_t* mrows;    // [nodes][mrow] dense link rows {plus[W], minus[W], n[W], d_u}, as in kernels_mma.cu
+  int mrow;                // ints per dense row
   const double* Hs;        // DEVICE [N][N]: H / hbar
   const double* delta;     // DEVICE [N]
   unsigned long long* tickets;
@@ -98,6 +100,14 @@ __device__ __forceinline__ void dmma(double& c0, double& c1, double a, double b)
                : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 __device__ __forceinline__ double neg(double v) { return -v; }
+// 16-byte read-only load of *ptr, executed only if ok; otherwise the destination keeps its contents
+__device__ __forceinline__ void ldg_if(double2& r, const double2* ptr, bool ok) {
+  asm volatile("{\n"
+      ".reg .pred p;\n"
+      "setp.ne.s32 p, %3, 0;\n"
+      "@p ld.global.nc.v2.f64 {%0, %1}, [%2];\n"
+      "}\n" : "+d"(r.x), "+d"(r.y) : "l"(ptr), "r"((int)ok));
+}
 
 template <int N, bool HERM>
 __global__ void __launch_bounds__(LargeCfg<N>::THREADS, 1)
@@ -164,6 +174,19 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
     if (warp == 0 && lane == 0) {
       if (next < nodes) lbulk_prefetch_l2(p.x + (size_t)next * NN, (unsigned)NN * 16);
       traw = atomicAdd(P.tickets, 1ULL);
+    }
+
+    if (HERM) {
+      // the NEXT node's dense link row -> L2; THIS node's neighbour rows (row b of sigma_{u +- e_l}, b the bath of
+      // mode l) -> L2 behind the contraction, so that the coupling phase pays L2 round trips only
+      if (warp == 2 && lane == 0 && next < nodes)
+        lbulk_prefetch_l2(P.mrows + (size_t)next * P.mrow, (unsigned)P.mrow * 4);
+      const int32_t* lr0 = P.mrows + (size_t)node * P.mrow;
+      for (int q = threadIdx.x; q < 2 * p.W; q += C::THREADS) {
+        const int idx = __ldg(lr0 + q);
+        const int l = q < p.W ? q : q - p.W;
+        if (idx >= 0) lbulk_prefetch_l2(p.x + (size_t)idx * NN + (size_t)(l / p.M) * N, (unsigned)N * 16);
+      }
     }
 
     // ---- C = (H/hbar) sigma - sigma (H/hbar) on the FP64 tensor cores (Eq. 12) --------------------
@@ -248,7 +271,65 @@ rhs_large_kernel(const __grid_constant__ LargeParams<N> P) {
 
     // ---- couplings to sigma_{u +- e_l}: row b and column b of the neighbour (Eq. 15-17, 23, 25, 35-36) --
     //      (HERM: the row part only, added to Z; Z^dagger supplies the column part)
-    {
+    if (HERM) {
+      // Row-wise: a lane owns rows b = i0w + 8 rg + rho; row b is touched by the links of the modes of bath b only
+      // (site map: bath b <-> state b), which it looks up in the node's dense link row and gathers all at once --
+      // 2 M CT independent 16-byte loads per row, predicated on the link's existence.  (Walking the node's link list
+      // instead made every warp step through ~W links one after the other: 5.2 of 28.0 ms per launch on config 5.)
+      const int32_t* lr = P.mrows + (size_t)node * P.mrow;
+      const int W = p.W, M = p.M;
+      for (int kk = 0; kk < M; ++kk) {
+        int up[RG], dn[RG], nn[RG];
+#pragma unroll
+        for (int rg = 0; rg < RG; ++rg) {
+          const int l = (i0w + 8 * rg + rho) * M + kk;
+          up[rg] = __ldg(lr + l); dn[rg] = __ldg(lr + W + l); nn[rg] = __ldg(lr + 2 * W + l);
+        }
+        // "+" links (one per row below the top level): two rows' loads in flight at a time
+#pragma unroll
+        for (int r2 = 0; r2 < RG; r2 += 2) {
+          double2 wu[2][CT];
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            if (r2 + h < RG) {
+              const int b = i0w + 8 * (r2 + h) + rho;
+              const double2* nu = p.x + (size_t)(up[r2 + h] < 0 ? 0 : up[r2 + h]) * NN + (size_t)b * N + j0w + t;
+#pragma unroll
+              for (int ct = 0; ct < CT; ++ct) { wu[h][ct] = make_double2(0.0, 0.0); ldg_if(wu[h][ct], nu + 4 * ct, up[r2 + h] >= 0); }
+            }
+          }
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            if (r2 + h < RG) {
+              const int rg = r2 + h;
+              const double a = sSqrt[nn[rg] + 1] * P.cP[(i0w + 8 * rg + rho) * M + kk];      // i a+
+#pragma unroll
+              for (int ct = 0; ct < CT; ++ct) {
+                acc[rg][ct].x = fma(-a, wu[h][ct].y, acc[rg][ct].x);
+                acc[rg][ct].y = fma(a, wu[h][ct].x, acc[rg][ct].y);
+              }
+            }
+          }
+        }
+        // "-" links exist only where n_l > 0 (at most D per node): skipped when no lane of the warp has one
+#pragma unroll
+        for (int rg = 0; rg < RG; ++rg) {
+          if (__any_sync(0xffffffffu, dn[rg] >= 0)) {
+            const int b = i0w + 8 * rg + rho, l = b * M + kk;
+            const double2* nd = p.x + (size_t)(dn[rg] < 0 ? 0 : dn[rg]) * NN + (size_t)b * N + j0w + t;
+            double2 wd[CT];
+#pragma unroll
+            for (int ct = 0; ct < CT; ++ct) { wd[ct] = make_double2(0.0, 0.0); ldg_if(wd[ct], nd + 4 * ct, dn[rg] >= 0); }
+            const double sn = sSqrt[nn[rg]], fx = sn * P.cX[l], fo = sn * P.cO[l];              // i a-x + a-o
+#pragma unroll
+            for (int ct = 0; ct < CT; ++ct) {
+              acc[rg][ct].x = fma(fo, wd[ct].x, fma(-fx, wd[ct].y, acc[rg][ct].x));
+              acc[rg][ct].y = fma(fo, wd[ct].y, fma(fx, wd[ct].x, acc[rg][ct].y));
+            }
+          }
+        }
+      }
+    } else {
       const int64_t e0 = P.lptr[node], e1 = P.lptr[node + 1];
       for (int64_t e = e0; e < e1; ++e) {
         const int4 ent = P.lent[e];
@@ -363,14 +444,15 @@ size_t large_smem() {
 }
 
 template <int N, bool HERM>
-cudaError_t launch_large_t(const RhsParams& p, const int64_t* lptr, const int4* lent, const double* Hs_dev,
+cudaError_t launch_large_t(const RhsParams& p, const int64_t* lptr, const int4* lent, const int32_t* mrows, int mrow,
+                           const double* Hs_dev,
                            const double* delta_dev, const double* a_plus, const double* a_minus_x,
                            const double* a_minus_o, int sms, unsigned long long* tickets,
                            unsigned long long* ticket_base, cudaStream_t s) {
   using C = LargeCfg<N>;
   if (p.W > kLargeMaxModes) return cudaErrorInvalidValue;
   LargeParams<N> P;
-  P.p = p; P.lptr = lptr; P.lent = lent; P.Hs = Hs_dev; P.delta = delta_dev;
+  P.p = p; P.lptr = lptr; P.lent = lent; P.mrows = mrows; P.mrow = mrow; P.Hs = Hs_dev; P.delta = delta_dev;
   const int D1 = p.D + 1;
   for (int l = 0; l < kLargeMaxModes; ++l) {
     const bool on = l < p.W && p.D >= 1;
@@ -407,16 +489,17 @@ cudaError_t launch_large_t(const RhsParams& p, const int64_t* lptr, const int4* 
 
 bool large_supported(int N, int W) { return (N == 32 || N == 64 || N == 96) && W <= kLargeMaxModes; }
 
-cudaError_t launch_rhs_large(const RhsParams& p, const int64_t* lptr, const void* lent, const double* Hs_dev,
+cudaError_t launch_rhs_large(const RhsParams& p, const int64_t* lptr, const void* lent, const int32_t* mrows, int mrow,
+                             const double* Hs_dev,
                              const double* delta_dev, const double* a_plus, const double* a_minus_x,
                              const double* a_minus_o, int hermitian, int sms, unsigned long long* tickets,
                              unsigned long long* ticket_base, cudaStream_t s) {
   const int4* le = reinterpret_cast<const int4*>(lent);
 #define HEOM_LARGE_CASE(n)                                                                                              \
   case n:                                                                                                               \
-    return hermitian ? launch_large_t<n, true>(p, lptr, le, Hs_dev, delta_dev, a_plus, a_minus_x, a_minus_o, sms,       \
+    return hermitian ? launch_large_t<n, true>(p, lptr, le, mrows, mrow, Hs_dev, delta_dev, a_plus, a_minus_x, a_minus_o, sms,       \
                                                tickets, ticket_base, s)                                                 \
-                     : launch_large_t<n, false>(p, lptr, le, Hs_dev, delta_dev, a_plus, a_minus_x, a_minus_o, sms,      \
+                     : launch_large_t<n, false>(p, lptr, le, mrows, mrow, Hs_dev, delta_dev, a_plus, a_minus_x, a_minus_o, sms,      \
                                                 tickets, ticket_base, s);
   switch (p.N) {
     HEOM_LARGE_CASE(32) HEOM_LARGE_CASE(64) HEOM_LARGE_CASE(96)
