@@ -97,6 +97,26 @@ def test_rhs_parity_hermitian_state(N, K, D, order):
     assert rel_err(g.rhs(), o.rhs()) < RHS_TOL
 
 
+@pytest.mark.parametrize("N,K,D", [(32, 1, 2), (32, 0, 3), (64, 0, 2), (96, 0, 1), (96, 1, 1)])
+def test_rhs_and_steps_hermitian_state_tensor_core(N, K, D):
+    """Dense HERMITIAN random state on the tensor-core kernel (N = 32, 64, 96): one product H sigma, row-wise gathers from
+    the dense link rows ("+" and "-" links of every mode, M = 1 and 2), Z + Z^dagger -- every term fires in every element.
+    RHS and three RK4 steps (Horner stages: epilogue from the fragment layout) against the oracle, exact Hermiticity."""
+    w = _small(N, K, D, T=77.0 if K >= 1 else 300.0, seed=5 * N + K + D)
+    o, g = _pair(w)
+    st = workloads.random_state(o.nodes, N, seed=41 + N, hermitian=True)
+    o.set_full_state(st); g.set_full_state(st)
+    assert g.kernel_name() == "rhs_large_herm_kernel"
+    ref, got = o.rhs(), g.rhs()
+    assert rel_err(got, ref) < RHS_TOL
+    assert np.array_equal(got, np.conj(np.swapaxes(got, 1, 2)))
+    o.rk4_steps(0.25, 3); g.rk4_steps(0.25, 3)
+    got = g.get_full_state()
+    assert rel_err(got, o.get_full_state()) < STATE_TOL
+    assert np.array_equal(got, np.conj(np.swapaxes(got, 1, 2)))
+    assert g.kernel_name() == "rhs_large_herm_kernel"
+
+
 @pytest.mark.parametrize("kernel", [1, 2])
 def test_dimer_1000_steps(kernel):
     """BASELINE config 1 in full: kernel = 1 propagates it in one launch of the tiny-hierarchy kernel, kernel = 2
