@@ -24,7 +24,10 @@
 //     as in kernels_hpipe.cu: only P1 = H sigma runs on the tensor cores (4 N^3 instead of 8 N^3 flop), only ROWS
 //     of the neighbours are gathered (contiguous), and Z is transposed through the sigma tile's shared memory
 //     once the contraction is done with it.  Element (j,i) is produced by exactly the conjugate operations of
-//     (i,j): the state stays bit-exactly Hermitian.
+//     (i,j): the state stays bit-exactly Hermitian.  The rows are gathered ROW-WISE: a lane looks the links of the
+//     rows it owns up in the node's dense link row {plus[W], minus[W], n[W]} (bath b <-> row b in these contexts) and
+//     issues their loads independently of one another; all neighbour rows of the node are bulk-prefetched into L2 at
+//     the top of the node, behind the contraction.  (General states walk the compact link list.)
 #include "kernels.cuh"
 
 #include <cmath>

@@ -156,3 +156,21 @@ def test_general_create_validation_without_gpu():
         g.set_option(name, good)
         with pytest.raises(HeomError):
             g.set_option(name, bad)
+
+
+def test_level_max_static_rejects_bad_arguments_without_a_gpu():
+    """heom_level_max_static checks its arguments before any CUDA call: depth beyond HEOM_STATIC_MAX_DEPTH, NULL
+    pointers and sizes out of range return HEOM_EINVAL with a message, with or without a device."""
+    import ctypes as C
+    from paper_1803_03498_b200 import STATIC_MAX_DEPTH
+    lib = load_library()
+    hdr = open(os.path.join(ROOT, "include", "heom.h")).read()
+    assert f"#define HEOM_STATIC_MAX_DEPTH {STATIC_MAX_DEPTH}" in hdr
+    fake = 0x1000                                   # never dereferenced: the call fails before touching memory
+    assert lib.heom_level_max_static(0, fake, fake, 3, 4, STATIC_MAX_DEPTH + 1, fake, None) == -1
+    assert b"outside 0..63" in lib.heom_static_last_error()
+    assert lib.heom_level_max_static(0, None, fake, 3, 4, 2, fake, None) == -1
+    assert b"NULL" in lib.heom_static_last_error()
+    assert lib.heom_level_max_static(0, fake, fake, -1, 4, 2, fake, None) == -1
+    assert lib.heom_level_max_static(-1, fake, fake, 3, 4, 2, fake, None) == -1
+    assert b"device" in lib.heom_static_last_error()
