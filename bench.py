@@ -47,15 +47,18 @@ def measured_peaks():
 
 def ncu_traffic(name, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch (average over the four stage launches of one RK4
-    step) from the committed `ncu --set full` captures, listed with their sources in profiles/traffic.json;
+    step) from the committed `ncu --set full` captures, listed with their sources in profiles/traffic.csv;
     None if the capture is of another kernel than the one this run used."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    import csv
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
-        with open(p) as f:
-            ent = json.load(f).get(name)
-        return (ent["bytes_per_launch"], ent["source"]) if ent and ent.get("kernel") == kernel else (None, None)
+        with open(p, newline="") as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == name and row["kernel"] == kernel:
+                    return int(row["bytes_per_launch"]), row["source"]
     except (OSError, ValueError, KeyError):
-        return None, None
+        pass
+    return None, None
 
 
 class ClockSampler:
