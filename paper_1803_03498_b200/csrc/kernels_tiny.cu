@@ -12,6 +12,7 @@ namespace {
 constexpr int kTinyThreads = 512;
 constexpr int kTinyMaxElems = 2048;    // nodes * N * N
 constexpr int kTinyMaxLinks = 4096;    // nodes * W
+constexpr int kTinyFastLinks = 16;     // links per matrix element the fast path keeps in registers: 4 M <= 16
 
 struct TinyParams {
   RhsParams p;          // tables as for the generic kernel; p.x = the state y (DEVICE), read and written
@@ -101,6 +102,101 @@ rk4_tiny_kernel(const TinyParams T) {
   };
 
   const double dt = T.dt;
+  if (total <= kTinyThreads && 4 * M <= kTinyFastLinks) {
+    // ---- fast path: one matrix element per thread for the whole propagation.  Everything that does not change from
+    //      stage to stage -- the element's indices, its damping rate, and for every link that touches it the
+    //      neighbour's element index and the complex factor (Eq. 35-36 with the signs of Eq. 23, 25) -- is worked
+    //      out ONCE into registers; a stage is then the commutator, one FMA pair per link and the RK4 update.
+    //      (The generic loop below redoes two integer divisions, the table walks and the validity branches per
+    //      element and stage: 1.5 us per stage on the dimer, against the few hundred cycles the arithmetic needs.)
+    const int e = threadIdx.x;
+    const bool on = e < total;
+    const int s = on ? e / NN : 0, q = on ? e - s * NN : 0, i = q / N, j = q - i * N;
+    const int sig = s * NN;
+    const double dd = sDamp[s] + sT[q];
+    int lidx[kTinyFastLinks];
+    double lre[kTinyFastLinks], lim[kTinyFastLinks];
+    int cnt = 0;
+    auto add = [&](int idx, double re, double im) {
+#pragma unroll
+      for (int t = 0; t < kTinyFastLinks; ++t)
+        if (t == cnt) { lidx[t] = idx; lre[t] = re; lim[t] = im; }
+      ++cnt;
+    };
+#pragma unroll
+    for (int t = 0; t < kTinyFastLinks; ++t) { lidx[t] = 0; lre[t] = 0.0; lim[t] = 0.0; }
+    if (on) {
+      const int32_t* pl = sPlus + s * W;
+      const int32_t* mi = sMinus + s * W;
+      const uint8_t* tu = sTup + s * W;
+      if (i != j) {
+        for (int side = 0; side < 2; ++side) {
+          const int b = side == 0 ? i : j;
+          const double sx = side == 0 ? 1.0 : -1.0;
+          for (int k = 0; k < M; ++k) {
+            const int l = b * M + k, n = tu[l];
+            if (pl[l] >= 0) add(pl[l] * NN + q, 0.0, sx * sAp[l * D1 + n]);                       // i a+
+            if (mi[l] >= 0) add(mi[l] * NN + q, sAo[l * D1 + n], sx * sAx[l * D1 + n]);           // a-o + i a-x
+          }
+        }
+      } else {
+        for (int k = 0; k < M; ++k) {                         // diagonal: V^x = 0, V^o = 2
+          const int l = i * M + k;
+          if (mi[l] >= 0) add(mi[l] * NN + q, 2.0 * sAo[l * D1 + tu[l]], 0.0);
+        }
+      }
+    }
+    auto rhs_fast = [&](const double2* x) -> double2 {
+      double cr = 0.0, ci = 0.0;                             // Eq. 12
+      for (int m = 0; m < N; ++m) {
+        const double him = sH[i * N + m], hmj = sH[m * N + j];
+        const double2 a = x[sig + m * N + j], b = x[sig + i * N + m];
+        cr = fma(him, a.x, cr); ci = fma(him, a.y, ci);
+        cr = fma(-hmj, b.x, cr); ci = fma(-hmj, b.y, ci);
+      }
+      double kr = ci * p.inv_hbar, ki = -cr * p.inv_hbar;
+      const double2 own = x[sig + q];
+      kr = fma(-dd, own.x, kr); ki = fma(-dd, own.y, ki);   // Eq. 13-14
+#pragma unroll
+      for (int t = 0; t < kTinyFastLinks; ++t) {
+        if (t < cnt) {                                       // Eq. 15-17
+          const double2 v = x[lidx[t]];
+          kr = fma(lre[t], v.x, fma(-lim[t], v.y, kr));
+          ki = fma(lre[t], v.y, fma(lim[t], v.x, ki));
+        }
+      }
+      return make_double2(kr, ki);
+    };
+    for (int step = 0; step < T.nsteps; ++step) {
+      double2 y = make_double2(0.0, 0.0), a = y;
+      if (on) {                                              // k1 = f(y)
+        const double2 k = rhs_fast(sY);
+        y = sY[e];
+        sXa[e] = make_double2(fma(dt / 2.0, k.x, y.x), fma(dt / 2.0, k.y, y.y));
+        a = make_double2(fma(dt / 6.0, k.x, y.x), fma(dt / 6.0, k.y, y.y));
+      }
+      __syncthreads();
+      if (on) {                                              // k2 = f(y + dt/2 k1)
+        const double2 k = rhs_fast(sXa);
+        sXb[e] = make_double2(fma(dt / 2.0, k.x, y.x), fma(dt / 2.0, k.y, y.y));
+        a = make_double2(fma(dt / 3.0, k.x, a.x), fma(dt / 3.0, k.y, a.y));
+      }
+      __syncthreads();
+      if (on) {                                              // k3 = f(y + dt/2 k2)
+        const double2 k = rhs_fast(sXb);
+        sXa[e] = make_double2(fma(dt, k.x, y.x), fma(dt, k.y, y.y));
+        a = make_double2(fma(dt / 3.0, k.x, a.x), fma(dt / 3.0, k.y, a.y));
+      }
+      __syncthreads();
+      if (on) {                                              // k4 = f(y + dt k3)
+        const double2 k = rhs_fast(sXa);
+        sY[e] = make_double2(fma(dt / 6.0, k.x, a.x), fma(dt / 6.0, k.y, a.y));
+      }
+      __syncthreads();
+    }
+    if (on) gy[e] = sY[e];
+    return;
+  }
   for (int step = 0; step < T.nsteps; ++step) {
     for (int e = threadIdx.x; e < total; e += kTinyThreads) {          // k1 = f(y)
       const double2 k = rhs(sY, e), y = sY[e];
