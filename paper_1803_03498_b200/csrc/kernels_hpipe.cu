@@ -60,7 +60,9 @@ struct PipeCfg {
   // (N = 14): 6 warps 2.556, 7 warps 2.425, 8 warps 2.338 ms per step; 10 warps (168 registers, spills) 3.07.
   // N <= 8: 12 warps of 168 registers; 16 warps of 128 registers with one mode index per gather batch: the same time.
   static constexpr int MAXW = (N <= 8) ? 12 : 8;
-  static constexpr int MAXW_GENERAL = (N <= 8) ? 8 : 6;   // general states need more registers per thread
+  // general states need more registers per thread (up to 251); N > 8, config 4 with hermitian=0: 6 warps 4.37, 7 warps 4.22,
+  // 8 warps 4.39 ms per step
+  static constexpr int MAXW_GENERAL = (N <= 8) ? 8 : 7;
   static constexpr int SMEM_BUDGET = 224 * 1024;
   static constexpr int KB = (16 / N) > 0 ? (16 / N) : 1;   // mode indices kk per gather batch (<= 32 loads)
   static constexpr int NP4 = (N + 3) / 4 * 4;         // ints per index group
