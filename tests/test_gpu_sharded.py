@@ -210,3 +210,55 @@ def test_partition_launch_cost_follows_owned_rows():
                     for wd, r, o, gh, t in out))
     for wd, r, o, gh, t in out:
         assert t < (1.0 / wd + 0.5 * gh / (o + gh) / wd + 0.12) * t_full
+
+
+def _nccl_worker(rank, world, port, halo, q):
+    """One rank of the multi-GPU parity run: its own GPU, NCCL, ShardedHeom against the oracle."""
+    import os
+    import torch
+    import torch.distributed as dist
+    from paper_1803_03498_b200.sharded import ShardedHeom
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", rank))
+    try:
+        w = workloads.fmo_like().with_(D=4)
+        sh = ShardedHeom(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D, rank, world, device=rank,
+                         halo=halo).bind()
+        sh.set_state(w.sigma0())
+        sh.rk4_steps(w.dt_fs, 60)
+        got = sh.gather_state(w.nodes)
+        pop, tr = sh.populations() if rank == 0 else (None, None)
+        if rank == 0:
+            o = Oracle(w.H_cm, w.lambda_cm, w.nu_per_fs, w.T_kelvin, w.K, w.D)
+            o.set_state(w.sigma0()); o.rk4_steps(w.dt_fs, 60)
+            q.put((float(rel_err(got, o.get_full_state())), float(abs(tr - 1.0))))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("halo", ["slices", "nodes"])
+def test_sharded_nccl_two_gpus(halo):
+    """ONE hierarchy over two GPUs through NCCL (one process per GPU): stage-wise stepping with the halo exchange
+    after every stage, final state of all ranks against the oracle.  Needs two GPUs: skipped on the one-GPU boxes
+    this repository has been measured on (the exchange logic is covered there by the one-GPU emulation above and
+    by the gloo world-size-2/3 tests of test_partition_host.py)."""
+    import socket
+    import torch
+    import torch.multiprocessing as mp
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_nccl_worker, args=(r, 2, port, halo, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    for p in procs:
+        p.join(600)
+        assert p.exitcode == 0
+    err, dtr = q.get(timeout=10)
+    assert err < STATE_TOL and dtr < 1e-11
